@@ -1,0 +1,56 @@
+"""The five BASELINE.json configs plus the tiny self-test config "T"."""
+from dataclasses import dataclass
+
+BASE_SEED = 220607660
+
+
+@dataclass(frozen=True)
+class GWConfig:
+    name: str
+    mesh: tuple          # (nk1, nk2, nk3), Γ-centred
+    nao: int             # N_orb
+    naux: int            # N_aux
+    ntau: int            # N_τ
+    nw: int              # N_ω (bosonic points used on this path)
+    beta: float          # inverse temperature, Ha^-1 (β=700)
+    elo: float           # Fock eigenvalue window [elo, ehi], μ = 0
+    ehi: float
+    gap: float           # gap at μ
+    seed: int
+    spin_deg: int = 2    # closed shell: Σ_σσ' of Eq. 28b
+
+    @property
+    def nk(self):
+        return self.mesh[0] * self.mesh[1] * self.mesh[2]
+
+    def bytes_V(self):
+        return self.nk ** 2 * self.naux * self.nao ** 2 * 16
+
+    def flops_nominal(self):
+        """Algorithm 1 taken literally, 8 flops per complex multiply-add."""
+        nk, nao, naux, nt, nw = self.nk, self.nao, self.naux, self.ntau, self.nw
+        per = 8.0 * (naux * naux * nao * nao + 2 * naux * nao ** 3)
+        s1 = nt * nk * nk * per
+        s3 = s1
+        tr = 2 * 8.0 * nw * nt * nk * naux * naux
+        sol = nw * nk * (28.0 / 3.0) * naux ** 3
+        s4 = nk * nk * 8.0 * 2 * naux * nao ** 3
+        return {"stage1": s1, "stage2_transforms": tr, "stage2_solve": sol,
+                "stage3": s3, "stage4": s4, "total": s1 + s3 + tr + sol + s4}
+
+
+CONFIGS = {
+    "0": GWConfig("cfg0", (1, 1, 1), 4, 16, 32, 32, 100.0, -1.0, 1.0, 0.0, BASE_SEED + 0),
+    "1": GWConfig("cfg1", (2, 2, 2), 26, 100, 104, 104, 700.0, -2.0, 3.0, 0.04, BASE_SEED + 1),
+    "2": GWConfig("cfg2", (4, 4, 4), 26, 200, 104, 104, 700.0, -2.0, 3.0, 0.04, BASE_SEED + 2),
+    "3": GWConfig("cfg3", (5, 5, 5), 26, 200, 104, 104, 700.0, -2.0, 3.0, 0.04, BASE_SEED + 3),
+    "4": GWConfig("cfg4", (4, 4, 4), 52, 400, 120, 120, 1000.0, -3.0, 5.0, 0.04, BASE_SEED + 4),
+    # tiny self-test config: odd and even mesh dims, -k != k, small beta so the grid is physically accurate
+    "T": GWConfig("cfgT", (3, 2, 1), 3, 5, 32, 32, 10.0, -1.0, 1.0, 0.0, BASE_SEED + 99),
+    # mid-size ragged config for parity tests: sizes that are not multiples of any tile
+    "R": GWConfig("cfgR", (3, 2, 2), 7, 37, 18, 18, 30.0, -1.5, 2.0, 0.04, BASE_SEED + 98),
+}
+
+
+def get_config(name) -> GWConfig:
+    return CONFIGS[str(name)]

@@ -1,0 +1,65 @@
+"""τ grid, bosonic Matsubara set and the transform matrices T_wt / T_tw (inputs of Eq. 28a / Eq. 30).
+
+The paper uses the IR basis with sparse sampling from IRBASIS and prints no formulas;
+irbasis / sparse_ir are not installed here.  BASELINE.json says "Chebyshev τ-nodes on [0,β]" and "transform
+matrices generated analytically from the grids".  Recipe = SURVEY.md §8c A7:
+
+  nodes     x_t = −cos(π(2t+1)/2N), τ_t = β(1+x_t)/2            (Chebyshev–Gauss roots, mirror symmetric)
+  bosonic   N non-negative indices: 0..⌊N/3⌋−1 dense, then geometrically spaced up to 4N
+  basis     even Chebyshev polynomials T_{2j}, j < N/2  (bosonic functions on this path are τ ↔ β−τ symmetric)
+  T_wt = Î·C          Î[a][j] = (β/2)∫ T_{2j}(x) cos(π n_a (x+1)) dx   (Gauss–Legendre), C = Chebyshev analysis
+  T_tw = T_even(x_t)ᵀ · pinv(Î)                                  (least squares)
+
+Both are real, stored as complex128.  These are *inputs*; kernels and oracle only apply them.
+"""
+import numpy as np
+
+
+def bosonic_set(N):
+    nd = N // 3
+    need = N - nd
+    sel = list(np.unique(np.round(np.geomspace(max(nd, 1), 4 * N, need)).astype(int)))
+    pool = [i for i in np.unique(np.round(np.geomspace(max(nd, 1), 4 * N, 40 * N)).astype(int))
+            if i not in sel and i >= nd]
+    while len(sel) < need:
+        sel.append(pool.pop(0))
+    S = sorted(set(list(range(nd)) + sorted(sel)[:need]))
+    extra = nd
+    while len(S) < N:            # top up with the smallest unused integers
+        if extra not in S:
+            S.append(extra)
+        extra += 1
+    return np.array(sorted(S), dtype=np.int64)
+
+
+def make_grids(ntau, nw, beta):
+    """Returns dict(tau[ntau], nbos[nw], T_wt[nw][ntau], T_tw[ntau][nw]) (complex128 matrices, zero imaginary part)."""
+    if nw != ntau:
+        raise ValueError("this recipe uses nw == ntau (PAPER.md:347: N_tau equals N_omega)")
+    N = ntau
+    t = np.arange(N)
+    half = -np.cos(np.pi * (2 * t[: (N + 1) // 2] + 1) / (2 * N))
+    x = np.empty(N)
+    x[: (N + 1) // 2] = half
+    x[N - 1 - np.arange(N // 2)] = -half[: N // 2]      # exact mirror symmetry: x[N-1-t] = -x[t]
+    if N % 2 == 1:
+        x[N // 2] = 0.0
+    tau = beta * (1.0 + x) / 2.0
+    tau[N - 1 - np.arange(N // 2)] = beta - tau[: N // 2]
+    S = bosonic_set(N)
+    L = N // 2
+    le = 2 * np.arange(L)
+    M = 2 * N + 2 * int(S.max()) + 300
+    xg, wg = np.polynomial.legendre.leggauss(M)
+    Tg = np.cos(np.outer(le, np.arccos(xg)))
+    Ie = np.array([(beta / 2) * (Tg * (wg * np.cos(np.pi * m * (xg + 1)))).sum(1) for m in S])
+    Tt = np.cos(np.outer(le, np.arccos(x)))
+    C = Tt * (2.0 / N)
+    C[0] *= 0.5
+    T_wt = Ie @ C
+    T_tw = Tt.T @ np.linalg.pinv(Ie)
+    cond = np.linalg.cond(Ie)
+    if not cond < 1e3:
+        raise RuntimeError(f"ill-conditioned sampling set: cond={cond:.3e}")
+    return {"tau": tau, "nbos": S, "T_wt": np.ascontiguousarray(T_wt.astype(np.complex128)),
+            "T_tw": np.ascontiguousarray(T_tw.astype(np.complex128)), "cond": cond}

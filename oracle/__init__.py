@@ -1,0 +1,171 @@
+"""ctypes front-end of the CPU oracle (oracle/gwref.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+It never imports the CUDA package and shares no code with it.  See gwref.c for the equations it follows
+(Eq. 22, 28a, 28b, 29, 30, 31; Algorithm 1) and tests/test_oracle_pins.py for what pins it.
+"""
+import ctypes
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libgwref.so")
+_lib = None
+
+
+def build(force=False):
+    """Compile gwref.c with gcc (-O2, OpenMP over the outermost independent loop only)."""
+    src = os.path.join(_HERE, "gwref.c")
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", _SO, src, "-lm"])
+    return _SO
+
+
+class Dims(ctypes.Structure):
+    _fields_ = [("nk1", ctypes.c_int32), ("nk2", ctypes.c_int32), ("nk3", ctypes.c_int32),
+                ("nao", ctypes.c_int32), ("naux", ctypes.c_int32), ("ntau", ctypes.c_int32),
+                ("nw", ctypes.c_int32), ("spin_deg", ctypes.c_int32), ("beta", ctypes.c_double)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_SO)
+        _lib.gwref_num_threads.restype = ctypes.c_int
+        for name in ("gwref_kadd", "gwref_ksub", "gwref_p0t_slice", "gwref_polarization", "gwref_dyson",
+                     "gwref_screened_interaction_q", "gwref_screened_interaction", "gwref_sigma_slice",
+                     "gwref_selfenergy", "gwref_exchange_slice", "gwref_exchange"):
+            getattr(_lib, name).restype = ctypes.c_int
+        _lib.gwref_transform.restype = None
+    return _lib
+
+
+def num_threads():
+    return int(lib().gwref_num_threads())
+
+
+def _dims(cfg):
+    return Dims(cfg.mesh[0], cfg.mesh[1], cfg.mesh[2], cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.spin_deg, cfg.beta)
+
+
+def _p(a):
+    assert a.dtype == np.complex128 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+class VBlocks:
+    """Table of nk*nk block pointers.  `blocks` is either the full array V[k1][k2][Q][i][j] or a dict
+    {(k1,k2): ndarray[naux][nao][nao]} holding only the resident blocks (big configs, sampled slices)."""
+
+    def __init__(self, cfg, blocks):
+        nk = cfg.nk
+        self.keep = blocks
+        self.table = (ctypes.c_void_p * (nk * nk))()
+        if isinstance(blocks, dict):
+            for (k1, k2), b in blocks.items():
+                assert b.shape == (cfg.naux, cfg.nao, cfg.nao)
+                self.table[k1 * nk + k2] = _p(b)
+        else:
+            assert blocks.shape == (nk, nk, cfg.naux, cfg.nao, cfg.nao)
+            base = blocks.ctypes.data
+            step = cfg.naux * cfg.nao * cfg.nao * 16
+            for i in range(nk * nk):
+                self.table[i] = base + i * step
+
+
+def kadd(cfg, k, q):
+    d = _dims(cfg)
+    return lib().gwref_kadd(ctypes.byref(d), int(k), int(q))
+
+
+def ksub(cfg, k, q):
+    d = _dims(cfg)
+    return lib().gwref_ksub(ctypes.byref(d), int(k), int(q))
+
+
+def p0t_slice(cfg, vb, G_t, G_tbar, q):
+    """Eq. 28b for one (q, tau_t).  G_t = G[t], G_tbar = G[ntau-1-t], each [nk][nao][nao]."""
+    out = np.empty((cfg.naux, cfg.naux), np.complex128)
+    d = _dims(cfg)
+    rc = lib().gwref_p0t_slice(ctypes.byref(d), vb.table, _p(G_t), _p(G_tbar), int(q), _p(out))
+    if rc:
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out
+
+
+def polarization(cfg, vb, G):
+    out = np.empty((cfg.ntau, cfg.nk, cfg.naux, cfg.naux), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_polarization(ctypes.byref(d), vb.table, _p(G), _p(out)):
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out
+
+
+def dyson(P):
+    """Eq. 29 for one matrix: (I - P)^-1 P."""
+    n = P.shape[0]
+    X = np.empty_like(P)
+    if lib().gwref_dyson(n, _p(np.ascontiguousarray(P)), _p(X)):
+        raise RuntimeError("oracle: zero pivot")
+    return X
+
+
+def screened_interaction_q(cfg, T_wt, T_tw, P0t_q, want_freq=False):
+    """Stage 2 for one q.  P0t_q: packed [ntau][naux][naux]."""
+    ps = cfg.naux * cfg.naux
+    Wt_q = np.empty((cfg.ntau, cfg.naux, cfg.naux), np.complex128)
+    P0w = np.empty((cfg.nw, cfg.naux, cfg.naux), np.complex128)
+    Ww = np.empty((cfg.nw, cfg.naux, cfg.naux), np.complex128)
+    d = _dims(cfg)
+    rc = lib().gwref_screened_interaction_q(ctypes.byref(d), _p(T_wt), _p(T_tw), _p(np.ascontiguousarray(P0t_q)),
+                                            ctypes.c_size_t(ps), _p(Wt_q), ctypes.c_size_t(ps), _p(P0w), _p(Ww))
+    if rc:
+        raise RuntimeError("oracle: zero pivot")
+    return (Wt_q, P0w, Ww) if want_freq else Wt_q
+
+
+def screened_interaction(cfg, T_wt, T_tw, P0t, want_freq=False):
+    Wt = np.empty_like(P0t)
+    P0w = np.empty((cfg.nw, cfg.nk, cfg.naux, cfg.naux), np.complex128) if want_freq else None
+    Ww = np.empty((cfg.nw, cfg.nk, cfg.naux, cfg.naux), np.complex128) if want_freq else None
+    d = _dims(cfg)
+    rc = lib().gwref_screened_interaction(ctypes.byref(d), _p(T_wt), _p(T_tw), _p(P0t), _p(Wt),
+                                          _p(P0w) if want_freq else None, _p(Ww) if want_freq else None)
+    if rc:
+        raise RuntimeError("oracle: zero pivot")
+    return (Wt, P0w, Ww) if want_freq else Wt
+
+
+def sigma_slice(cfg, vb, G_t, Wt_t, k):
+    """Eq. 31 for one (k, tau_t).  G_t: [nk][nao][nao], Wt_t: [nk][naux][naux]."""
+    out = np.empty((cfg.nao, cfg.nao), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_sigma_slice(ctypes.byref(d), vb.table, _p(G_t), _p(Wt_t), int(k), _p(out)):
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out
+
+
+def selfenergy(cfg, vb, G, Wt):
+    out = np.empty((cfg.ntau, cfg.nk, cfg.nao, cfg.nao), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_selfenergy(ctypes.byref(d), vb.table, _p(G), _p(Wt), _p(out)):
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out
+
+
+def exchange_slice(cfg, vb, gamma, k):
+    out = np.empty((cfg.nao, cfg.nao), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_exchange_slice(ctypes.byref(d), vb.table, _p(gamma), int(k), _p(out)):
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out
+
+
+def exchange(cfg, vb, gamma):
+    out = np.empty((cfg.nk, cfg.nao, cfg.nao), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_exchange(ctypes.byref(d), vb.table, _p(gamma), _p(out)):
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out

@@ -1,0 +1,297 @@
+"""Pins of the CPU oracle against things that are NOT the oracle.
+
+Each test is chosen so that a plausible mistake in oracle/gwref.c (dropped term, wrong sign, wrong index,
+transposed operand, wrong k±q table, wrong normalisation) fails at least one of them.
+"""
+import numpy as np
+import pytest
+
+import gwgen
+from gwgen.configs import GWConfig
+from gwgen.fock import fermi
+
+
+def relerr(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P1: scalar closed form (north_star: "closed form for nk=1, nao=1, naux=1").
+#   G(tau) = -e^{-eps tau}/(1+e^{-beta eps}); V = v real.  G(tau) G(beta-tau) = f(1-f) is tau independent, so
+#   P0t = -s v^2 f(1-f);  P0w = p delta_{n0}, p = -s v^2 beta f(1-f);  Ww = p/(1-p) delta_{n0};
+#   Wt = p/(beta(1-p));  Sigma(tau) = -v^2 G(tau) p/(beta(1-p));  K = -v^2 f.       (Eq. 22, 28-31 with 1x1 matrices)
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("s", [1, 2])
+@pytest.mark.parametrize("eps,v,beta", [(0.37, 0.8, 10.0), (-0.11, 1.3, 25.0)])
+def test_P1_scalar_closed_form(oracle_lib, s, eps, v, beta):
+    N = 32
+    cfg = GWConfig("P1", (1, 1, 1), 1, 1, N, N, beta, -1, 1, 0.0, 1, spin_deg=s)
+    gr = gwgen.make_grids(N, N, beta)
+    tau = gr["tau"]
+    f = 1.0 / (1.0 + np.exp(beta * eps))
+    g = -np.exp(-eps * tau) / (1.0 + np.exp(-beta * eps))
+    G = g.reshape(N, 1, 1, 1).astype(np.complex128)
+    V = np.full((1, 1, 1, 1, 1), v, np.complex128)
+    vb = oracle_lib.VBlocks(cfg, V)
+    P0t = oracle_lib.polarization(cfg, vb, G)
+    assert np.allclose(P0t.ravel(), -s * v * v * f * (1 - f), rtol=1e-13, atol=0)
+    Wt, P0w, Ww = oracle_lib.screened_interaction(cfg, gr["T_wt"], gr["T_tw"], P0t, want_freq=True)
+    p = -s * v * v * beta * f * (1 - f)
+    expect_w = np.where(gr["nbos"] == 0, p, 0.0)
+    assert np.max(np.abs(P0w.ravel() - expect_w)) < 1e-11 * abs(p)
+    assert np.max(np.abs(Ww.ravel() - np.where(gr["nbos"] == 0, p / (1 - p), 0.0))) < 1e-11 * max(1.0, abs(p))
+    assert np.max(np.abs(Wt.ravel() - p / (beta * (1 - p)))) < 1e-10 * abs(p / (beta * (1 - p)))
+    Sg = oracle_lib.selfenergy(cfg, vb, G, Wt)
+    assert relerr(Sg.ravel(), -v * v * g * p / (beta * (1 - p))) < 1e-10
+    K = oracle_lib.exchange(cfg, vb, np.full((1, 1, 1), f, np.complex128))
+    assert abs(K.ravel()[0] - (-v * v * f)) < 1e-14
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P2: Lindhard closed form for a Fock-built G (textbook non-interacting polarisation in the eigenbasis):
+#   Vt^Q = U_k^+ V^Q(k,k+q) U_{k+q}
+#   P0(q,tau)  = -(s/Nk) sum_k sum_ca Vt^Q_ca conj(Vt^Q'_ca) f_c (1-f_a) e^{-(e_a-e_c) tau}
+#   P0(q,iOm)  = -(s/Nk) sum_k sum_ca Vt^Q_ca conj(Vt^Q'_ca) (f_c-f_a)/(e_a-e_c-iOm)      (beta f_c(1-f_a) at n=0 if e_a=e_c)
+# A different contraction order in a different basis; uses the generator's eps, U, and mesh tables (not the oracle's).
+# ----------------------------------------------------------------------------------------------------------------
+def lindhard_tau(p, q, t):
+    cfg, mesh = p.cfg, p.mesh
+    add = mesh.add_table()
+    V = p.V.numpy()
+    beta = cfg.beta
+    out = np.zeros((cfg.naux, cfg.naux), complex)
+    logf = lambda e: -np.logaddexp(0.0, beta * e)
+    for k in range(cfg.nk):
+        kq = add[k][q]
+        Vt = np.einsum("dc,Qda,ab->Qcb", p.U[k].conj(), V[k, kq], p.U[kq])
+        de = p.eps[kq][None, :] - p.eps[k][:, None]                       # [c][a]
+        w = np.exp(logf(p.eps[k])[:, None] + logf(-p.eps[kq])[None, :] - de * p.tau[t])
+        out += np.einsum("Qca,ca,Pca->QP", Vt, w, Vt.conj())
+    return -cfg.spin_deg / cfg.nk * out
+
+
+def lindhard_omega(p, q, ns):
+    cfg, mesh = p.cfg, p.mesh
+    add = mesh.add_table()
+    V = p.V.numpy()
+    beta = cfg.beta
+    ns = np.asarray(ns)
+    Om = 2 * np.pi * ns / beta
+    out = np.zeros((len(ns), cfg.naux, cfg.naux), complex)
+    f = fermi(p.eps, beta)
+    for k in range(cfg.nk):
+        kq = add[k][q]
+        Vt = np.einsum("dc,Qda,ab->Qcb", p.U[k].conj(), V[k, kq], p.U[kq]).reshape(cfg.naux, -1)
+        de = (p.eps[kq][None, :] - p.eps[k][:, None]).ravel()
+        df = (f[k][:, None] - f[kq][None, :]).ravel()
+        deg = np.abs(de) < 1e-13
+        w = np.where(deg[None, :], 0.0, df[None, :] / (np.where(deg, 1.0, de)[None, :] - 1j * Om[:, None]))
+        wdeg = (beta * f[k][:, None] * (1 - f[kq][None, :])).ravel()
+        w = w + np.where(deg[None, :] & (ns[:, None] == 0), wdeg[None, :], 0.0)
+        M = (Vt[:, None, :] * Vt.conj()[None, :, :]).reshape(cfg.naux * cfg.naux, -1)   # [(QP)][(ca)]
+        out += (w @ M.T).reshape(len(ns), cfg.naux, cfg.naux)
+    return -cfg.spin_deg / cfg.nk * out
+
+
+@pytest.mark.parametrize("name", ["T", "R", "0"])
+def test_P2_lindhard_tau(problems, oracle_results, name):
+    p = problems(name)
+    P0t = oracle_results(name)["P0t"]
+    rng = np.random.default_rng(5)
+    for _ in range(6):
+        q = int(rng.integers(p.cfg.nk)); t = int(rng.integers(p.cfg.ntau))
+        assert relerr(P0t[t, q], lindhard_tau(p, q, t)) < 1e-12
+
+
+def test_P2_lindhard_omega(problems, oracle_results):
+    # stage 2a to the accuracy of the grid: beta=10, N=32 gives ~1e-12
+    p = problems("T")
+    P0w = oracle_results("T")["P0w"]
+    for q in range(p.cfg.nk):
+        assert relerr(P0w[:, q], lindhard_omega(p, q, p.nbos)) < 1e-10
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P3: definiteness / Hermiticity end to end (sign reading R1 of DESIGN.md): P0t <= 0 Hermitian, I - P0w HPD with
+# eigenvalues >= 1 (what the paper's *Cholesky* solver needs), Ww in (-1,0], -Sigma >= 0, -K >= 0.
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["T", "R"])
+def test_P3_definiteness(problems, oracle_results, name):
+    cfg = problems(name).cfg
+    r = oracle_results(name)
+    herm = lambda A: np.abs(A - np.conj(np.swapaxes(A, -1, -2))).max() / np.abs(A).max()
+    for key in ("P0t", "P0w", "Ww", "Wt", "Sigma", "K"):
+        assert herm(r[key]) < 1e-12, key
+    tol = 1e-12
+    assert max(np.linalg.eigvalsh(r["P0t"][t, q]).max() for t in range(cfg.ntau) for q in range(cfg.nk)) < tol
+    I = np.eye(cfg.naux)
+    assert min(np.linalg.eigvalsh(I - r["P0w"][n, q]).min() for n in range(cfg.nw) for q in range(cfg.nk)) > 1 - 1e-9
+    ev = np.array([np.linalg.eigvalsh(r["Ww"][n, q]) for n in range(cfg.nw) for q in range(cfg.nk)])
+    assert ev.max() < 1e-9 and ev.min() > -1.0
+    assert max(np.linalg.eigvalsh(r["Sigma"][t, k]).max() for t in range(cfg.ntau) for k in range(cfg.nk)) < tol
+    assert max(np.linalg.eigvalsh(r["K"][k]).max() for k in range(cfg.nk)) < tol
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P4: P0^{-q}_{Q'Q}(tau_t) = P0^{q}_{QQ'}(tau_{tbar}) (always); P0^q(tau_tbar) = P0^q(tau_t) under TR inputs.
+# P5: north_star's checks: Sigma_ij(k,tau) = conj Sigma_ji(k,tau); Sigma(-k) = Sigma(k)^*.
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["T", "R"])
+def test_P4_P5_symmetries(problems, oracle_results, name):
+    p = problems(name)
+    r = oracle_results(name)
+    neg = p.mesh.neg()
+    P0t, Sg, K = r["P0t"], r["Sigma"], r["K"]
+    assert relerr(np.swapaxes(P0t[:, neg], -1, -2), P0t[::-1]) < 1e-13
+    assert relerr(P0t[::-1], P0t) < 1e-13
+    assert relerr(np.conj(np.swapaxes(Sg, -1, -2)), Sg) < 1e-13
+    assert relerr(Sg[:, neg], np.conj(Sg)) < 1e-13
+    assert relerr(K[neg], np.conj(K)) < 1e-13
+
+
+def test_P4_mesh_tables_match_generator(problems, oracle_lib):
+    # the oracle has its own k±q arithmetic; the generator another; they must agree (3x2x2 mesh: odd and even dims)
+    p = problems("R")
+    add, sub = p.mesh.add_table(), p.mesh.sub_table()
+    for k in range(p.cfg.nk):
+        for q in range(p.cfg.nk):
+            assert oracle_lib.kadd(p.cfg, k, q) == add[k][q]
+            assert oracle_lib.ksub(p.cfg, k, q) == sub[k][q]
+    assert add[sub[5][3]][3] == 5
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P6: brute force on the tiny config T: exact P0(iOm_n) (Lindhard) for |n| <= 4e5 -> Dyson per n -> explicit
+# Matsubara sum Wt(tau_t) = (1/beta) sum_n W(iOm_n) e^{-iOm_n tau_t} (Eq. 29, 30) -> compared with the oracle's
+# sparse-grid pipeline (Eq. 28a matrix, LU, Eq. 30 matrix).  Pins the transform pair and Dyson as physics.
+# ----------------------------------------------------------------------------------------------------------------
+def test_P6_bruteforce_matsubara(problems, oracle_results):
+    p = problems("T")
+    cfg = p.cfg
+    Wt = oracle_results("T")["Wt"]
+    nb, chunk = 400000, 50000
+    I = np.eye(cfg.naux)
+    ref = np.zeros_like(Wt)
+    for q in range(cfg.nk):
+        acc = np.zeros((cfg.ntau, cfg.naux, cfg.naux), complex)
+        for lo in range(-nb, nb + 1, chunk):
+            nn = np.arange(lo, min(lo + chunk, nb + 1))
+            Pn = lindhard_omega(p, q, nn)
+            Wn = np.linalg.solve(I[None] - Pn, Pn)
+            ph = np.exp(-1j * np.outer(p.tau, 2 * np.pi * nn / cfg.beta))
+            acc += np.tensordot(ph, Wn, axes=(1, 0))
+        ref[:, q] = acc / cfg.beta
+    assert relerr(Wt, ref) < 1e-8
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P7: trace identity tying stage 3 to stage 1 (exact at every tau node, for arbitrary Wt):
+#   sum_k tr[Sigma[t][k] G[tbar][k]] = (1/s) sum_q tr[Wt[t][q] P0t[tbar][q]]
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["T", "R", "0"])
+def test_P7_trace_identity(problems, oracle_results, oracle_lib, name):
+    p = problems(name)
+    cfg = p.cfg
+    r = oracle_results(name)
+    rng = np.random.default_rng(11)
+    # arbitrary (non-physical, non-Hermitian) W to make the identity bite on index order
+    Wr = rng.normal(size=r["Wt"].shape) + 1j * rng.normal(size=r["Wt"].shape)
+    vb = oracle_lib.VBlocks(cfg, p.V.numpy())
+    for W, Sg in ((r["Wt"], r["Sigma"]), (Wr, oracle_lib.selfenergy(cfg, vb, p.G, Wr))):
+        lhs = np.einsum("tkij,tkji->t", Sg, p.G[::-1])
+        rhs = np.einsum("tqab,tqba->t", W, r["P0t"][::-1]) / cfg.spin_deg
+        assert np.max(np.abs(lhs - rhs) / np.abs(rhs)) < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P8: residual of the solve, independent of the oracle's LU: (I - P0w) Ww = P0w and Ww = (I - P0w)^-1 - I (Eq. 29)
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["T", "R"])
+def test_P8_dyson_residual(problems, oracle_results, name):
+    cfg = problems(name).cfg
+    r = oracle_results(name)
+    I = np.eye(cfg.naux)
+    for n in range(cfg.nw):
+        for q in range(cfg.nk):
+            P, W = r["P0w"][n, q], r["Ww"][n, q]
+            assert np.linalg.norm((I - P) @ W - P) <= 1e-13 * max(np.linalg.norm(P), 1e-300) + 1e-300
+            assert relerr(W, np.linalg.inv(I - P) - I) < 1e-10 or np.linalg.norm(W) < 1e-12
+
+
+def test_P8_dyson_nonhermitian_pivoting(oracle_lib):
+    # generic complex matrix that needs row exchanges
+    rng = np.random.default_rng(3)
+    P = rng.normal(size=(9, 9)) + 1j * rng.normal(size=(9, 9))
+    P[0, 0] = 1.0   # makes (I-P)[0,0] exactly zero -> first pivot must be exchanged
+    X = oracle_lib.dyson(P)
+    assert relerr(X, np.linalg.solve(np.eye(9) - P, P)) < 1e-12
+
+
+def test_transform_matches_definition(problems, oracle_results):
+    # Eq. 28a / Eq. 30 as matrix applications (numpy tensordot = re-statement with a library routine on the same matrices)
+    p = problems("R")
+    r = oracle_results("R")
+    assert relerr(r["P0w"], np.tensordot(p.T_wt, r["P0t"], axes=(1, 0))) < 1e-13
+    assert relerr(r["Wt"], np.tensordot(p.T_tw, r["Ww"], axes=(1, 0))) < 1e-13
+
+
+def test_transform_rows_integrate_constants(problems):
+    # normalisation of Eq. 28a: sum_t T_wt[n][t] = beta delta_{n0}; Eq. 30 maps a constant in Omega_0 to 1/beta
+    for name in ("0", "T", "1"):
+        cfg = gwgen.get_config(name)
+        gr = gwgen.make_grids(cfg.ntau, cfg.nw, cfg.beta)
+        rs = gr["T_wt"].sum(axis=1)
+        assert abs(rs[0] - cfg.beta) < 1e-12 * cfg.beta
+        assert np.abs(rs[1:]).max() < 1e-11 * cfg.beta
+        assert np.allclose(gr["tau"][::-1], cfg.beta - gr["tau"], rtol=0, atol=4e-16 * cfg.beta)
+        e0 = np.zeros(cfg.nw); e0[0] = 1.0
+        assert np.abs(gr["T_tw"] @ e0 - 1.0 / cfg.beta).max() < 1e-11 / cfg.beta
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P9: exchange limit cross-checks two entry points: Eq. 31 with G := -gamma and W := I equals -K of Eq. 22.
+# ----------------------------------------------------------------------------------------------------------------
+def test_P9_exchange_limit(problems, oracle_results, oracle_lib):
+    p = problems("R")
+    cfg = p.cfg
+    vb = oracle_lib.VBlocks(cfg, p.V.numpy())
+    I = np.ascontiguousarray(np.broadcast_to(np.eye(cfg.naux, dtype=complex), (cfg.nk, cfg.naux, cfg.naux)))
+    for k in (0, 3, cfg.nk - 1):
+        S = oracle_lib.sigma_slice(cfg, vb, np.ascontiguousarray(-p.gamma), I, k)
+        assert relerr(S, -oracle_results("R")["K"][k]) < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P10: literal 4-index evaluation of Eq. 28b / 31 / 22 (no temporaries) with numpy einsum, using the generator's tables.
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["T", "0"])
+def test_P10_literal_einsum(problems, oracle_results, name):
+    p = problems(name)
+    cfg = p.cfg
+    r = oracle_results(name)
+    V = p.V.numpy()
+    add, sub = p.mesh.add_table(), p.mesh.sub_table()
+    N, nk = cfg.ntau, cfg.nk
+    S = np.zeros_like(r["Sigma"]); K = np.zeros_like(r["K"])
+    for t in range(N):
+        for k in range(nk):
+            for q in range(nk):
+                km = sub[k][q]
+                S[t, k] += np.einsum("ab,Qia,QP,Pbj->ij", p.G[t, km], V[k, km], r["Wt"][t, q], V[km, k])
+    S *= -1.0 / nk
+    for k in range(nk):
+        for kp in range(nk):
+            K[k] += np.einsum("Qia,ab,Qbj->ij", V[k, kp], p.gamma[kp], V[kp, k])
+    K *= -1.0 / nk
+    assert relerr(r["Sigma"], S) < 1e-13
+    assert relerr(r["K"], K) < 1e-13
+    # Eq. 28b, reading R1 of DESIGN.md: the printed "-1/Nk" is the antiperiodicity sign of G(-tau) = -G(beta-tau),
+    # so the array contracted is G[tbar] and P0t = -(s/Nk) sum_k V G^k[tbar] G^{k+q}[t] V  (index pattern exactly as printed).
+    lit = np.zeros_like(r["P0t"])
+    for t in range(N):
+        for q in range(nk):
+            for k in range(nk):
+                kq = add[k][q]
+                lit[t, q] += np.einsum("Qda,cd,ab,Pbc->QP", V[k, kq], p.G[N - 1 - t, k], p.G[t, kq], V[kq, k])
+    lit *= -cfg.spin_deg / nk
+    assert relerr(r["P0t"], lit) < 1e-13
