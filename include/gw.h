@@ -1,0 +1,121 @@
+/*
+ * gw.h — C ABI of libgw_b200: one scGW iteration's self-energy build on one B200 (sm_100a).
+ *
+ * Method: "Fully self-consistent finite-temperature GW in Gaussian Bloch orbitals for solids",
+ * arXiv 2206.07660.  The four calls follow Algorithm 1 and the static
+ * exchange of Eq. 22; citations per function below.  All arithmetic is complex FP64.
+ *
+ * Conventions
+ *   - gw_c128 is layout-compatible with C99 `double complex`, std::complex<double>, cuDoubleComplex,
+ *     torch.complex128.  All arrays are dense, row-major, 16-byte aligned.
+ *   - "device" pointers are CUDA global memory of the current device; the caller owns every buffer,
+ *     the library allocates nothing on the four hot calls, keeps no state between calls and never
+ *     frees caller memory.  Inputs are const and unmodified; outputs are fully overwritten.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  The calls only
+ *     enqueue work; they never synchronise the host.
+ *   - k-mesh: Γ-centred nk1 x nk2 x nk3, nk = nk1*nk2*nk3, k = (i1*nk2+i2)*nk3+i3,
+ *     k±q and −k component-wise modulo (momentum conservation).
+ *   - q sharding ("first layer of parallelization"): a call works on the q-points
+ *     q_begin <= q < q_end only; nq = q_end - q_begin.  P0t / Wt hold nq q-points (index q - q_begin);
+ *     Sigma / K then hold this shard's partial sums, to be summed over shards by the caller
+ *     (one all-reduce).  q_begin = 0, q_end = nk is the single-GPU case.
+ *   - Preconditions (documented, not "fixed" silently): the τ grid is mirror symmetric,
+ *     τ[ntau-1-t] = β − τ[t], so that G(−τ_t) = −G(β−τ_t) = −G[ntau-1-t] (Eq. 28b);
+ *     I − P̃0(q,iΩ) is Hermitian positive definite (true for time-reversal symmetric inputs; the paper
+ *     solves Eq. 29 with a Cholesky solver).  A non-positive pivot is reported through
+ *     `info`, never by abort.
+ *   - Return value: 0 = GW_OK; negative = caller error (GW_E*); positive = cudaError_t of a failed
+ *     launch.  No C++ exception crosses this boundary.
+ */
+#ifndef GW_B200_H
+#define GW_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { double re, im; } gw_c128;
+
+enum {
+  GW_OK = 0,
+  GW_EINVAL = -1,   /* null / misaligned pointer, non-positive size, bad q range */
+  GW_ENOMEM = -2,   /* workspace too small */
+  GW_EARCH = -3,    /* current device is not sm_100 */
+  GW_ESHAPE = -4    /* size outside what the kernels support (nao > 64, ntau or nw > 128) */
+};
+
+typedef struct {
+  int32_t nk1, nk2, nk3;   /* k-mesh */
+  int32_t nao;             /* N_orb */
+  int32_t naux;            /* N_aux */
+  int32_t ntau;            /* N_tau */
+  int32_t nw;              /* N_omega: bosonic Matsubara sampling points */
+  int32_t spin_deg;        /* s of the spin sum in Eq. 28b: 2 = closed shell, 1 = one spin channel */
+  int32_t q_begin, q_end;  /* q shard [q_begin, q_end) */
+  double beta;             /* inverse temperature (informational; the grids enter through T_wt/T_tw) */
+  const gw_c128 *V;        /* device [nk][nk][naux][nao][nao]: V^{k1 k2}_{ij}(Q), Eq. 6-7 */
+  const gw_c128 *T_wt;     /* device [nw][ntau]: bosonic τ→iΩ transform matrix, Eq. 28a */
+  const gw_c128 *T_tw;     /* device [ntau][nw]: bosonic iΩ→τ transform matrix, Eq. 30 */
+} gw_problem;
+
+/* Stage 1 — Eq. 28b, Algorithm 1 first k loop:
+ *   P0t[t][q-q_begin][Q][Q'] = -(s/N_k) Σ_k Σ_abcd V[k][k+q][Q][d][a] G[t][k+q][a][b] V[k+q][k][Q'][b][c] G[ntau-1-t][k][c][d]
+ * (the printed "-1/N_k" is the antiperiodicity sign of G(−τ); reading R1).
+ *   G   : device [ntau][nk][nao][nao]      in
+ *   P0t : device [ntau][nq][naux][naux]    out */
+int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P0t, void *stream);
+
+/* Stage 2 — Eq. 28a, 29, 30, Algorithm 1 middle part, for every q of the shard:
+ *   P0w[n] = Σ_t T_wt[n][t] P0t[t];   Ww[n] = (I − P0w[n])^-1 P0w[n]  (Cholesky);   Wt[t] = Σ_n T_tw[t][n] Ww[n]
+ *   P0t : device [ntau][nq][naux][naux]    in
+ *   Wt  : device [ntau][nq][naux][naux]    out; may alias P0t (then P0t is overwritten)
+ *   work: device scratch of at least gw_workspace_bytes(p) bytes, 256-byte aligned
+ *   info: device int32[2] or NULL.  Set to {-1,-1} on success, else {q, n} of one failing factorisation. */
+int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, void *work, size_t work_bytes,
+                            int32_t *info, void *stream);
+
+/* Stage 3 — Eq. 31, Algorithm 1 second k loop:
+ *   Sigma[t][k][i][j] = -(1/N_k) Σ_{q in shard} Σ_QQ' Σ_ab V[k][k-q][Q][i][a] G[t][k-q][a][b] Wt[t][q-q_begin][Q][Q'] V[k-q][k][Q'][b][j]
+ *   G     : device [ntau][nk][nao][nao]    in
+ *   Wt    : device [ntau][nq][naux][naux]  in
+ *   Sigma : device [ntau][nk][nao][nao]    out */
+int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c128 *Sigma, void *stream);
+
+/* Stage 4 — static exchange, Eq. 22:
+ *   K[k][i][j] = -(1/N_k) Σ_{q in shard, k'=k-q} Σ_Q Σ_ab V[k][k'][Q][i][a] gamma[k'][a][b] V[k'][k][Q][b][j]
+ *   gamma : device [nk][nao][nao]  in (density matrix γ^k = −G^k(β⁻))
+ *   K     : device [nk][nao][nao]  out */
+int gw_exchange(const gw_problem *p, const gw_c128 *gamma, gw_c128 *K, void *stream);
+
+/* Scratch needed by gw_screened_interaction for this problem (bytes; host-side arithmetic only). */
+size_t gw_workspace_bytes(const gw_problem *p);
+
+/* Whole iteration with HOST buffers (the end-to-end path timed as `e2e` by bench.py): uploads V, G, gamma,
+ * T_wt, T_tw, runs the four stages above on `stream`, downloads Sigma and K, and synchronises the stream.
+ * All pointers here (including p->V, p->T_wt, p->T_tw) are HOST memory (pinned memory makes the copies
+ * asynchronous).  Device memory is allocated and freed inside the call.  Optional outputs may be NULL:
+ *   P0t_out, Wt_out : host [ntau][nq][naux][naux];  stage_ms: host float[6] = H2D, stage 1..4, D2H times (ms). */
+int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, const gw_c128 *gamma, gw_c128 *Sigma, gw_c128 *K,
+                            gw_c128 *P0t_out, gw_c128 *Wt_out, float *stage_ms, void *stream);
+
+/* Executed FP64 flops of the last configuration of each stage kernel for `p` (what the kernels actually
+ * issue, padding and recomputation included; 2 flops per real FMA).  out: host double[4] = stage 1..4. */
+int gw_executed_flops(const gw_problem *p, double *out);
+
+/* Number of kernels the four hot calls launch for `p` (host arithmetic; used for bench.py's gpu_launches). */
+int gw_launch_count(const gw_problem *p);
+
+/* Register-resident DMMA.8x8x4 loop on all SMs for about `ms` milliseconds; returns sustained FP64 TFLOP/s
+ * in *tflops (the "measured FP64 peak" the roofline divides by; MEASURED_PEAKS.json has no FP64 entry). */
+int gw_fp64_peak(double ms, double *tflops, void *stream);
+
+const char *gw_strerror(int code);
+int gw_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GW_B200_H */

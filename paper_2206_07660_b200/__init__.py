@@ -1,0 +1,16 @@
+"""paper_2206_07660_b200 — thin Python binding of libgw_b200 (include/gw.h).
+
+Argument marshalling only: every step of the hot path (Eq. 22, 28a, 28b, 29, 30, 31; Algorithm 1)
+runs in the CUDA kernels under csrc/.  PyTorch is used for device memory and streams, nothing else.
+There is no CPU fallback: if the shared library is missing or the device is not sm_100 the calls raise.
+"""
+import ctypes
+import os
+
+from .binding import (GWProblem, GWError, lib, lib_path, gw_polarization, gw_screened_interaction, gw_selfenergy,
+                      gw_exchange, gw_workspace_bytes, gw_sigma_iteration, gw_sigma_iteration_host,
+                      gw_executed_flops, gw_launch_count, gw_fp64_peak, gw_strerror, gw_version, debug_set_naive)
+
+__all__ = ["GWProblem", "GWError", "lib", "lib_path", "gw_polarization", "gw_screened_interaction", "gw_selfenergy",
+           "gw_exchange", "gw_workspace_bytes", "gw_sigma_iteration", "gw_sigma_iteration_host", "gw_executed_flops",
+           "gw_launch_count", "gw_fp64_peak", "gw_strerror", "gw_version", "debug_set_naive"]

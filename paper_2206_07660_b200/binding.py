@@ -1,0 +1,220 @@
+"""ctypes marshalling for include/gw.h.  Same names as the C ABI."""
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libgw_b200.so")
+_lib = None
+
+
+class GWError(RuntimeError):
+    pass
+
+
+class _CProblem(ctypes.Structure):
+    _fields_ = [("nk1", ctypes.c_int32), ("nk2", ctypes.c_int32), ("nk3", ctypes.c_int32),
+                ("nao", ctypes.c_int32), ("naux", ctypes.c_int32), ("ntau", ctypes.c_int32), ("nw", ctypes.c_int32),
+                ("spin_deg", ctypes.c_int32), ("q_begin", ctypes.c_int32), ("q_end", ctypes.c_int32),
+                ("beta", ctypes.c_double),
+                ("V", ctypes.c_void_p), ("T_wt", ctypes.c_void_p), ("T_tw", ctypes.c_void_p)]
+
+
+def lib_path():
+    return _SO
+
+
+def lib():
+    """Load libgw_b200.so; fails loudly if it has not been built (python -m paper_2206_07660_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise GWError(f"{_SO} is missing: build it with `python paper_2206_07660_b200/build.py` "
+                          "(there is no CPU fallback)")
+        L = ctypes.CDLL(_SO)
+        P = ctypes.POINTER(_CProblem)
+        vp, sz = ctypes.c_void_p, ctypes.c_size_t
+        L.gw_polarization.argtypes = [P, vp, vp, vp]
+        L.gw_screened_interaction.argtypes = [P, vp, vp, vp, sz, vp, vp]
+        L.gw_selfenergy.argtypes = [P, vp, vp, vp, vp]
+        L.gw_exchange.argtypes = [P, vp, vp, vp]
+        L.gw_workspace_bytes.argtypes = [P]
+        L.gw_workspace_bytes.restype = sz
+        L.gw_sigma_iteration_host.argtypes = [P, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.gw_executed_flops.argtypes = [P, ctypes.POINTER(ctypes.c_double)]
+        L.gw_launch_count.argtypes = [P]
+        L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
+        L.gw_strerror.argtypes = [ctypes.c_int]
+        L.gw_strerror.restype = ctypes.c_char_p
+        L.gw_debug_set_naive.argtypes = [ctypes.c_int]
+        L.gw_debug_set_naive.restype = None
+        for n in ("gw_polarization", "gw_screened_interaction", "gw_selfenergy", "gw_exchange",
+                  "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_version"):
+            getattr(L, n).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def gw_strerror(code):
+    return lib().gw_strerror(int(code)).decode()
+
+
+def gw_version():
+    return int(lib().gw_version())
+
+
+def debug_set_naive(on):
+    lib().gw_debug_set_naive(1 if on else 0)
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise GWError(f"{what} failed: {gw_strerror(rc)} (code {rc})")
+
+
+def _dev(t, shape, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()):
+        raise GWError(f"{name}: need a contiguous CUDA complex128 tensor")
+    if tuple(t.shape) != tuple(shape):
+        raise GWError(f"{name}: shape {tuple(t.shape)} != expected {tuple(shape)}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+class GWProblem:
+    """The POD problem descriptor of gw.h plus the tensors it points to (kept alive here).
+
+    V, T_wt, T_tw: CUDA complex128 tensors for the device calls, or CPU tensors for gw_sigma_iteration_host."""
+
+    def __init__(self, mesh, nao, naux, ntau, nw, beta, V, T_wt, T_tw, spin_deg=2, q_begin=0, q_end=None):
+        self.mesh = tuple(int(m) for m in mesh)
+        self.nk = self.mesh[0] * self.mesh[1] * self.mesh[2]
+        self.nao, self.naux, self.ntau, self.nw = int(nao), int(naux), int(ntau), int(nw)
+        self.beta, self.spin_deg = float(beta), int(spin_deg)
+        self.q_begin = int(q_begin)
+        self.q_end = self.nk if q_end is None else int(q_end)
+        self.nq = self.q_end - self.q_begin
+        self.V, self.T_wt, self.T_tw = V, T_wt, T_tw
+        for name, t, shape in (("V", V, (self.nk, self.nk, naux, nao, nao)), ("T_wt", T_wt, (nw, ntau)),
+                               ("T_tw", T_tw, (ntau, nw))):
+            if t.dtype != torch.complex128 or not t.is_contiguous() or tuple(t.shape) != shape:
+                raise GWError(f"{name}: need contiguous complex128 of shape {shape}, got {tuple(t.shape)} {t.dtype}")
+        self.c = _CProblem(self.mesh[0], self.mesh[1], self.mesh[2], self.nao, self.naux, self.ntau, self.nw,
+                           self.spin_deg, self.q_begin, self.q_end, self.beta,
+                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr())
+
+    @property
+    def on_device(self):
+        return self.V.is_cuda
+
+    def shard(self, q_begin, q_end):
+        return GWProblem(self.mesh, self.nao, self.naux, self.ntau, self.nw, self.beta, self.V, self.T_wt, self.T_tw,
+                         self.spin_deg, q_begin, q_end)
+
+    def ref(self):
+        return ctypes.byref(self.c)
+
+
+def gw_workspace_bytes(prob):
+    return int(lib().gw_workspace_bytes(prob.ref()))
+
+
+def gw_polarization(prob, G, P0t=None, stream=None):
+    """Stage 1, Eq. 28b.  G [ntau][nk][nao][nao] -> P0t [ntau][nq][naux][naux]."""
+    g = _dev(G, (prob.ntau, prob.nk, prob.nao, prob.nao), "G")
+    if P0t is None:
+        P0t = torch.empty((prob.ntau, prob.nq, prob.naux, prob.naux), dtype=torch.complex128, device=G.device)
+    _check(lib().gw_polarization(prob.ref(), g, _dev(P0t, (prob.ntau, prob.nq, prob.naux, prob.naux), "P0t"),
+                                 _stream(stream)), "gw_polarization")
+    return P0t
+
+
+def gw_screened_interaction(prob, P0t, Wt=None, work=None, info=None, stream=None):
+    """Stage 2, Eq. 28a + 29 + 30.  Wt may alias P0t (pass Wt=P0t)."""
+    shape = (prob.ntau, prob.nq, prob.naux, prob.naux)
+    if Wt is None:
+        Wt = torch.empty(shape, dtype=torch.complex128, device=P0t.device)
+    nbytes = gw_workspace_bytes(prob)
+    if work is None:
+        work = torch.empty(nbytes, dtype=torch.uint8, device=P0t.device)
+    if info is None:
+        info = torch.empty(2, dtype=torch.int32, device=P0t.device)
+    _check(lib().gw_screened_interaction(prob.ref(), _dev(P0t, shape, "P0t"), _dev(Wt, shape, "Wt"),
+                                         ctypes.c_void_p(work.data_ptr()), ctypes.c_size_t(work.numel()),
+                                         ctypes.c_void_p(info.data_ptr()), _stream(stream)), "gw_screened_interaction")
+    return Wt, info
+
+
+def gw_selfenergy(prob, G, Wt, Sigma=None, stream=None):
+    """Stage 3, Eq. 31."""
+    gshape = (prob.ntau, prob.nk, prob.nao, prob.nao)
+    if Sigma is None:
+        Sigma = torch.empty(gshape, dtype=torch.complex128, device=G.device)
+    _check(lib().gw_selfenergy(prob.ref(), _dev(G, gshape, "G"),
+                               _dev(Wt, (prob.ntau, prob.nq, prob.naux, prob.naux), "Wt"),
+                               _dev(Sigma, gshape, "Sigma"), _stream(stream)), "gw_selfenergy")
+    return Sigma
+
+
+def gw_exchange(prob, gamma, K=None, stream=None):
+    """Stage 4, Eq. 22."""
+    shape = (prob.nk, prob.nao, prob.nao)
+    if K is None:
+        K = torch.empty(shape, dtype=torch.complex128, device=gamma.device)
+    _check(lib().gw_exchange(prob.ref(), _dev(gamma, shape, "gamma"), _dev(K, shape, "K"), _stream(stream)), "gw_exchange")
+    return K
+
+
+def gw_sigma_iteration(prob, G, gamma, bufs=None, stream=None):
+    """The whole hot path on device-resident inputs: four C-ABI calls on one stream.  Returns dict of outputs."""
+    b = bufs if bufs is not None else {}
+    P0t = gw_polarization(prob, G, b.get("P0t"), stream)
+    Wt, info = gw_screened_interaction(prob, P0t, b.get("Wt", P0t) if bufs is not None else None, b.get("work"), b.get("info"), stream)
+    Sigma = gw_selfenergy(prob, G, Wt, b.get("Sigma"), stream)
+    K = gw_exchange(prob, gamma, b.get("K"), stream)
+    return {"P0t": P0t, "Wt": Wt, "Sigma": Sigma, "K": K, "info": info}
+
+
+def gw_sigma_iteration_host(prob, G, gamma, Sigma=None, K=None, want_P0t=False, want_Wt=False, stream=None):
+    """End-to-end call with HOST buffers (pinned recommended); copies are inside the call."""
+    if prob.on_device:
+        raise GWError("gw_sigma_iteration_host needs a GWProblem built from CPU tensors")
+    for name, t in (("G", G), ("gamma", gamma)):
+        if t.is_cuda or t.dtype != torch.complex128 or not t.is_contiguous():
+            raise GWError(f"{name}: need a contiguous CPU complex128 tensor")
+    pin = G.is_pinned()
+    mk = lambda shape: torch.empty(shape, dtype=torch.complex128, pin_memory=pin)
+    if Sigma is None:
+        Sigma = mk((prob.ntau, prob.nk, prob.nao, prob.nao))
+    if K is None:
+        K = mk((prob.nk, prob.nao, prob.nao))
+    pshape = (prob.ntau, prob.nq, prob.naux, prob.naux)
+    P0t = mk(pshape) if want_P0t else None
+    Wt = mk(pshape) if want_Wt else None
+    ms = (ctypes.c_float * 6)()
+    vp = lambda t: ctypes.c_void_p(t.data_ptr()) if t is not None else None
+    _check(lib().gw_sigma_iteration_host(prob.ref(), vp(G), vp(gamma), vp(Sigma), vp(K), vp(P0t), vp(Wt),
+                                         ctypes.cast(ms, ctypes.c_void_p), _stream(stream)), "gw_sigma_iteration_host")
+    return {"Sigma": Sigma, "K": K, "P0t": P0t, "Wt": Wt, "stage_ms": list(ms)}
+
+
+def gw_executed_flops(prob):
+    out = (ctypes.c_double * 4)()
+    _check(lib().gw_executed_flops(prob.ref(), out), "gw_executed_flops")
+    return list(out)
+
+
+def gw_launch_count(prob):
+    return int(lib().gw_launch_count(prob.ref()))
+
+
+def gw_fp64_peak(ms=200.0, stream=None):
+    out = ctypes.c_double(0.0)
+    _check(lib().gw_fp64_peak(ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_fp64_peak")
+    return out.value

@@ -1,0 +1,196 @@
+// gw_api.cu — the C ABI of include/gw.h: argument validation, dispatch, the host-buffer iteration and the
+// FP64 peak probe.  No torch types, no exceptions across the boundary.
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include "gw_common.cuh"
+
+static int g_naive = -1;
+static bool use_naive() {
+  if (g_naive < 0) { const char *e = getenv("GW_DEBUG_NAIVE"); g_naive = (e && e[0] == '1') ? 1 : 0; }
+  return g_naive == 1;
+}
+extern "C" void gw_debug_set_naive(int on) { g_naive = on ? 1 : 0; }
+
+static int check_arch() {
+  static int cached = 0;
+  if (cached) return cached == 1 ? GW_OK : GW_EARCH;
+  int dev = 0, major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return GW_EARCH; }
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return GW_EARCH; }
+  cached = (major == 10) ? 1 : 2;
+  return cached == 1 ? GW_OK : GW_EARCH;
+}
+
+static bool aligned16(const void *p) { return p && (((uintptr_t)p) & 15) == 0; }
+
+static int check_problem(const gw_problem *p, bool need_T) {
+  if (!p) return GW_EINVAL;
+  if (p->nk1 <= 0 || p->nk2 <= 0 || p->nk3 <= 0 || p->nao <= 0 || p->naux <= 0 || p->ntau <= 0 || p->nw <= 0) return GW_EINVAL;
+  if (p->spin_deg != 1 && p->spin_deg != 2) return GW_EINVAL;
+  const int64_t nk = (int64_t)p->nk1 * p->nk2 * p->nk3;
+  if (nk > (1 << 20)) return GW_EINVAL;
+  if (p->q_begin < 0 || p->q_end > nk || p->q_begin >= p->q_end) return GW_EINVAL;
+  if (!aligned16(p->V)) return GW_EINVAL;
+  if (need_T && (!aligned16(p->T_wt) || !aligned16(p->T_tw))) return GW_EINVAL;
+  if (p->nao > 64 || p->ntau > 128 || p->nw > 128) return GW_ESHAPE;
+  return GW_OK;
+}
+
+extern "C" int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P0t, void *stream) {
+  int rc = check_problem(p, false); if (rc) return rc;
+  if (!aligned16(G) || !aligned16(P0t)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  return use_naive() ? gw_naive_stage1(p, (const c128 *)G, (c128 *)P0t, st) : gw_launch_stage1(p, (const c128 *)G, (c128 *)P0t, st);
+}
+
+extern "C" size_t gw_workspace_bytes(const gw_problem *p) {
+  if (check_problem(p, false) != GW_OK) return 0;
+  GwDims d = gw_dims(p);
+  size_t naive = 2 * (size_t)d.nw * d.nq * d.naux * d.naux * sizeof(c128);
+  size_t fast = gw_stage2_workspace(p);
+  return (naive > fast ? naive : fast) + 256;
+}
+
+extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, void *work, size_t work_bytes,
+                                       int32_t *info, void *stream) {
+  int rc = check_problem(p, true); if (rc) return rc;
+  if (!aligned16(P0t) || !aligned16(Wt) || !work || (((uintptr_t)work) & 255)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  return use_naive() ? gw_naive_stage2(p, (const c128 *)P0t, (c128 *)Wt, work, work_bytes, info, st)
+                     : gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, work, work_bytes, info, st);
+}
+
+extern "C" int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c128 *Sigma, void *stream) {
+  int rc = check_problem(p, false); if (rc) return rc;
+  if (!aligned16(G) || !aligned16(Wt) || !aligned16(Sigma)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  return use_naive() ? gw_naive_stage3(p, (const c128 *)G, (const c128 *)Wt, (c128 *)Sigma, st)
+                     : gw_launch_stage3(p, (const c128 *)G, (const c128 *)Wt, (c128 *)Sigma, st);
+}
+
+extern "C" int gw_exchange(const gw_problem *p, const gw_c128 *gamma, gw_c128 *K, void *stream) {
+  int rc = check_problem(p, false); if (rc) return rc;
+  if (!aligned16(gamma) || !aligned16(K)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  return use_naive() ? gw_naive_stage4(p, (const c128 *)gamma, (c128 *)K, st) : gw_launch_stage4(p, (const c128 *)gamma, (c128 *)K, st);
+}
+
+extern "C" int gw_executed_flops(const gw_problem *p, double *out) {
+  int rc = check_problem(p, false); if (rc) return rc;
+  if (!out) return GW_EINVAL;
+  gw_stage_flops(p, out);
+  return GW_OK;
+}
+
+extern "C" int gw_launch_count(const gw_problem *p) {
+  if (check_problem(p, false) != GW_OK) return 0;
+  return gw_stage_launches(p);
+}
+
+#define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { rc = (int)e_; goto done; } } while (0)
+
+extern "C" int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, const gw_c128 *gamma, gw_c128 *Sigma, gw_c128 *K,
+                                       gw_c128 *P0t_out, gw_c128 *Wt_out, float *stage_ms, void *stream) {
+  int rc = check_problem(p, true); if (rc) return rc;
+  if (!G || !gamma || !Sigma || !K) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  GwDims d = gw_dims(p);
+  const size_t n2 = (size_t)d.nao * d.nao, a2 = (size_t)d.naux * d.naux;
+  const size_t bV = (size_t)d.nk * d.nk * d.naux * n2 * 16, bG = (size_t)d.ntau * d.nk * n2 * 16, bg = (size_t)d.nk * n2 * 16;
+  const size_t bP = (size_t)d.ntau * d.nq * a2 * 16, bT = (size_t)d.nw * d.ntau * 16;
+  c128 *dV = 0, *dG = 0, *dg = 0, *dP = 0, *dS = 0, *dK = 0, *dTwt = 0, *dTtw = 0; void *dW = 0; int32_t *dinfo = 0;
+  cudaEvent_t ev[7]; for (int i = 0; i < 7; i++) ev[i] = 0;
+  gw_problem dp = *p;
+  size_t wb = 0;
+  for (int i = 0; i < 7; i++) CU(cudaEventCreate(&ev[i]));
+  CU(cudaMalloc(&dV, bV)); CU(cudaMalloc(&dG, bG)); CU(cudaMalloc(&dg, bg)); CU(cudaMalloc(&dP, bP));
+  CU(cudaMalloc(&dS, bG)); CU(cudaMalloc(&dK, bg)); CU(cudaMalloc(&dTwt, bT)); CU(cudaMalloc(&dTtw, bT));
+  CU(cudaMalloc(&dinfo, 8));
+  dp.V = (const gw_c128 *)dV; dp.T_wt = (const gw_c128 *)dTwt; dp.T_tw = (const gw_c128 *)dTtw;
+  wb = gw_workspace_bytes(&dp);
+  CU(cudaMalloc(&dW, wb));
+  CU(cudaEventRecord(ev[0], st));
+  CU(cudaMemcpyAsync(dV, p->V, bV, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dG, G, bG, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dg, gamma, bg, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dTwt, p->T_wt, bT, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dTtw, p->T_tw, bT, cudaMemcpyHostToDevice, st));
+  CU(cudaEventRecord(ev[1], st));
+  if ((rc = gw_polarization(&dp, (gw_c128 *)dG, (gw_c128 *)dP, st))) goto done;
+  if (P0t_out) CU(cudaMemcpyAsync(P0t_out, dP, bP, cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(ev[2], st));
+  if ((rc = gw_screened_interaction(&dp, (gw_c128 *)dP, (gw_c128 *)dP, dW, wb, dinfo, st))) goto done;
+  CU(cudaEventRecord(ev[3], st));
+  if ((rc = gw_selfenergy(&dp, (gw_c128 *)dG, (gw_c128 *)dP, (gw_c128 *)dS, st))) goto done;
+  CU(cudaEventRecord(ev[4], st));
+  if ((rc = gw_exchange(&dp, (gw_c128 *)dg, (gw_c128 *)dK, st))) goto done;
+  CU(cudaEventRecord(ev[5], st));
+  if (Wt_out) CU(cudaMemcpyAsync(Wt_out, dP, bP, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(Sigma, dS, bG, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(K, dK, bg, cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(ev[6], st));
+  CU(cudaStreamSynchronize(st));
+  if (stage_ms) for (int i = 0; i < 6; i++) CU(cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]));
+done:
+  cudaFree(dV); cudaFree(dG); cudaFree(dg); cudaFree(dP); cudaFree(dS); cudaFree(dK); cudaFree(dTwt); cudaFree(dTtw); cudaFree(dW); cudaFree(dinfo);
+  for (int i = 0; i < 7; i++) if (ev[i]) cudaEventDestroy(ev[i]);
+  return rc;
+}
+
+// ---- FP64 peak probe: register-resident DMMA.8x8x4 loop, 8 independent accumulators per warp ----
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, int iters) {
+  double acc[8][2];
+#pragma unroll
+  for (int i = 0; i < 8; i++) { acc[i][0] = threadIdx.x * 1e-3 + i; acc[i][1] = i; }
+  double a = 1e-3 + threadIdx.x * 1e-9, b = 1e-3;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 8; i++) dmma884(acc[i][0], acc[i][1], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; i++) s += acc[i][0] + acc[i][1];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int gw_fp64_peak(double ms, double *tflops, void *stream) {
+  if (!tflops || !(ms > 0)) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, nsm = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  double *out = 0; cudaEvent_t e0 = 0, e1 = 0; float t = 0;
+  const int iters = 20000, grid = nsm * 2;
+  const double fl = 2.0 * 256 * 8 * (double)iters * 8 * grid;   // per launch
+  int reps = 1;
+  CU(cudaMalloc(&out, sizeof(double) * grid * 256));
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  fp64_peak_kernel<<<grid, 256, 0, st>>>(out, iters);            // warm-up, ~2.6 ms
+  reps = (int)(ms / 2.6) + 1;
+  CU(cudaEventRecord(e0, st));
+  for (int r = 0; r < reps; r++) fp64_peak_kernel<<<grid, 256, 0, st>>>(out, iters);
+  CU(cudaEventRecord(e1, st));
+  CU(cudaEventSynchronize(e1));
+  CU(cudaEventElapsedTime(&t, e0, e1));
+  *tflops = fl * reps / (t * 1e-3) * 1e-12;
+done:
+  cudaFree(out); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1);
+  return rc;
+}
+
+extern "C" const char *gw_strerror(int code) {
+  switch (code) {
+    case GW_OK: return "ok";
+    case GW_EINVAL: return "invalid argument (null/misaligned pointer, non-positive size or bad q range)";
+    case GW_ENOMEM: return "workspace too small";
+    case GW_EARCH: return "current device is not sm_100 (B200)";
+    case GW_ESHAPE: return "size not supported by the kernels (nao > 64, ntau or nw > 128)";
+    default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown error";
+  }
+}
+extern "C" int gw_version(void) { return 100; }
