@@ -59,6 +59,8 @@ typedef struct {
   const gw_c128 *V;        /* device [nk][nk][naux][nao][nao]: V^{k1 k2}_{ij}(Q), Eq. 6-7 */
   const gw_c128 *T_wt;     /* device [nw][ntau]: bosonic τ→iΩ transform matrix, Eq. 28a */
   const gw_c128 *T_tw;     /* device [ntau][nw]: bosonic iΩ→τ transform matrix, Eq. 30 */
+  void *work;              /* device scratch shared by the four calls (L2-resident intermediates, solver copies), */
+  size_t work_bytes;       /*   at least gw_workspace_bytes(p) bytes, 256-byte aligned; contents are don't-care    */
 } gw_problem;
 
 /* Stage 1 — Eq. 28b, Algorithm 1 first k loop:
@@ -72,10 +74,8 @@ int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P0t, void *s
  *   P0w[n] = Σ_t T_wt[n][t] P0t[t];   Ww[n] = (I − P0w[n])^-1 P0w[n]  (Cholesky);   Wt[t] = Σ_n T_tw[t][n] Ww[n]
  *   P0t : device [ntau][nq][naux][naux]    in
  *   Wt  : device [ntau][nq][naux][naux]    out; may alias P0t (then P0t is overwritten)
- *   work: device scratch of at least gw_workspace_bytes(p) bytes, 256-byte aligned
  *   info: device int32[2] or NULL.  Set to {-1,-1} on success, else {q, n} of one failing factorisation. */
-int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, void *work, size_t work_bytes,
-                            int32_t *info, void *stream);
+int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, void *stream);
 
 /* Stage 3 — Eq. 31, Algorithm 1 second k loop:
  *   Sigma[t][k][i][j] = -(1/N_k) Σ_{q in shard} Σ_QQ' Σ_ab V[k][k-q][Q][i][a] G[t][k-q][a][b] Wt[t][q-q_begin][Q][Q'] V[k-q][k][Q'][b][j]
@@ -90,7 +90,8 @@ int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c
  *   K     : device [nk][nao][nao]  out */
 int gw_exchange(const gw_problem *p, const gw_c128 *gamma, gw_c128 *K, void *stream);
 
-/* Scratch needed by gw_screened_interaction for this problem (bytes; host-side arithmetic only). */
+/* Scratch (p->work) needed by the four calls for this problem: the maximum over the stages (bytes; host-side
+ * arithmetic only, p->work / p->work_bytes are ignored). */
 size_t gw_workspace_bytes(const gw_problem *p);
 
 /* Whole iteration with HOST buffers (the end-to-end path timed as `e2e` by bench.py): uploads V, G, gamma,

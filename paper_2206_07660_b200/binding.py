@@ -18,7 +18,8 @@ class _CProblem(ctypes.Structure):
                 ("nao", ctypes.c_int32), ("naux", ctypes.c_int32), ("ntau", ctypes.c_int32), ("nw", ctypes.c_int32),
                 ("spin_deg", ctypes.c_int32), ("q_begin", ctypes.c_int32), ("q_end", ctypes.c_int32),
                 ("beta", ctypes.c_double),
-                ("V", ctypes.c_void_p), ("T_wt", ctypes.c_void_p), ("T_tw", ctypes.c_void_p)]
+                ("V", ctypes.c_void_p), ("T_wt", ctypes.c_void_p), ("T_tw", ctypes.c_void_p),
+                ("work", ctypes.c_void_p), ("work_bytes", ctypes.c_size_t)]
 
 
 def lib_path():
@@ -36,7 +37,7 @@ def lib():
         P = ctypes.POINTER(_CProblem)
         vp, sz = ctypes.c_void_p, ctypes.c_size_t
         L.gw_polarization.argtypes = [P, vp, vp, vp]
-        L.gw_screened_interaction.argtypes = [P, vp, vp, vp, sz, vp, vp]
+        L.gw_screened_interaction.argtypes = [P, vp, vp, vp, vp]
         L.gw_selfenergy.argtypes = [P, vp, vp, vp, vp]
         L.gw_exchange.argtypes = [P, vp, vp, vp]
         L.gw_workspace_bytes.argtypes = [P]
@@ -107,7 +108,16 @@ class GWProblem:
                 raise GWError(f"{name}: need contiguous complex128 of shape {shape}, got {tuple(t.shape)} {t.dtype}")
         self.c = _CProblem(self.mesh[0], self.mesh[1], self.mesh[2], self.nao, self.naux, self.ntau, self.nw,
                            self.spin_deg, self.q_begin, self.q_end, self.beta,
-                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr())
+                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr(), None, 0)
+        self.work = None
+        if V.is_cuda:
+            self.set_work(torch.empty(int(lib().gw_workspace_bytes(ctypes.byref(self.c))), dtype=torch.uint8, device=V.device))
+
+    def set_work(self, work):
+        """Attach the device workspace (uint8 CUDA tensor of at least gw_workspace_bytes bytes)."""
+        self.work = work
+        self.c.work = work.data_ptr()
+        self.c.work_bytes = work.numel()
 
     @property
     def on_device(self):
@@ -135,18 +145,14 @@ def gw_polarization(prob, G, P0t=None, stream=None):
     return P0t
 
 
-def gw_screened_interaction(prob, P0t, Wt=None, work=None, info=None, stream=None):
+def gw_screened_interaction(prob, P0t, Wt=None, info=None, stream=None):
     """Stage 2, Eq. 28a + 29 + 30.  Wt may alias P0t (pass Wt=P0t)."""
     shape = (prob.ntau, prob.nq, prob.naux, prob.naux)
     if Wt is None:
         Wt = torch.empty(shape, dtype=torch.complex128, device=P0t.device)
-    nbytes = gw_workspace_bytes(prob)
-    if work is None:
-        work = torch.empty(nbytes, dtype=torch.uint8, device=P0t.device)
     if info is None:
         info = torch.empty(2, dtype=torch.int32, device=P0t.device)
     _check(lib().gw_screened_interaction(prob.ref(), _dev(P0t, shape, "P0t"), _dev(Wt, shape, "Wt"),
-                                         ctypes.c_void_p(work.data_ptr()), ctypes.c_size_t(work.numel()),
                                          ctypes.c_void_p(info.data_ptr()), _stream(stream)), "gw_screened_interaction")
     return Wt, info
 
@@ -175,7 +181,7 @@ def gw_sigma_iteration(prob, G, gamma, bufs=None, stream=None):
     """The whole hot path on device-resident inputs: four C-ABI calls on one stream.  Returns dict of outputs."""
     b = bufs if bufs is not None else {}
     P0t = gw_polarization(prob, G, b.get("P0t"), stream)
-    Wt, info = gw_screened_interaction(prob, P0t, b.get("Wt", P0t) if bufs is not None else None, b.get("work"), b.get("info"), stream)
+    Wt, info = gw_screened_interaction(prob, P0t, b.get("Wt", P0t) if bufs is not None else None, b.get("info"), stream)
     Sigma = gw_selfenergy(prob, G, Wt, b.get("Sigma"), stream)
     K = gw_exchange(prob, gamma, b.get("K"), stream)
     return {"P0t": P0t, "Wt": Wt, "Sigma": Sigma, "K": K, "info": info}

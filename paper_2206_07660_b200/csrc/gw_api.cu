@@ -48,19 +48,23 @@ extern "C" int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P
 extern "C" size_t gw_workspace_bytes(const gw_problem *p) {
   if (check_problem(p, false) != GW_OK) return 0;
   GwDims d = gw_dims(p);
-  size_t naive = 2 * (size_t)d.nw * d.nq * d.naux * d.naux * sizeof(c128);
-  size_t fast = gw_stage2_workspace(p);
-  return (naive > fast ? naive : fast) + 256;
+  size_t m = 2 * (size_t)d.nw * d.nq * d.naux * d.naux * sizeof(c128);   // debug reference kernels
+  size_t s;
+  if ((s = gw_stage1_workspace(p)) > m) m = s;
+  if ((s = gw_stage2_workspace(p)) > m) m = s;
+  if ((s = gw_stage3_workspace(p)) > m) m = s;
+  if ((s = gw_stage4_workspace(p)) > m) m = s;
+  return (m + 255) / 256 * 256;
 }
 
-extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, void *work, size_t work_bytes,
-                                       int32_t *info, void *stream) {
+extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, void *stream) {
   int rc = check_problem(p, true); if (rc) return rc;
-  if (!aligned16(P0t) || !aligned16(Wt) || !work || (((uintptr_t)work) & 255)) return GW_EINVAL;
+  if (!aligned16(P0t) || !aligned16(Wt)) return GW_EINVAL;
+  if (!p->work || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  return use_naive() ? gw_naive_stage2(p, (const c128 *)P0t, (c128 *)Wt, work, work_bytes, info, st)
-                     : gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, work, work_bytes, info, st);
+  return use_naive() ? gw_naive_stage2(p, (const c128 *)P0t, (c128 *)Wt, p->work, p->work_bytes, info, st)
+                     : gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, st);
 }
 
 extern "C" int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c128 *Sigma, void *stream) {
@@ -115,6 +119,7 @@ extern "C" int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, co
   dp.V = (const gw_c128 *)dV; dp.T_wt = (const gw_c128 *)dTwt; dp.T_tw = (const gw_c128 *)dTtw;
   wb = gw_workspace_bytes(&dp);
   CU(cudaMalloc(&dW, wb));
+  dp.work = dW; dp.work_bytes = wb;
   CU(cudaEventRecord(ev[0], st));
   CU(cudaMemcpyAsync(dV, p->V, bV, cudaMemcpyHostToDevice, st));
   CU(cudaMemcpyAsync(dG, G, bG, cudaMemcpyHostToDevice, st));
@@ -125,7 +130,7 @@ extern "C" int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, co
   if ((rc = gw_polarization(&dp, (gw_c128 *)dG, (gw_c128 *)dP, st))) goto done;
   if (P0t_out) CU(cudaMemcpyAsync(P0t_out, dP, bP, cudaMemcpyDeviceToHost, st));
   CU(cudaEventRecord(ev[2], st));
-  if ((rc = gw_screened_interaction(&dp, (gw_c128 *)dP, (gw_c128 *)dP, dW, wb, dinfo, st))) goto done;
+  if ((rc = gw_screened_interaction(&dp, (gw_c128 *)dP, (gw_c128 *)dP, dinfo, st))) goto done;
   CU(cudaEventRecord(ev[3], st));
   if ((rc = gw_selfenergy(&dp, (gw_c128 *)dG, (gw_c128 *)dP, (gw_c128 *)dS, st))) goto done;
   CU(cudaEventRecord(ev[4], st));

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <string.h>
 #include "../../include/gw.h"
 
 typedef double2 c128;   // (re, im); layout-compatible with gw_c128
@@ -66,10 +67,14 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 
 // kernel launchers implemented per stage
 int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t st);
-int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, void *work, size_t work_bytes, int32_t *info, cudaStream_t st);
+int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *info, cudaStream_t st);
 int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st);
 int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st);
+size_t gw_stage1_workspace(const gw_problem *p);
 size_t gw_stage2_workspace(const gw_problem *p);
+size_t gw_stage3_workspace(const gw_problem *p);
+size_t gw_stage4_workspace(const gw_problem *p);
+double gw_stage1_flops(const gw_problem *p);
 void gw_stage_flops(const gw_problem *p, double *out4);
 int gw_stage_launches(const gw_problem *p);
 
