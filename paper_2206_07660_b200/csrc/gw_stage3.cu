@@ -1,0 +1,381 @@
+// gw_stage3.cu — stage 3, Eq. 31 (Algorithm 1 second k loop):
+//
+//   Sigma[t][k][i][j] = -(1/N_k) Σ_q Σ_QQ' Σ_ab V[k][k-q][Q][i][a] G[t][k-q][a][b] Wt[t][q][Q][Q'] V[k-q][k][Q'][b][j]
+//
+// Formulation (exact algebra, mirror image of stage 1; V1 = V[k][k-q], V2 = V[k-q][k]):
+//   main  :  U[Q][(b,j)]  = Σ_Q' Wt[Q][Q'] V2[Q'][(b,j)]              GEMM, M = Q panel, N = nao², K = naux
+//   pass A:  T[Q][a][j]   = Σ_b G[a][b] U[Q][b][j]                     rows (Q,j) flat, K = nao
+//   final :  Sigma[i][j] += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]             K = (Q,a)
+// A persistent CTA owns one (t,k): it loops over q and over Q panels, and keeps the nao x nao Sigma accumulator in
+// registers for the whole item, so the q-sum needs no cross-CTA reduction and the result is deterministic.
+// U and T live in two per-CTA slabs of the workspace (L2 resident); the raw V2 block is the only big stream.
+#include "gw_common.cuh"
+
+namespace s3 {
+
+constexpr int NTHR = 256, NSTAGE = 3;
+constexpr int PASS_ROWS = 64, KC = 8, MT_W = 2, NJ = 7, TM = 32;
+
+struct Params {
+  GwDims d;
+  const c128 *V, *G, *Wt;
+  c128 *Sigma, *scratch;
+  unsigned *counter;
+  int nqt, nitems;
+  int ldp, ksp, ndt;      // pass / G smem row stride, k-steps over nao, tiles over nao
+  int ldt;                // row stride of the T block in the final jobs
+  int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
+  int ldb;                // row stride of the main-job B part
+  int stage_units;
+  size_t slab_units;      // complex elements per slab (two slabs per CTA)
+};
+
+__device__ __forceinline__ void cp_async16_zfill(void *smem, const void *gmem, bool ok) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  int n = ok ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(n));
+}
+
+__device__ __forceinline__ void issue_pass_job(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp) {
+  const int nrow = min(PASS_ROWS, rows_total - row0);
+  const int total = nrow * nao;
+  const c128 *s = src + (size_t)row0 * nao;
+  for (int i = threadIdx.x; i < total; i += NTHR) {
+    const int r = i / nao, a = i - r * nao;
+    cp_async16(stage + r * ldp + a, s + i);
+  }
+}
+
+// main job: A = W[tm rows][k0..k0+8) swizzled; B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
+__device__ __forceinline__ void issue_main_job(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
+                                               int n0, int ncols, int ldb, int k0) {
+  for (int i = threadIdx.x; i < TM * KC; i += NTHR) {
+    const int r = i >> 3, u = i & 7;
+    const bool ok = (r < tm_rows) && (k0 + u < naux);
+    cp_async16_zfill(stage + r * KC + (u ^ ((r & 1) << 2)), ok ? W + (size_t)r * naux + k0 + u : W, ok);
+  }
+  c128 *sB = stage + TM * KC;
+  const int total = KC * ncols;
+  for (int i = threadIdx.x; i < total; i += NTHR) {
+    const int r = i / ncols, cc = i - r * ncols;
+    const bool ok = (k0 + r < naux) && (n0 + cc < n2);
+    cp_async16_zfill(sB + r * ldb + cc, ok ? V2 + (size_t)(k0 + r) * n2 + n0 + cc : V2, ok);
+  }
+}
+
+// final job for one Q: A = V1[Q] as [i][ldp]; B = T[Q] as [a][ldt] with rows a >= nao zero-filled
+__device__ __forceinline__ void issue_final_job(c128 *stage, const c128 *V1Q, const c128 *TQ, int nao, int ldp, int ldt, int ksp, int naop) {
+  const int n2 = nao * nao;
+  for (int i = threadIdx.x; i < n2; i += NTHR) {
+    const int r = i / nao, a = i - r * nao;
+    cp_async16(stage + r * ldp + a, V1Q + i);
+  }
+  c128 *sB = stage + naop * ldp;
+  const int rowsB = 4 * ksp;
+  for (int i = threadIdx.x; i < rowsB * nao; i += NTHR) {
+    const int r = i / nao, j = i - r * nao;
+    const bool ok = r < nao;
+    cp_async16_zfill(sB + r * ldt + j, ok ? TQ + i : TQ, ok);
+  }
+}
+
+// pass A: rows (Q,j) of Ut times G^T: out T[(Q*nao + a)*nao + j]
+template <int KSP_MAX>
+__device__ __forceinline__ void passA_compute(const c128 *sStage, const c128 *sG, c128 *slabT, int row0, int rows_total,
+                                              int nao, int ldp, int ksp, int ndt) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  if (row0 + 8 * w >= rows_total) return;
+  c128 a[KSP_MAX];
+#pragma unroll
+  for (int ks = 0; ks < KSP_MAX; ks++)
+    if (ks < ksp) a[ks] = sStage[(8 * w + g) * ldp + 4 * ks + c];
+  const int row = row0 + 8 * w + g;
+  const bool rok = row < rows_total;
+  const int Q = row / nao, j = row - Q * nao;
+  for (int nt = 0; nt < ndt; nt++) {
+    double cr[2] = {0.0, 0.0}, ci[2] = {0.0, 0.0};
+    const c128 *bp = sG + (8 * nt + g) * ldp + c;
+#pragma unroll
+    for (int ks = 0; ks < KSP_MAX; ks++)
+      if (ks < ksp) cmma(cr, ci, a[ks], bp[4 * ks]);
+    const int col = 8 * nt + 2 * c;   // a index
+    if (rok) {
+      if (col < nao) slabT[((size_t)Q * nao + col) * nao + j] = make_double2(cr[0], ci[0]);
+      if (col + 1 < nao) slabT[((size_t)Q * nao + col + 1) * nao + j] = make_double2(cr[1], ci[1]);
+    }
+  }
+}
+
+template <int KSP_MAX, int NCT>
+__global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  c128 *smem = reinterpret_cast<c128 *>(smem_raw);
+  const GwDims d = P.d;
+  const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, naop = 8 * P.ndt, ndt = P.ndt;
+  c128 *sG = smem;                    // [naop][ldp]: sG[a][b] = G[t][k-q][a][b]  (operand [n=a][k=b] of pass A)
+  c128 *sStage = sG + naop * ldp;
+  __shared__ int s_item;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  const int mh = w >> 2;                              // m-half: m-tiles 2*mh, 2*mh+1
+  const int sw = (g & 1) << 2;
+  c128 *slabU = P.scratch + (size_t)blockIdx.x * 2 * P.slab_units;
+  c128 *slabT = slabU + P.slab_units;
+  const size_t vb = (size_t)naux * n2;
+  const int ntiles_out = ndt * ndt;
+
+  {
+    const int tot = naop * ldp + NSTAGE * P.stage_units;
+    for (int i = threadIdx.x; i < tot; i += NTHR) smem[i] = make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+
+  for (;;) {
+    if (threadIdx.x == 0) s_item = (int)atomicAdd(P.counter, 1u);
+    __syncthreads();
+    const int item = s_item;
+    __syncthreads();
+    if (item >= P.nitems) break;
+    const int t = item % d.ntau, k = item / d.ntau;
+
+    double sgr[NCT][2], sgi[NCT][2];
+#pragma unroll
+    for (int i = 0; i < NCT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+
+    for (int ql = 0; ql < d.nq; ql++) {
+      const int q = d.q0 + ql, kp = gw_ksub(d, k, q);
+      const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
+      const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
+      const c128 *Gp = P.G + ((size_t)t * d.nk + kp) * n2;
+      const c128 *Wq = P.Wt + ((size_t)t * d.nq + ql) * naux * naux;
+      __syncthreads();
+      for (int i = threadIdx.x; i < n2; i += NTHR) { const int r = i / nao, cc = i - r * nao; sG[r * ldp + cc] = Gp[i]; }
+
+      for (int qt = 0; qt < P.nqt; qt++) {
+        const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
+        const c128 *W = Wq + (size_t)Q0 * naux;
+        const int nmain = (naux + KC - 1) / KC;
+        // ---- main GEMM, N chunk by N chunk; U^T written to slabU as [(Q,j)][b] ----
+        for (int ch = 0; ch < P.nchunk; ch++) {
+          const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);     // n-tiles of this chunk
+          const int n0 = nt0 * 8, ncols = ntc * 8;
+          const int noff = ((w & 3) - mh + 4) & 3;
+          const int njm = (ntc > noff) ? (ntc - noff + 3) / 4 : 0;
+          double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
+#pragma unroll
+          for (int i = 0; i < MT_W; i++)
+#pragma unroll
+            for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
+          int issued = 0;
+          for (; issued < NSTAGE - 1; issued++) {
+            if (issued < nmain) issue_main_job(sStage + (issued % NSTAGE) * P.stage_units, W, tm_rows, naux, V2, n2, n0, ncols, P.ldb, issued * KC);
+            cp_async_commit();
+          }
+          for (int jb = 0; jb < nmain; jb++) {
+            cp_async_wait<NSTAGE - 2>();
+            __syncthreads();
+            const int nx = jb + NSTAGE - 1;
+            if (nx < nmain) issue_main_job(sStage + (nx % NSTAGE) * P.stage_units, W, tm_rows, naux, V2, n2, n0, ncols, P.ldb, nx * KC);
+            cp_async_commit();
+            const c128 *sA = sStage + (jb % NSTAGE) * P.stage_units;
+            const c128 *sB = sA + TM * KC;
+            if (mh * MT_W < mtc) {
+#pragma unroll
+              for (int ks = 0; ks < KC / 4; ks++) {
+                const int u = (4 * ks + c) ^ sw;
+                c128 a[MT_W];
+#pragma unroll
+                for (int i = 0; i < MT_W; i++) a[i] = sA[(8 * (mh * MT_W + i) + g) * KC + u];
+                const c128 *brow = sB + (4 * ks + c) * P.ldb + g;
+#pragma unroll
+                for (int jn = 0; jn < NJ; jn++) {
+                  if (jn < njm) {
+                    const c128 b = brow[8 * (noff + 4 * jn)];
+#pragma unroll
+                    for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
+                  }
+                }
+              }
+            }
+          }
+          cp_async_wait<0>();
+          // store U^T: element (Q, n=(b,j)) -> slabU[(Q*nao + j)*nao + b]
+#pragma unroll
+          for (int i = 0; i < MT_W; i++) {
+            const int Ql = 8 * (mh * MT_W + i) + g;
+#pragma unroll
+            for (int jn = 0; jn < NJ; jn++) {
+              if (jn < njm && Ql < tm_rows) {
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                  const int n = n0 + 8 * (noff + 4 * jn) + 2 * c + e;
+                  if (n < n2) {
+                    const int b = n / nao, j = n - b * nao;
+                    slabU[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
+                  }
+                }
+              }
+            }
+          }
+          __syncthreads();
+        }
+        // ---- pass A: T[Q][a][j] = Σ_b G[a][b] U[Q][b][j] ----
+        {
+          const int rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
+          int issued = 0;
+          for (; issued < NSTAGE - 1; issued++) {
+            if (issued < npass) issue_pass_job(sStage + (issued % NSTAGE) * P.stage_units, slabU, issued * PASS_ROWS, rows, nao, ldp);
+            cp_async_commit();
+          }
+          for (int jb = 0; jb < npass; jb++) {
+            cp_async_wait<NSTAGE - 2>();
+            __syncthreads();
+            const int nx = jb + NSTAGE - 1;
+            if (nx < npass) issue_pass_job(sStage + (nx % NSTAGE) * P.stage_units, slabU, nx * PASS_ROWS, rows, nao, ldp);
+            cp_async_commit();
+            passA_compute<KSP_MAX>(sStage + (jb % NSTAGE) * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
+          }
+          cp_async_wait<0>();
+          __syncthreads();
+        }
+        // ---- final: Sigma[i][j] += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; one job per Q ----
+        {
+          const c128 *V1t = V1 + (size_t)Q0 * n2;
+          int issued = 0;
+          for (; issued < NSTAGE - 1; issued++) {
+            if (issued < tm_rows) issue_final_job(sStage + (issued % NSTAGE) * P.stage_units, V1t + (size_t)issued * n2, slabT + (size_t)issued * n2, nao, ldp, P.ldt, P.ksp, naop);
+            cp_async_commit();
+          }
+          for (int jb = 0; jb < tm_rows; jb++) {
+            cp_async_wait<NSTAGE - 2>();
+            __syncthreads();
+            const int nx = jb + NSTAGE - 1;
+            if (nx < tm_rows) issue_final_job(sStage + (nx % NSTAGE) * P.stage_units, V1t + (size_t)nx * n2, slabT + (size_t)nx * n2, nao, ldp, P.ldt, P.ksp, naop);
+            cp_async_commit();
+            const c128 *sA = sStage + (jb % NSTAGE) * P.stage_units;
+            const c128 *sB = sA + naop * ldp;
+#pragma unroll
+            for (int ti = 0; ti < NCT; ti++) {
+              const int tile = w + 8 * ti;
+              if (tile < ntiles_out) {
+                const int mi = tile / ndt, nj = tile - mi * ndt;
+                const c128 *ap = sA + (8 * mi + g) * ldp + c;
+                const c128 *bp = sB + c * P.ldt + 8 * nj + g;
+                for (int ks = 0; ks < P.ksp; ks++) cmma(sgr[ti], sgi[ti], ap[4 * ks], bp[4 * ks * P.ldt]);
+              }
+            }
+          }
+          cp_async_wait<0>();
+          __syncthreads();
+        }
+      }
+    }
+    // ---- epilogue ----
+    const double pref = -1.0 / (double)d.nk;
+    c128 *out = P.Sigma + ((size_t)t * d.nk + k) * n2;
+#pragma unroll
+    for (int ti = 0; ti < NCT; ti++) {
+      const int tile = w + 8 * ti;
+      if (tile < ntiles_out) {
+        const int mi = tile / ndt, nj = tile - mi * ndt;
+        const int i = 8 * mi + g, j = 8 * nj + 2 * c;
+        if (i < nao) {
+          if (j < nao) out[i * nao + j] = make_double2(pref * sgr[ti][0], pref * sgi[ti][0]);
+          if (j + 1 < nao) out[i * nao + j + 1] = make_double2(pref * sgr[ti][1], pref * sgi[ti][1]);
+        }
+      }
+    }
+  }
+}
+
+struct Plan {
+  int ksp_max, nct, nqt, nitems, ldp, ksp, ndt, ldt, nnt, nchunk, cht, ldb, stage_units, grid;
+  size_t smem, slab_units, work_bytes;
+  bool ok;
+};
+
+static Plan make_plan(const gw_problem *p) {
+  Plan pl; memset(&pl, 0, sizeof(pl));
+  GwDims d = gw_dims(p);
+  pl.ksp = (d.nao + 3) / 4;
+  if (pl.ksp > 16) { pl.ok = false; return pl; }
+  pl.ksp_max = pl.ksp <= 7 ? 7 : (pl.ksp <= 13 ? 13 : 16);
+  pl.ndt = (d.nao + 7) / 8;
+  pl.nct = (pl.ndt * pl.ndt + 7) / 8 <= 2 ? 2 : 8;
+  int r4 = pl.ksp * 4; if (r4 % 8 == 0) r4 += 4;
+  pl.ldp = r4;
+  int naop = 8 * pl.ndt;
+  pl.ldt = naop + 2;                       // ≡ 2 (mod 8): conflict-free K-major B fragments
+  pl.nnt = (d.nao * d.nao + 7) / 8;
+  pl.nchunk = (pl.nnt + 4 * NJ - 1) / (4 * NJ);
+  pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
+  pl.ldb = pl.cht * 8 + 2;
+  pl.nqt = (d.naux + TM - 1) / TM;
+  pl.nitems = d.ntau * d.nk;
+  int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + KC * pl.ldb, s_fin = naop * pl.ldp + 4 * pl.ksp * pl.ldt + 8;
+  pl.stage_units = s_pass;
+  if (s_main > pl.stage_units) pl.stage_units = s_main;
+  if (s_fin > pl.stage_units) pl.stage_units = s_fin;
+  pl.smem = ((size_t)naop * pl.ldp + (size_t)NSTAGE * pl.stage_units) * sizeof(c128);
+  int dev = 0, nsm = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  if (nsm <= 0) nsm = 148;
+  pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
+  pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
+  pl.work_bytes = 256 + (size_t)nsm * 2 * pl.slab_units * sizeof(c128);
+  pl.ok = pl.smem <= 227 * 1024;
+  return pl;
+}
+
+}  // namespace s3
+
+size_t gw_stage3_workspace(const gw_problem *p) {
+  s3::Plan pl = s3::make_plan(p);
+  return pl.ok ? pl.work_bytes : 0;
+}
+
+double gw_stage3_flops(const gw_problem *p) {
+  s3::Plan pl = s3::make_plan(p);
+  if (!pl.ok) return 0.0;
+  GwDims d = gw_dims(p);
+  double tiles = 0.0;
+  const double nmain = (d.naux + s3::KC - 1) / s3::KC;
+  for (int qt = 0; qt < pl.nqt; qt++) {
+    const int tm_rows = (d.naux - qt * s3::TM) < s3::TM ? (d.naux - qt * s3::TM) : s3::TM;
+    const int mtc = (tm_rows + 7) / 8;
+    const double mtiles = (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
+    tiles += mtiles * pl.nnt * (s3::KC / 4) * nmain;                         // main
+    tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.ndt * pl.ksp;           // pass A
+    tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.ksp;                      // final
+  }
+  return tiles * (double)d.nq * d.nk * d.ntau * 2048.0;
+}
+
+template <int KSP_MAX, int NCT>
+static int launch_sigma(const s3::Plan &pl, const s3::Params &P, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(s3::sigma_kernel<KSP_MAX, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  if (e != cudaSuccess) return (int)e;
+  s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR, pl.smem, st>>>(P);
+  return (int)cudaGetLastError();
+}
+
+int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
+  s3::Plan pl = s3::make_plan(p);
+  if (!pl.ok) return GW_ESHAPE;
+  if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
+  s3::Params P;
+  P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
+  P.counter = (unsigned *)p->work;
+  P.scratch = (c128 *)((char *)p->work + 256);
+  P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt;
+  P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.slab_units = pl.slab_units;
+  cudaError_t e = cudaMemsetAsync(p->work, 0, 256, st);
+  if (e != cudaSuccess) return (int)e;
+  if (pl.nct == 2) {
+    if (pl.ksp_max == 7) return launch_sigma<7, 2>(pl, P, st);
+    if (pl.ksp_max == 13) return launch_sigma<13, 2>(pl, P, st);
+    return launch_sigma<16, 2>(pl, P, st);
+  } else {
+    if (pl.ksp_max == 7) return launch_sigma<7, 8>(pl, P, st);
+    if (pl.ksp_max == 13) return launch_sigma<13, 8>(pl, P, st);
+    return launch_sigma<16, 8>(pl, P, st);
+  }
+}

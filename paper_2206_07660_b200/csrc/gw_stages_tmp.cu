@@ -1,10 +1,8 @@
 // temporary: forward to the naive kernels until the optimised stages land
 #include "gw_common.cuh"
 int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *info, cudaStream_t st) { return gw_naive_stage2(p, P0t, Wt, p->work, p->work_bytes, info, st); }
-int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *S, cudaStream_t st) { return gw_naive_stage3(p, G, Wt, S, st); }
 int gw_launch_stage4(const gw_problem *p, const c128 *g, c128 *K, cudaStream_t st) { return gw_naive_stage4(p, g, K, st); }
 size_t gw_stage2_workspace(const gw_problem *p) { return 0; }
-size_t gw_stage3_workspace(const gw_problem *p) { return 0; }
 size_t gw_stage4_workspace(const gw_problem *p) { return 0; }
-void gw_stage_flops(const gw_problem *p, double *o) { o[0] = gw_stage1_flops(p); o[1] = o[2] = o[3] = 0; }
+void gw_stage_flops(const gw_problem *p, double *o) { o[0] = gw_stage1_flops(p); o[2] = gw_stage3_flops(p); o[1] = o[3] = 0; }
 int gw_stage_launches(const gw_problem *p) { return 6; }
