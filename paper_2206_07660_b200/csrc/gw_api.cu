@@ -48,7 +48,7 @@ extern "C" int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P
 extern "C" size_t gw_workspace_bytes(const gw_problem *p) {
   if (check_problem(p, false) != GW_OK) return 0;
   GwDims d = gw_dims(p);
-  size_t m = 2 * (size_t)d.nw * d.nq * d.naux * d.naux * sizeof(c128);   // debug reference kernels
+  size_t m = use_naive() ? 2 * (size_t)d.nw * d.nq * d.naux * d.naux * sizeof(c128) : 0;   // debug reference kernels only
   size_t s;
   if ((s = gw_stage1_workspace(p)) > m) m = s;
   if ((s = gw_stage2_workspace(p)) > m) m = s;

@@ -76,6 +76,7 @@ size_t gw_stage3_workspace(const gw_problem *p);
 size_t gw_stage4_workspace(const gw_problem *p);
 double gw_stage1_flops(const gw_problem *p);
 double gw_stage3_flops(const gw_problem *p);
+double gw_stage4_flops(const gw_problem *p);
 void gw_stage_flops(const gw_problem *p, double *out4);
 int gw_stage_launches(const gw_problem *p);
 

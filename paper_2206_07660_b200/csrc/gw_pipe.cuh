@@ -1,0 +1,137 @@
+// gw_pipe.cuh — building blocks shared by the stage kernels: cp.async stage jobs and complex-tile DMMA passes.
+// All kernels run 256 threads (8 warps) per CTA, one CTA per SM, with an NSTAGE-deep cp.async ring of stage buffers.
+#pragma once
+#include "gw_common.cuh"
+
+namespace gwp {
+
+constexpr int NTHR = 256, NSTAGE = 3;
+constexpr int PASS_ROWS = 64;   // rows per pass job: one 8-row m-tile per warp
+
+__device__ __forceinline__ void cp_async16_zfill(void *smem, const void *gmem, bool ok) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  int n = ok ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(n));
+}
+
+// rows [row0, row0+64) of a dense (rows x nao) matrix -> stage[r][ldp]
+__device__ __forceinline__ void issue_pass_job(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp) {
+  const int nrow = min(PASS_ROWS, rows_total - row0);
+  const int total = nrow * nao;
+  const c128 *s = src + (size_t)row0 * nao;
+  for (int i = threadIdx.x; i < total; i += NTHR) {
+    const int r = i / nao, a = i - r * nao;
+    cp_async16(stage + r * ldp + a, s + i);
+  }
+}
+
+// One pass job: this warp's m-tile (8 rows of a flat (Q,x) row index) times the nao x nao matrix held in sG as
+// [n][k] (K contiguous, zero padded):  out(row, n) = Σ_k stage[row][k] * sG[n][k].
+//   TRANSPOSED = true : row = (Q,x) -> out[(Q*nao + n)*nao + x]   (per-Q transpose)
+//   TRANSPOSED = false: out[row*nao + n]
+template <int KSP_MAX, bool TRANSPOSED>
+__device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
+                                             int nao, int ldp, int ksp, int ndt) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  if (row0 + 8 * w >= rows_total) return;   // whole m-tile beyond the panel (warp-uniform)
+  c128 a[KSP_MAX];
+#pragma unroll
+  for (int ks = 0; ks < KSP_MAX; ks++)
+    if (ks < ksp) a[ks] = sStage[(8 * w + g) * ldp + 4 * ks + c];
+  const int row = row0 + 8 * w + g;
+  const bool rok = row < rows_total;
+  int Q = 0, x = 0;
+  if (TRANSPOSED) { Q = row / nao; x = row - Q * nao; }
+  for (int nt = 0; nt < ndt; nt++) {
+    double cr[2] = {0.0, 0.0}, ci[2] = {0.0, 0.0};
+    const c128 *bp = sG + (8 * nt + g) * ldp + c;
+#pragma unroll
+    for (int ks = 0; ks < KSP_MAX; ks++)
+      if (ks < ksp) cmma(cr, ci, a[ks], bp[4 * ks]);
+    const int col = 8 * nt + 2 * c;
+    if (rok) {
+      if (TRANSPOSED) {
+        if (col < nao) out[((size_t)Q * nao + col) * nao + x] = make_double2(cr[0], ci[0]);
+        if (col + 1 < nao) out[((size_t)Q * nao + col + 1) * nao + x] = make_double2(cr[1], ci[1]);
+      } else {
+        if (col < nao) out[(size_t)row * nao + col] = make_double2(cr[0], ci[0]);
+        if (col + 1 < nao) out[(size_t)row * nao + col + 1] = make_double2(cr[1], ci[1]);
+      }
+    }
+  }
+}
+
+// "final" job for one Q: A = Aq (nao x nao, [i][a]) -> stage[i][ldp]; B = Bq (nao x nao, [a][j]) -> [a][ldt], rows a >= nao zero
+__device__ __forceinline__ void issue_final_job(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop) {
+  const int n2 = nao * nao;
+  for (int i = threadIdx.x; i < n2; i += NTHR) {
+    const int r = i / nao, a = i - r * nao;
+    cp_async16(stage + r * ldp + a, Aq + i);
+  }
+  c128 *sB = stage + naop * ldp;
+  const int rowsB = 4 * ksp;
+  for (int i = threadIdx.x; i < rowsB * nao; i += NTHR) {
+    const int r = i / nao;
+    const bool ok = r < nao;
+    cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + i : Bq, ok);
+  }
+}
+
+// acc[i][j] += Σ_a A[i][a] B[a][j] for the output tiles owned by this warp (tile = w + 8*ti over an ndt x ndt grid)
+template <int NCT>
+__device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[NCT][2], double (&sgi)[NCT][2], int ldp, int ldt,
+                                              int ksp, int ndt, int naop) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  const c128 *sA = stage, *sB = stage + naop * ldp;
+#pragma unroll
+  for (int ti = 0; ti < NCT; ti++) {
+    const int tile = w + 8 * ti;
+    if (tile < ndt * ndt) {
+      const int mi = tile / ndt, nj = tile - mi * ndt;
+      const c128 *ap = sA + (8 * mi + g) * ldp + c;
+      const c128 *bp = sB + c * ldt + 8 * nj + g;
+      for (int ks = 0; ks < ksp; ks++) cmma(sgr[ti], sgi[ti], ap[4 * ks], bp[4 * ks * ldt]);
+    }
+  }
+}
+
+// store the warp-owned tiles of an nao x nao result, scaled
+template <int NCT>
+__device__ __forceinline__ void final_store(c128 *out, const double (&sgr)[NCT][2], const double (&sgi)[NCT][2], double pref, int nao, int ndt) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+#pragma unroll
+  for (int ti = 0; ti < NCT; ti++) {
+    const int tile = w + 8 * ti;
+    if (tile < ndt * ndt) {
+      const int mi = tile / ndt, nj = tile - mi * ndt;
+      const int i = 8 * mi + g, j = 8 * nj + 2 * c;
+      if (i < nao) {
+        if (j < nao) out[i * nao + j] = make_double2(pref * sgr[ti][0], pref * sgi[ti][0]);
+        if (j + 1 < nao) out[i * nao + j + 1] = make_double2(pref * sgr[ti][1], pref * sgi[ti][1]);
+      }
+    }
+  }
+}
+
+// pass-geometry shared by the stages
+struct PassGeom { int ldp, ksp, ksp_max, ndt, naop, ldt, nct; bool ok; };
+static inline PassGeom pass_geom(int nao) {
+  PassGeom g;
+  g.ksp = (nao + 3) / 4;
+  g.ok = g.ksp <= 16;
+  g.ksp_max = g.ksp <= 7 ? 7 : (g.ksp <= 13 ? 13 : 16);
+  g.ndt = (nao + 7) / 8;
+  g.naop = 8 * g.ndt;
+  int r4 = g.ksp * 4; if (r4 % 8 == 0) r4 += 4;   // ≡ 4 (mod 8): conflict-free K-contiguous fragments
+  g.ldp = r4;
+  g.ldt = g.naop + 2;                              // ≡ 2 (mod 8): conflict-free K-major fragments
+  g.nct = (g.ndt * g.ndt + 7) / 8 <= 2 ? 2 : 8;
+  return g;
+}
+static inline int gw_num_sms() {
+  int dev = 0, nsm = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) { cudaGetLastError(); nsm = 148; }
+  return nsm;
+}
+
+}  // namespace gwp

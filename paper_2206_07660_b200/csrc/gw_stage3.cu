@@ -9,12 +9,12 @@
 // A persistent CTA owns one (t,k): it loops over q and over Q panels, and keeps the nao x nao Sigma accumulator in
 // registers for the whole item, so the q-sum needs no cross-CTA reduction and the result is deterministic.
 // U and T live in two per-CTA slabs of the workspace (L2 resident); the raw V2 block is the only big stream.
-#include "gw_common.cuh"
+#include "gw_pipe.cuh"
 
 namespace s3 {
 
-constexpr int NTHR = 256, NSTAGE = 3;
-constexpr int PASS_ROWS = 64, KC = 8, MT_W = 2, NJ = 7, TM = 32;
+using gwp::NTHR; using gwp::NSTAGE; using gwp::PASS_ROWS;
+constexpr int KC = 8, MT_W = 2, NJ = 7, TM = 32;
 
 struct Params {
   GwDims d;
@@ -30,21 +30,7 @@ struct Params {
   size_t slab_units;      // complex elements per slab (two slabs per CTA)
 };
 
-__device__ __forceinline__ void cp_async16_zfill(void *smem, const void *gmem, bool ok) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  int n = ok ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(n));
-}
-
-__device__ __forceinline__ void issue_pass_job(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp) {
-  const int nrow = min(PASS_ROWS, rows_total - row0);
-  const int total = nrow * nao;
-  const c128 *s = src + (size_t)row0 * nao;
-  for (int i = threadIdx.x; i < total; i += NTHR) {
-    const int r = i / nao, a = i - r * nao;
-    cp_async16(stage + r * ldp + a, s + i);
-  }
-}
+using gwp::cp_async16_zfill; using gwp::issue_pass_job; using gwp::issue_final_job;
 
 // main job: A = W[tm rows][k0..k0+8) swizzled; B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
 __device__ __forceinline__ void issue_main_job(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
@@ -63,49 +49,6 @@ __device__ __forceinline__ void issue_main_job(c128 *stage, const c128 *W, int t
   }
 }
 
-// final job for one Q: A = V1[Q] as [i][ldp]; B = T[Q] as [a][ldt] with rows a >= nao zero-filled
-__device__ __forceinline__ void issue_final_job(c128 *stage, const c128 *V1Q, const c128 *TQ, int nao, int ldp, int ldt, int ksp, int naop) {
-  const int n2 = nao * nao;
-  for (int i = threadIdx.x; i < n2; i += NTHR) {
-    const int r = i / nao, a = i - r * nao;
-    cp_async16(stage + r * ldp + a, V1Q + i);
-  }
-  c128 *sB = stage + naop * ldp;
-  const int rowsB = 4 * ksp;
-  for (int i = threadIdx.x; i < rowsB * nao; i += NTHR) {
-    const int r = i / nao, j = i - r * nao;
-    const bool ok = r < nao;
-    cp_async16_zfill(sB + r * ldt + j, ok ? TQ + i : TQ, ok);
-  }
-}
-
-// pass A: rows (Q,j) of Ut times G^T: out T[(Q*nao + a)*nao + j]
-template <int KSP_MAX>
-__device__ __forceinline__ void passA_compute(const c128 *sStage, const c128 *sG, c128 *slabT, int row0, int rows_total,
-                                              int nao, int ldp, int ksp, int ndt) {
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
-  if (row0 + 8 * w >= rows_total) return;
-  c128 a[KSP_MAX];
-#pragma unroll
-  for (int ks = 0; ks < KSP_MAX; ks++)
-    if (ks < ksp) a[ks] = sStage[(8 * w + g) * ldp + 4 * ks + c];
-  const int row = row0 + 8 * w + g;
-  const bool rok = row < rows_total;
-  const int Q = row / nao, j = row - Q * nao;
-  for (int nt = 0; nt < ndt; nt++) {
-    double cr[2] = {0.0, 0.0}, ci[2] = {0.0, 0.0};
-    const c128 *bp = sG + (8 * nt + g) * ldp + c;
-#pragma unroll
-    for (int ks = 0; ks < KSP_MAX; ks++)
-      if (ks < ksp) cmma(cr, ci, a[ks], bp[4 * ks]);
-    const int col = 8 * nt + 2 * c;   // a index
-    if (rok) {
-      if (col < nao) slabT[((size_t)Q * nao + col) * nao + j] = make_double2(cr[0], ci[0]);
-      if (col + 1 < nao) slabT[((size_t)Q * nao + col + 1) * nao + j] = make_double2(cr[1], ci[1]);
-    }
-  }
-}
-
 template <int KSP_MAX, int NCT>
 __global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -121,7 +64,6 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
   c128 *slabU = P.scratch + (size_t)blockIdx.x * 2 * P.slab_units;
   c128 *slabT = slabU + P.slab_units;
   const size_t vb = (size_t)naux * n2;
-  const int ntiles_out = ndt * ndt;
 
   {
     const int tot = naop * ldp + NSTAGE * P.stage_units;
@@ -232,7 +174,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
             const int nx = jb + NSTAGE - 1;
             if (nx < npass) issue_pass_job(sStage + (nx % NSTAGE) * P.stage_units, slabU, nx * PASS_ROWS, rows, nao, ldp);
             cp_async_commit();
-            passA_compute<KSP_MAX>(sStage + (jb % NSTAGE) * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
+            gwp::pass_compute<KSP_MAX, true>(sStage + (jb % NSTAGE) * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
           }
           cp_async_wait<0>();
           __syncthreads();
@@ -251,18 +193,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
             const int nx = jb + NSTAGE - 1;
             if (nx < tm_rows) issue_final_job(sStage + (nx % NSTAGE) * P.stage_units, V1t + (size_t)nx * n2, slabT + (size_t)nx * n2, nao, ldp, P.ldt, P.ksp, naop);
             cp_async_commit();
-            const c128 *sA = sStage + (jb % NSTAGE) * P.stage_units;
-            const c128 *sB = sA + naop * ldp;
-#pragma unroll
-            for (int ti = 0; ti < NCT; ti++) {
-              const int tile = w + 8 * ti;
-              if (tile < ntiles_out) {
-                const int mi = tile / ndt, nj = tile - mi * ndt;
-                const c128 *ap = sA + (8 * mi + g) * ldp + c;
-                const c128 *bp = sB + c * P.ldt + 8 * nj + g;
-                for (int ks = 0; ks < P.ksp; ks++) cmma(sgr[ti], sgi[ti], ap[4 * ks], bp[4 * ks * P.ldt]);
-              }
-            }
+            gwp::final_compute<NCT>(sStage + (jb % NSTAGE) * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
           }
           cp_async_wait<0>();
           __syncthreads();
@@ -272,18 +203,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
     // ---- epilogue ----
     const double pref = -1.0 / (double)d.nk;
     c128 *out = P.Sigma + ((size_t)t * d.nk + k) * n2;
-#pragma unroll
-    for (int ti = 0; ti < NCT; ti++) {
-      const int tile = w + 8 * ti;
-      if (tile < ntiles_out) {
-        const int mi = tile / ndt, nj = tile - mi * ndt;
-        const int i = 8 * mi + g, j = 8 * nj + 2 * c;
-        if (i < nao) {
-          if (j < nao) out[i * nao + j] = make_double2(pref * sgr[ti][0], pref * sgi[ti][0]);
-          if (j + 1 < nao) out[i * nao + j + 1] = make_double2(pref * sgr[ti][1], pref * sgi[ti][1]);
-        }
-      }
-    }
+    gwp::final_store<NCT>(out, sgr, sgi, pref, nao, ndt);
   }
 }
 

@@ -1,0 +1,178 @@
+// gw_stage4.cu — stage 4, static exchange, Eq. 22:
+//
+//   K[k][i][j] = -(1/N_k) Σ_k' Σ_Q Σ_ab V[k][k'][Q][i][a] gamma[k'][a][b] V[k'][k][Q][b][j]
+//
+// Per (k,k') pair, with V1 = V[k][k'], V2 = V[k'][k] (each V block is read exactly once per call):
+//   pass :  X[Q][i][b]  = Σ_a V1[Q][i][a] gamma[k'][a][b]          rows (Q,i) flat, K = nao
+//   final:  part[i][j] += Σ_(Q,b) X[Q][i][b] V2[Q][b][j]            K = (Q,b)
+// One persistent CTA per (k, q = k-k') item keeps the nao x nao partial in registers over all Q, writes it to the
+// workspace, and a second kernel sums the partials over q in a fixed order (deterministic, no atomics).
+#include "gw_pipe.cuh"
+
+namespace s4 {
+
+using gwp::NTHR; using gwp::NSTAGE; using gwp::PASS_ROWS;
+constexpr int TM = 32;
+
+struct Params {
+  GwDims d;
+  const c128 *V, *gamma;
+  c128 *part, *scratch;
+  unsigned *counter;
+  int nitems, ldp, ksp, ndt, ldt, stage_units;
+  size_t slab_units;
+};
+
+template <int KSP_MAX, int NCT>
+__global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  c128 *smem = reinterpret_cast<c128 *>(smem_raw);
+  const GwDims d = P.d;
+  const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, ndt = P.ndt, naop = 8 * ndt;
+  c128 *sGt = smem;                   // [naop][ldp]: sGt[b][a] = gamma[k'][a][b]
+  c128 *sStage = sGt + naop * ldp;
+  __shared__ int s_item;
+  c128 *slab = P.scratch + (size_t)blockIdx.x * P.slab_units;
+  const size_t vb = (size_t)naux * n2;
+  {
+    const int tot = naop * ldp + NSTAGE * P.stage_units;
+    for (int i = threadIdx.x; i < tot; i += NTHR) smem[i] = make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+  for (;;) {
+    if (threadIdx.x == 0) s_item = (int)atomicAdd(P.counter, 1u);
+    __syncthreads();
+    const int item = s_item;
+    __syncthreads();
+    if (item >= P.nitems) break;
+    const int ql = item % d.nq, k = item / d.nq;
+    const int kp = gw_ksub(d, k, d.q0 + ql);
+    const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb, *V2 = P.V + ((size_t)kp * d.nk + k) * vb;
+    const c128 *gm = P.gamma + (size_t)kp * n2;
+    for (int i = threadIdx.x; i < n2; i += NTHR) { const int r = i / nao, cc = i - r * nao; sGt[cc * ldp + r] = gm[i]; }
+    double sgr[NCT][2], sgi[NCT][2];
+#pragma unroll
+    for (int i = 0; i < NCT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+    for (int Q0 = 0; Q0 < naux; Q0 += TM) {
+      const int tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
+      const c128 *V1t = V1 + (size_t)Q0 * n2, *V2t = V2 + (size_t)Q0 * n2;
+      int issued = 0;
+      for (; issued < NSTAGE - 1; issued++) {
+        if (issued < npass) gwp::issue_pass_job(sStage + (issued % NSTAGE) * P.stage_units, V1t, issued * PASS_ROWS, rows, nao, ldp);
+        cp_async_commit();
+      }
+      for (int jb = 0; jb < npass; jb++) {
+        cp_async_wait<NSTAGE - 2>();
+        __syncthreads();
+        const int nx = jb + NSTAGE - 1;
+        if (nx < npass) gwp::issue_pass_job(sStage + (nx % NSTAGE) * P.stage_units, V1t, nx * PASS_ROWS, rows, nao, ldp);
+        cp_async_commit();
+        gwp::pass_compute<KSP_MAX, false>(sStage + (jb % NSTAGE) * P.stage_units, sGt, slab, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
+      }
+      cp_async_wait<0>();
+      __syncthreads();
+      for (issued = 0; issued < NSTAGE - 1; issued++) {
+        if (issued < tm_rows) gwp::issue_final_job(sStage + (issued % NSTAGE) * P.stage_units, slab + (size_t)issued * n2, V2t + (size_t)issued * n2, nao, ldp, P.ldt, P.ksp, naop);
+        cp_async_commit();
+      }
+      for (int jb = 0; jb < tm_rows; jb++) {
+        cp_async_wait<NSTAGE - 2>();
+        __syncthreads();
+        const int nx = jb + NSTAGE - 1;
+        if (nx < tm_rows) gwp::issue_final_job(sStage + (nx % NSTAGE) * P.stage_units, slab + (size_t)nx * n2, V2t + (size_t)nx * n2, nao, ldp, P.ldt, P.ksp, naop);
+        cp_async_commit();
+        gwp::final_compute<NCT>(sStage + (jb % NSTAGE) * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
+      }
+      cp_async_wait<0>();
+      __syncthreads();
+    }
+    gwp::final_store<NCT>(P.part + ((size_t)ql * d.nk + k) * n2, sgr, sgi, 1.0, nao, ndt);
+  }
+}
+
+// K[k] = -(1/N_k) Σ_ql part[ql][k]   (fixed summation order)
+__global__ void exchange_reduce_kernel(GwDims d, const c128 *__restrict__ part, c128 *__restrict__ K) {
+  const size_t n = (size_t)d.nk * d.nao * d.nao;
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double re = 0.0, im = 0.0;
+  for (int ql = 0; ql < d.nq; ql++) { const c128 v = part[(size_t)ql * n + i]; re += v.x; im += v.y; }
+  const double pref = -1.0 / (double)d.nk;
+  K[i] = make_double2(pref * re, pref * im);
+}
+
+struct Plan { gwp::PassGeom g; int nitems, stage_units, grid; size_t smem, slab_units, part_units, work_bytes; bool ok; };
+
+static Plan make_plan(const gw_problem *p) {
+  Plan pl; memset(&pl, 0, sizeof(pl));
+  GwDims d = gw_dims(p);
+  pl.g = gwp::pass_geom(d.nao);
+  if (!pl.g.ok) { pl.ok = false; return pl; }
+  pl.nitems = d.nk * d.nq;
+  int s_pass = PASS_ROWS * pl.g.ldp, s_fin = pl.g.naop * pl.g.ldp + 4 * pl.g.ksp * pl.g.ldt + 8;
+  pl.stage_units = s_pass > s_fin ? s_pass : s_fin;
+  pl.smem = ((size_t)pl.g.naop * pl.g.ldp + (size_t)NSTAGE * pl.stage_units) * sizeof(c128);
+  const int nsm = gwp::gw_num_sms();
+  pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
+  pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
+  pl.part_units = (size_t)d.nq * d.nk * d.nao * d.nao;
+  pl.work_bytes = 256 + ((size_t)nsm * pl.slab_units + pl.part_units) * sizeof(c128);
+  pl.ok = pl.smem <= 227 * 1024;
+  return pl;
+}
+
+}  // namespace s4
+
+size_t gw_stage4_workspace(const gw_problem *p) {
+  s4::Plan pl = s4::make_plan(p);
+  return pl.ok ? pl.work_bytes : 0;
+}
+
+double gw_stage4_flops(const gw_problem *p) {
+  s4::Plan pl = s4::make_plan(p);
+  if (!pl.ok) return 0.0;
+  GwDims d = gw_dims(p);
+  double tiles = 0.0;
+  for (int Q0 = 0; Q0 < d.naux; Q0 += s4::TM) {
+    const int tm_rows = (d.naux - Q0) < s4::TM ? (d.naux - Q0) : s4::TM;
+    tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.g.ndt * pl.g.ksp + (double)tm_rows * pl.g.ndt * pl.g.ndt * pl.g.ksp;
+  }
+  return tiles * (double)d.nk * d.nq * 2048.0;
+}
+
+template <int KSP_MAX, int NCT>
+static int launch_exchange(const s4::Plan &pl, const s4::Params &P, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(s4::exchange_kernel<KSP_MAX, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  if (e != cudaSuccess) return (int)e;
+  s4::exchange_kernel<KSP_MAX, NCT><<<pl.grid, s4::NTHR, pl.smem, st>>>(P);
+  return (int)cudaGetLastError();
+}
+
+int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st) {
+  s4::Plan pl = s4::make_plan(p);
+  if (!pl.ok) return GW_ESHAPE;
+  if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
+  s4::Params P;
+  P.d = gw_dims(p); P.V = (const c128 *)p->V; P.gamma = gamma;
+  P.counter = (unsigned *)p->work;
+  P.scratch = (c128 *)((char *)p->work + 256);
+  P.part = P.scratch + (size_t)gwp::gw_num_sms() * pl.slab_units;
+  P.nitems = pl.nitems; P.ldp = pl.g.ldp; P.ksp = pl.g.ksp; P.ndt = pl.g.ndt; P.ldt = pl.g.ldt;
+  P.stage_units = pl.stage_units; P.slab_units = pl.slab_units;
+  cudaError_t e = cudaMemsetAsync(p->work, 0, 256, st);
+  if (e != cudaSuccess) return (int)e;
+  int rc;
+  if (pl.g.nct == 2) {
+    if (pl.g.ksp_max == 7) rc = launch_exchange<7, 2>(pl, P, st);
+    else if (pl.g.ksp_max == 13) rc = launch_exchange<13, 2>(pl, P, st);
+    else rc = launch_exchange<16, 2>(pl, P, st);
+  } else {
+    if (pl.g.ksp_max == 7) rc = launch_exchange<7, 8>(pl, P, st);
+    else if (pl.g.ksp_max == 13) rc = launch_exchange<13, 8>(pl, P, st);
+    else rc = launch_exchange<16, 8>(pl, P, st);
+  }
+  if (rc) return rc;
+  const size_t n = (size_t)P.d.nk * P.d.nao * P.d.nao;
+  s4::exchange_reduce_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(P.d, P.part, K);
+  return (int)cudaGetLastError();
+}
