@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py — one scGW iteration's self-energy build (Algorithm 1 + Eq. 22) on N B200s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path — gw_polarization, gw_screened_interaction, gw_selfenergy, gw_exchange
+ — over one synthetic problem whose inputs are resident in HBM.  Rank 0 prints ONE JSON line.
+Metric (BASELINE.json): Σ-build seconds per iteration (lower is better) with the FP64 TFLOP/s it corresponds to and the
+fraction of the measured B200 FP64 tensor-core peak.  See DESIGN.md "Measurement".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="2", help="gwgen config name (BASELINE.json configs 0-4); default 2")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=None)
+    return ap.parse_args()
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: mesh {cfg.mesh[0]}x{cfg.mesh[1]}x{cfg.mesh[2]} (nk={cfg.nk}), nao={cfg.nao}, naux={cfg.naux}, "
+            f"ntau=nw={cfg.ntau}, beta={cfg.beta:g}")
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# CPU baseline = the oracle as it stands, on a bounded sample of the same workload, extrapolated to one iteration
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, n_slices=None, want_detail=False):
+    """Times oracle slices of every stage on the host cores and extrapolates to seconds per full iteration.
+
+    Sample: n stage-1 (q,t) slices at one q, n stage-3 (k,t) slices at one k, stage 2 for one q, stage 4 for one k,
+    the slices run concurrently on `cores` threads (the oracle's own OpenMP loops run over exactly these slice calls).
+    Inputs: the same seeded generator as the GPU arm (only the V blocks the slices touch are generated).
+    """
+    import concurrent.futures as cf
+    import gwgen
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    n = n_slices or cores
+    mesh = gwgen.KMesh(cfg.mesh)
+    gr = gwgen.make_grids(cfg.ntau, cfg.nw, cfg.beta)
+    eps, U = gwgen.make_fock(cfg, mesh)
+    G = gwgen.greens_function(eps, U, gr["tau"], cfg.beta)
+    gamma = gwgen.density_matrix(eps, U, cfg.beta)
+    rng = np.random.default_rng(12345)
+    q = int(rng.integers(cfg.nk)); k = int(rng.integers(cfg.nk))
+    add, sub = mesh.add_table(), mesh.sub_table()
+    need = set()
+    for kk in range(cfg.nk):
+        need.add((kk, int(add[kk][q]))); need.add((int(add[kk][q]), kk))
+        need.add((k, int(sub[k][kk]))); need.add((int(sub[k][kk]), k))
+    blocks = {b: gwgen.make_V_block(cfg, mesh, b[0], b[1]).numpy() for b in sorted(need)}
+    vb = oracle.VBlocks(cfg, blocks)
+    ts = [int(x) for x in rng.choice(cfg.ntau, size=min(n, cfg.ntau), replace=False)]
+    pool = cf.ThreadPoolExecutor(max_workers=cores)
+    t0 = time.perf_counter()
+    p0 = list(pool.map(lambda t: oracle.p0t_slice(cfg, vb, G[t], G[cfg.ntau - 1 - t], q), ts))
+    t1 = time.perf_counter()
+    # stage 2 for one q on a synthetic-but-representative P0t_q: reuse the computed slices cyclically
+    P0t_q = np.stack([p0[i % len(p0)] for i in range(cfg.ntau)])
+    Wt_q = oracle.screened_interaction_q(cfg, gr["T_wt"], gr["T_tw"], P0t_q)
+    t2 = time.perf_counter()
+    Wt_t = np.ascontiguousarray(np.broadcast_to(Wt_q[0], (cfg.nk, cfg.naux, cfg.naux)))
+    sg = list(pool.map(lambda t: oracle.sigma_slice(cfg, vb, G[t], Wt_t, k), ts))
+    t3 = time.perf_counter()
+    oracle.exchange_slice(cfg, vb, gamma, k)
+    t4 = time.perf_counter()
+    pool.shutdown()
+    ns = len(ts)
+    full = ((t1 - t0) * cfg.ntau * cfg.nk / ns            # stage 1: ntau*nk slices, ns of them ran concurrently
+            + (t2 - t1) * cfg.nk / min(cores, cfg.nk)     # stage 2: nk q-points over the cores
+            + (t3 - t2) * cfg.ntau * cfg.nk / ns          # stage 3
+            + (t4 - t3) * cfg.nk / min(cores, cfg.nk))    # stage 4
+    detail = {"stage1_s": t1 - t0, "stage2_s": t2 - t1, "stage3_s": t3 - t2, "stage4_s": t4 - t3, "slices": ns}
+    sample = (f"{ns} stage-1 (q,t) slices + stage 2 for 1 q + {ns} stage-3 (k,t) slices + stage 4 for 1 k of {cfg.name}, "
+              f"run concurrently on {cores} threads; seconds/iteration extrapolated = slice time x number of slices")
+    return full, cores, sample, detail
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (tier framing: the oracle is the reference arm)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import gwgen
+    cfg = gwgen.get_config(args.config)
+    for _ in range(max(args.warmup, 0)):
+        oracle_sample(cfg, n_slices=2)
+    vals = []
+    t0 = time.perf_counter()
+    for _ in range(max(args.steps, 1)):
+        full, cores, sample, _ = oracle_sample(cfg)
+        vals.append(full)
+    wall = time.perf_counter() - t0
+    v = float(np.mean(vals))
+    nom = cfg.flops_nominal()["total"]
+    out = {"impl": "reference", "metric": "sigma_build_seconds_per_iteration", "value": v, "unit": "s", "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": v * 1e3, "higher_is_better": False,
+           "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(cfg), "note": "extrapolated from a bounded sample per step"},
+           "tflops_nominal": nom / v * 1e-12,
+           "cpu_baseline": {"value": v, "unit": "s", "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "sample_wall_s": wall}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                          "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t_begin, t_end):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            if ts < t_begin or ts > t_end:
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except Exception:
+                continue
+            for nme, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# dram traffic per launch of the dominant kernel from the committed ncu capture (profiles/), keyed by config; None = not captured
+NCU_TRAFFIC_BYTES = {}
+
+
+def run_ours(args):
+    import torch
+    import gwgen
+    import paper_2206_07660_b200 as gw
+    from paper_2206_07660_b200.dist import shard_range, allreduce_sum_
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = gwgen.get_config(args.config)
+    nom = cfg.flops_nominal()
+
+    # ---- synthetic inputs, resident in HBM (generation is not timed) ----
+    p = gwgen.make_problem(cfg, v_device=dev)
+    q0, q1 = shard_range(cfg.nk, world, rank)
+    prob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, p.V, torch.from_numpy(p.T_wt).to(dev),
+                        torch.from_numpy(p.T_tw).to(dev), cfg.spin_deg, q0, q1)
+    G = torch.from_numpy(p.G).to(dev)
+    gamma = torch.from_numpy(p.gamma).to(dev)
+    nq = q1 - q0
+    P = torch.empty((cfg.ntau, nq, cfg.naux, cfg.naux), dtype=torch.complex128, device=dev)   # P0t, then Wt in place
+    Sigma = torch.empty_like(G)
+    K = torch.empty_like(gamma)
+    info = torch.zeros(2, dtype=torch.int32, device=dev)
+    peak = gw.gw_fp64_peak(300.0)
+    executed = gw.gw_executed_flops(prob)
+    launches = gw.gw_launch_count(prob)
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        if ev: ev[0].record(stream)
+        gw.gw_polarization(prob, G, P, stream)
+        if ev: ev[1].record(stream)
+        gw.gw_screened_interaction(prob, P, P, info, stream)
+        if ev: ev[2].record(stream)
+        gw.gw_selfenergy(prob, G, P, Sigma, stream)
+        if ev: ev[3].record(stream)
+        gw.gw_exchange(prob, gamma, K, stream)
+        if ev: ev[4].record(stream)
+        if world > 1:
+            allreduce_sum_([Sigma, K])
+        if ev: ev[5].record(stream)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+    t_begin = time.perf_counter()
+    for s in range(args.steps):
+        step(evs[s])
+    barrier()
+    t_end = time.perf_counter()
+    clocks = sampler.stop(t_begin, t_end) if sampler else None
+    total_ms = evs[0][0].elapsed_time(evs[-1][5])
+    stage_ms = [float(np.mean([evs[s][i].elapsed_time(evs[s][i + 1]) for s in range(args.steps)])) for i in range(5)]
+    if world > 1:
+        import torch.distributed as dist
+        tt = torch.tensor([total_ms] + stage_ms, dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms, stage_ms = float(tt[0]), [float(x) for x in tt[1:]]
+    ms_per_step = total_ms / args.steps
+    info_host = info.cpu().tolist()
+
+    # ---- e2e: the same iteration through the C ABI with HOST buffers (copies inside the timed region) ----
+    e2e = None
+    h2d = cfg.bytes_V() + (G.numel() + gamma.numel() + 2 * cfg.nw * cfg.ntau) * 16
+    d2h = (Sigma.numel() + K.numel()) * 16
+    if not args.no_e2e and world == 1:
+        hV = torch.empty(p.V.shape, dtype=torch.complex128, pin_memory=True); hV.copy_(p.V)
+        hG = torch.from_numpy(p.G).pin_memory(); hg = torch.from_numpy(p.gamma).pin_memory()
+        hTw = torch.from_numpy(p.T_wt).pin_memory(); hTt = torch.from_numpy(p.T_tw).pin_memory()
+        hS = torch.empty(G.shape, dtype=torch.complex128, pin_memory=True)
+        hK = torch.empty(gamma.shape, dtype=torch.complex128, pin_memory=True)
+        Sig_dev_check = Sigma.cpu()
+        del P, Sigma, K, prob, G, gamma
+        p.V = None
+        torch.cuda.empty_cache()
+        hprob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, hV, hTw, hTt, cfg.spin_deg)
+        n_e2e = args.e2e_steps if args.e2e_steps is not None else min(args.steps, 2)
+        gw.gw_sigma_iteration_host(hprob, hG, hg, hS, hK)          # warm-up (context, allocator)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            r = gw.gw_sigma_iteration_host(hprob, hG, hg, hS, hK)
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        same = bool(torch.equal(hS, Sig_dev_check))
+        e2e = {"value": e2e_s, "unit": "s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": n_e2e,
+               "stage_ms": [round(x, 3) for x in r["stage_ms"]], "matches_device_resident_run": same}
+
+    if rank != 0:
+        return 0
+    # ---- roofline of the dominant kernel (stage 3's sigma_kernel or stage 1's p0_kernel, whichever is longer) ----
+    dom = 2 if stage_ms[2] >= stage_ms[0] else 0
+    dom_name = {0: "s1::p0_kernel (stage 1, Eq. 28b)", 2: "s3::sigma_kernel (stage 3, Eq. 31)"}[dom]
+    alg_flops = (nom["stage3"] if dom == 2 else nom["stage1"]) * nq / cfg.nk
+    achieved = alg_flops / (stage_ms[dom] * 1e-3) * 1e-12
+    roof = {"bound": "tensor", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+            "peak_source": "measured in this run: register-resident DMMA.8x8x4 loop on all SMs (gw_fp64_peak); "
+                           "MEASURED_PEAKS.json has no FP64 entry",
+            "flops": "algorithmic (Algorithm 1 literal, 8 flops per complex multiply-add); executed/algorithmic = %.3f"
+                     % (executed[dom] / alg_flops),
+            "achieved_executed": executed[dom] / (stage_ms[dom] * 1e-3) * 1e-12}
+    total_nom = nom["total"]
+    out = {"metric": "sigma_build_seconds_per_iteration", "value": ms_per_step * 1e-3, "unit": "s", "n_gpus": world,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
+           "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(cfg), "parallelism": f"q-shard x{world}", "l2": "inputs_larger_than_l2" if cfg.bytes_V() > 200e6 else "inputs_smaller_than_l2_no_flush",
+                      "V_bytes": cfg.bytes_V()},
+           "tflops_nominal": total_nom / (ms_per_step * 1e-3) * 1e-12,
+           "tflops_executed_per_gpu": sum(executed) / (ms_per_step * 1e-3) * 1e-12,
+           "frac_of_fp64_peak_nominal": total_nom / (ms_per_step * 1e-3) * 1e-12 / peak / world,
+           "fp64_peak_tflops_measured": peak,
+           "stage_ms": {"polarization": stage_ms[0], "screened_interaction": stage_ms[1], "selfenergy": stage_ms[2],
+                        "exchange": stage_ms[3], "allreduce": stage_ms[4]},
+           "roofline": roof, "gpu_launches": launches * args.steps,
+           "clocks": clocks, "info": info_host}
+    if e2e is not None:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        full, cores, sample, _ = oracle_sample(cfg)
+        out["cpu_baseline"] = {"value": full, "unit": "s", "cores": cores, "kind": "oracle", "sample": sample}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

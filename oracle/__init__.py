@@ -36,7 +36,8 @@ def lib():
         _lib.gwref_num_threads.restype = ctypes.c_int
         for name in ("gwref_kadd", "gwref_ksub", "gwref_p0t_slice", "gwref_polarization", "gwref_dyson",
                      "gwref_screened_interaction_q", "gwref_screened_interaction", "gwref_sigma_slice",
-                     "gwref_selfenergy", "gwref_exchange_slice", "gwref_exchange"):
+                     "gwref_selfenergy", "gwref_exchange_slice", "gwref_exchange", "gwref_sigma_slice_qrange",
+                     "gwref_exchange_slice_qrange"):
             getattr(_lib, name).restype = ctypes.c_int
         _lib.gwref_transform.restype = None
     return _lib
@@ -138,11 +139,13 @@ def screened_interaction(cfg, T_wt, T_tw, P0t, want_freq=False):
     return (Wt, P0w, Ww) if want_freq else Wt
 
 
-def sigma_slice(cfg, vb, G_t, Wt_t, k):
-    """Eq. 31 for one (k, tau_t).  G_t: [nk][nao][nao], Wt_t: [nk][naux][naux]."""
+def sigma_slice(cfg, vb, G_t, Wt_t, k, q_begin=0, q_end=None):
+    """Eq. 31 for one (k, tau_t).  G_t: [nk][nao][nao], Wt_t: [nk][naux][naux] (indexed by the global q).
+    q_begin/q_end restrict the q sum (one rank's partial sum)."""
     out = np.empty((cfg.nao, cfg.nao), np.complex128)
     d = _dims(cfg)
-    if lib().gwref_sigma_slice(ctypes.byref(d), vb.table, _p(G_t), _p(Wt_t), int(k), _p(out)):
+    q_end = cfg.nk if q_end is None else q_end
+    if lib().gwref_sigma_slice_qrange(ctypes.byref(d), vb.table, _p(G_t), _p(Wt_t), int(k), int(q_begin), int(q_end), _p(out)):
         raise RuntimeError("oracle: a needed V block is not resident")
     return out
 
@@ -155,10 +158,11 @@ def selfenergy(cfg, vb, G, Wt):
     return out
 
 
-def exchange_slice(cfg, vb, gamma, k):
+def exchange_slice(cfg, vb, gamma, k, q_begin=0, q_end=None):
     out = np.empty((cfg.nao, cfg.nao), np.complex128)
     d = _dims(cfg)
-    if lib().gwref_exchange_slice(ctypes.byref(d), vb.table, _p(gamma), int(k), _p(out)):
+    q_end = cfg.nk if q_end is None else q_end
+    if lib().gwref_exchange_slice_qrange(ctypes.byref(d), vb.table, _p(gamma), int(k), int(q_begin), int(q_end), _p(out)):
         raise RuntimeError("oracle: a needed V block is not resident")
     return out
 

@@ -224,14 +224,21 @@ int gwref_screened_interaction(const gwref_dims *d, const c128 *T_wt, const c128
 /* ---- Eq. 31, one (k, tau_t):
  *   Sigma[i][j] = -(1/N_k) sum_q sum_ab sum_QQ' G^{k-q}_{ab}(tau) V^{k,k-q}_{ia}(Q) P~^{q}_{QQ'}(tau) V^{k-q,k}_{bj}(Q')
  * G_t: [nk][nao][nao], Wt_t: [nk][naux][naux] at the same tau node. */
+int gwref_sigma_slice_qrange(const gwref_dims *d, const c128 *const *Vblk, const c128 *G_t, const c128 *Wt_t, int k,
+                             int q_begin, int q_end, c128 *out);
 int gwref_sigma_slice(const gwref_dims *d, const c128 *const *Vblk, const c128 *G_t, const c128 *Wt_t, int k, c128 *out) {
+  return gwref_sigma_slice_qrange(d, Vblk, G_t, Wt_t, k, 0, d->nk1 * d->nk2 * d->nk3, out);
+}
+/* same with the q sum restricted to q_begin <= q < q_end (one rank's partial sum) */
+int gwref_sigma_slice_qrange(const gwref_dims *d, const c128 *const *Vblk, const c128 *G_t, const c128 *Wt_t, int k,
+                             int q_begin, int q_end, c128 *out) {
   const int nk = d->nk1 * d->nk2 * d->nk3, nao = d->nao, naux = d->naux;
   const size_t n2 = (size_t)nao * nao, ps = (size_t)naux * naux;
   c128 *X = (c128 *)malloc(sizeof(c128) * naux * n2);
   c128 *Y = (c128 *)malloc(sizeof(c128) * naux * n2);
   c128 *acc = (c128 *)calloc(n2, sizeof(c128));
   int missing = 0;
-  for (int q = 0; q < nk; q++) {
+  for (int q = q_begin; q < q_end; q++) {
     const int kmq = gwref_ksub(d, k, q);
     const c128 *V1 = Vblk[(size_t)k * nk + kmq];  /* V[k][k-q] */
     const c128 *V2 = Vblk[(size_t)kmq * nk + k];  /* V[k-q][k] */
@@ -282,13 +289,19 @@ int gwref_selfenergy(const gwref_dims *d, const c128 *const *Vblk, const c128 *G
 
 /* ---- Eq. 22, one k:
  *   K[i][j] = -(1/N_k) sum_k' sum_ab sum_Q V^{k k'}_{ia}(Q) gamma^{k'}_{ab} V^{k' k}_{bj}(Q) */
+int gwref_exchange_slice_qrange(const gwref_dims *d, const c128 *const *Vblk, const c128 *gamma, int k, int q_begin, int q_end, c128 *out);
 int gwref_exchange_slice(const gwref_dims *d, const c128 *const *Vblk, const c128 *gamma, int k, c128 *out) {
+  return gwref_exchange_slice_qrange(d, Vblk, gamma, k, 0, d->nk1 * d->nk2 * d->nk3, out);
+}
+/* same with the k' sum restricted to k' = k - q, q_begin <= q < q_end */
+int gwref_exchange_slice_qrange(const gwref_dims *d, const c128 *const *Vblk, const c128 *gamma, int k, int q_begin, int q_end, c128 *out) {
   const int nk = d->nk1 * d->nk2 * d->nk3, nao = d->nao, naux = d->naux;
   const size_t n2 = (size_t)nao * nao;
   c128 *acc = (c128 *)calloc(n2, sizeof(c128));
   c128 *T = (c128 *)malloc(sizeof(c128) * n2);
   int missing = 0;
-  for (int kp = 0; kp < nk && !missing; kp++) {
+  for (int q = q_begin; q < q_end && !missing; q++) {
+    const int kp = gwref_ksub(d, k, q);
     const c128 *V1 = Vblk[(size_t)k * nk + kp], *V2 = Vblk[(size_t)kp * nk + k];
     if (!V1 || !V2) { missing = 1; break; }
     const c128 *g = gamma + (size_t)kp * n2;

@@ -1,0 +1,82 @@
+"""CPU-only checks of the boundary: the C-ABI library builds, loads without a GPU and exports every symbol that
+include/gw.h declares; host-side argument validation works without touching a device."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gwlib():
+    from paper_2206_07660_b200 import build as gwbuild
+    gwbuild.build()
+    import paper_2206_07660_b200 as gw
+    return gw
+
+
+def declared_symbols():
+    txt = open(os.path.join(ROOT, "include", "gw.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(gw_[a-z0-9_]+)\s*\(", txt)))
+
+
+def test_exports_every_declared_symbol(gwlib):
+    syms = declared_symbols()
+    assert {"gw_polarization", "gw_screened_interaction", "gw_selfenergy", "gw_exchange"} <= set(syms)
+    L = ctypes.CDLL(gwlib.lib_path())
+    for s in syms:
+        assert hasattr(L, s), s
+
+
+def test_no_torch_or_python_in_abi():
+    txt = open(os.path.join(ROOT, "include", "gw.h")).read()
+    assert "torch" not in re.sub(r"/\*.*?\*/", "", txt, flags=re.S).lower()
+    assert "at::" not in txt and "pybind" not in txt.lower()
+
+
+def test_strerror_and_version(gwlib):
+    assert gwlib.gw_version() >= 100
+    assert gwlib.gw_strerror(0) == "ok"
+    assert "sm_100" in gwlib.gw_strerror(-3)
+
+
+def test_validation_without_device(gwlib):
+    # host-only argument checks: bad sizes / null pointers are rejected before any CUDA call
+    from paper_2206_07660_b200.binding import _CProblem
+    L = gwlib.lib()
+    c = _CProblem(2, 2, 2, 26, 100, 104, 104, 2, 0, 8, 700.0, None, None, None, None, 0)
+    assert L.gw_polarization(ctypes.byref(c), None, None, None) == -1          # GW_EINVAL: null V
+    c.V = 4096
+    c.nao = 0
+    assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4096), ctypes.c_void_p(4096), None) == -1
+    c.nao = 26; c.q_begin = 5; c.q_end = 3
+    assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4096), ctypes.c_void_p(4096), None) == -1
+    c.q_begin = 0; c.q_end = 8; c.nao = 80
+    assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4096), ctypes.c_void_p(4096), None) == -4   # GW_ESHAPE
+    c.nao = 26
+    assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4097), ctypes.c_void_p(4096), None) == -1  # misaligned
+    assert L.gw_workspace_bytes(ctypes.byref(c)) > 0
+    assert L.gw_launch_count(ctypes.byref(c)) == 8
+
+
+def test_missing_library_fails_loudly(monkeypatch, gwlib):
+    import paper_2206_07660_b200.binding as b
+    monkeypatch.setattr(b, "_lib", None)
+    monkeypatch.setattr(b, "_SO", "/nonexistent/libgw_b200.so")
+    with pytest.raises(b.GWError):
+        b.lib()
+
+
+def test_product_path_does_not_import_oracle():
+    for root, _, files in os.walk(os.path.join(ROOT, "paper_2206_07660_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(root, f)).read()
+                assert "import oracle" not in txt and "gwref" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2206_07660_b200" not in txt.replace("paper_2206_07660_b200/csrc", ""), f
