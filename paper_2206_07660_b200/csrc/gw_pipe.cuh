@@ -113,6 +113,101 @@ __device__ __forceinline__ void final_store(c128 *out, const double (&sgr)[NCT][
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Warp-specialised pipeline: one producer warp fills a ring of stage buffers with cp.async (completion tracked by an
+// mbarrier per stage), NCONS consumer warps wait on "full", compute on FP64 tensor cores, and release "empty".
+// No CTA-wide barrier in steady state.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int NCONS = 8;                 // consumer warps
+constexpr int NPROD_THR = 128;           // producer threads (one warpgroup)
+constexpr int NTHR_WS = 32 * (NCONS + 4);   // consumers = two warpgroups; producer = warp NCONS of a third warpgroup
+
+// register rebalancing between the producer and consumer warpgroups (all warps of a warpgroup must execute it)
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (count must be pre-accounted: .noinc)
+__device__ __forceinline__ void cp_async_arrive_noinc(uint64_t *bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// exact n / d for n*d < 2^32 (d >= 1), without an integer divide in the inner loops
+struct FastDiv {
+  unsigned d, m;
+  __host__ __device__ FastDiv() : d(1), m(0) {}
+  __host__ explicit FastDiv(unsigned dd) : d(dd), m(dd <= 1 ? 0u : (unsigned)((1ull << 32) / dd + 1)) {}
+  __device__ __forceinline__ unsigned div(unsigned n) const { return m ? __umulhi(n, m) : n; }
+};
+
+struct Ring {
+  uint64_t *full, *empty;   // [nstage] each
+  int nstage;
+  unsigned it;              // job counter (same sequence on both sides)
+  __device__ __forceinline__ int stage() const { return (int)(it % (unsigned)nstage); }
+  __device__ __forceinline__ unsigned round() const { return it / (unsigned)nstage; }
+  // producer side
+  __device__ __forceinline__ int acquire() { const int s = stage(); mbar_wait(empty + s, (round() & 1u) ^ 1u); return s; }
+  __device__ __forceinline__ void commit() { cp_async_arrive_noinc(full + stage()); ++it; }
+  // consumer side
+  __device__ __forceinline__ int wait() { const int s = stage(); mbar_wait(full + s, round() & 1u); return s; }
+  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) mbar_arrive(empty + stage()); ++it; }
+};
+
+// producer-warpgroup versions of the job issue functions (128 threads: threadIdx.x - 32*NCONS)
+__device__ __forceinline__ void ws_issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd) {
+  const int nrow = min(PASS_ROWS, rows_total - row0);
+  const int total = nrow * nao;
+  const c128 *s = src + (size_t)row0 * nao;
+  for (int i = threadIdx.x - 32 * NCONS; i < total; i += NPROD_THR) {
+    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
+    cp_async16(stage + r * ldp + a, s + i);
+  }
+}
+__device__ __forceinline__ void ws_issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop, FastDiv fd) {
+  const int n2 = nao * nao;
+  const int lane = threadIdx.x - 32 * NCONS;
+  for (int i = lane; i < n2; i += NPROD_THR) {
+    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
+    cp_async16(stage + r * ldp + a, Aq + i);
+  }
+  c128 *sB = stage + naop * ldp;
+  const int rowsB = 4 * ksp;
+  for (int i = lane; i < rowsB * nao; i += NPROD_THR) {
+    const int r = (int)fd.div((unsigned)i);
+    const bool ok = r < nao;
+    cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + i : Bq, ok);
+  }
+}
+// nao x nao matrix -> sG[r][ldp] (TRANSPOSE: sG[c][ldp + r])
+template <bool TRANSPOSE>
+__device__ __forceinline__ void ws_issue_matrix(c128 *sG, const c128 *src, int nao, int ldp, FastDiv fd) {
+  const int n2 = nao * nao;
+  for (int i = threadIdx.x - 32 * NCONS; i < n2; i += NPROD_THR) {
+    const int r = (int)fd.div((unsigned)i), cc = i - r * nao;
+    cp_async16(TRANSPOSE ? sG + cc * ldp + r : sG + r * ldp + cc, src + i);
+  }
+}
+
+// consumer-side pass: like pass_compute but the warp index is the consumer warp index (0..7) and no early return
+// before the ring release is needed (caller releases).
 // pass-geometry shared by the stages
 struct PassGeom { int ldp, ksp, ksp_max, ndt, naop, ldt, nct; bool ok; };
 static inline PassGeom pass_geom(int nao) {

@@ -13,202 +13,237 @@
 
 namespace s3 {
 
-using gwp::NTHR; using gwp::NSTAGE; using gwp::PASS_ROWS;
+using gwp::NCONS; using gwp::NTHR_WS; using gwp::PASS_ROWS; using gwp::FastDiv; using gwp::Ring;
+constexpr int NSTAGE_MAX = 8;
 constexpr int KC = 8, MT_W = 2, NJ = 7, TM = 32;
 
 struct Params {
   GwDims d;
   const c128 *V, *G, *Wt;
   c128 *Sigma, *scratch;
-  unsigned *counter;
   int nqt, nitems;
   int ldp, ksp, ndt;      // pass / G smem row stride, k-steps over nao, tiles over nao
   int ldt;                // row stride of the T block in the final jobs
   int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
   int ldb;                // row stride of the main-job B part
-  int stage_units;
+  int stage_units, nstage;
   size_t slab_units;      // complex elements per slab (two slabs per CTA)
+  FastDiv fd_nao;
 };
 
-using gwp::cp_async16_zfill; using gwp::issue_pass_job; using gwp::issue_final_job;
-
-// main job: A = W[tm rows][k0..k0+8) swizzled; B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
-__device__ __forceinline__ void issue_main_job(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
-                                               int n0, int ncols, int ldb, int k0) {
-  for (int i = threadIdx.x; i < TM * KC; i += NTHR) {
-    const int r = i >> 3, u = i & 7;
-    const bool ok = (r < tm_rows) && (k0 + u < naux);
-    cp_async16_zfill(stage + r * KC + (u ^ ((r & 1) << 2)), ok ? W + (size_t)r * naux + k0 + u : W, ok);
+// main job (producer warpgroup): A = W[tm rows][k0..k0+8) swizzled; B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
+__device__ __forceinline__ void ws_issue_main(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
+                                              int n0, int ncols, int ldb, int k0) {
+  const int pt = threadIdx.x - 32 * NCONS;
+  {
+    const int u = pt & 7, rsub = pt >> 3;
+    const bool kok = k0 + u < naux;
+    for (int r = rsub; r < TM; r += 16) {
+      const bool ok = kok && (r < tm_rows);
+      gwp::cp_async16_zfill(stage + r * KC + (u ^ ((r & 1) << 2)), ok ? W + (size_t)r * naux + k0 + u : W, ok);
+    }
   }
   c128 *sB = stage + TM * KC;
-  const int total = KC * ncols;
-  for (int i = threadIdx.x; i < total; i += NTHR) {
-    const int r = i / ncols, cc = i - r * ncols;
-    const bool ok = (k0 + r < naux) && (n0 + cc < n2);
-    cp_async16_zfill(sB + r * ldb + cc, ok ? V2 + (size_t)(k0 + r) * n2 + n0 + cc : V2, ok);
+#pragma unroll
+  for (int r = 0; r < KC; r++) {
+    const bool rok = k0 + r < naux;
+    const c128 *src = V2 + (size_t)(k0 + r) * n2 + n0;
+    for (int cc = pt; cc < ncols; cc += gwp::NPROD_THR) {
+      const bool ok = rok && (n0 + cc < n2);
+      gwp::cp_async16_zfill(sB + r * ldb + cc, ok ? src + cc : V2, ok);
+    }
+  }
+}
+
+template <int NJM>
+__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, int ldb, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
+#pragma unroll
+  for (int ks = 0; ks < KC / 4; ks++) {
+    const int u = (4 * ks + c) ^ sw;
+    c128 a[MT_W], b[NJM];
+#pragma unroll
+    for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
+    const c128 *brow = sBw + (4 * ks + c) * ldb;
+#pragma unroll
+    for (int jn = 0; jn < NJM; jn++) b[jn] = brow[32 * jn];
+#pragma unroll
+    for (int jn = 0; jn < NJM; jn++)
+#pragma unroll
+      for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
   }
 }
 
 template <int KSP_MAX, int NCT>
-__global__ void __launch_bounds__(NTHR, 1) sigma_kernel(const Params P) {
+__global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   c128 *smem = reinterpret_cast<c128 *>(smem_raw);
   const GwDims d = P.d;
   const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, naop = 8 * P.ndt, ndt = P.ndt;
   c128 *sG = smem;                    // [naop][ldp]: sG[a][b] = G[t][k-q][a][b]  (operand [n=a][k=b] of pass A)
   c128 *sStage = sG + naop * ldp;
-  __shared__ int s_item;
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
-  const int mh = w >> 2;                              // m-half: m-tiles 2*mh, 2*mh+1
-  const int sw = (g & 1) << 2;
+  const int NSTAGE = P.nstage;
+  __shared__ uint64_t bars[2 * NSTAGE_MAX + 2];
+  uint64_t *bar_full = bars, *bar_empty = bars + NSTAGE_MAX, *bar_g = bars + 2 * NSTAGE_MAX, *bar_phase = bars + 2 * NSTAGE_MAX + 1;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   c128 *slabU = P.scratch + (size_t)blockIdx.x * 2 * P.slab_units;
   c128 *slabT = slabU + P.slab_units;
   const size_t vb = (size_t)naux * n2;
-
   {
     const int tot = naop * ldp + NSTAGE * P.stage_units;
-    for (int i = threadIdx.x; i < tot; i += NTHR) smem[i] = make_double2(0.0, 0.0);
+    for (int i = threadIdx.x; i < tot; i += NTHR_WS) smem[i] = make_double2(0.0, 0.0);
+    if (threadIdx.x == 0) {
+      for (int i = 0; i < NSTAGE; i++) { gwp::mbar_init(bar_full + i, gwp::NPROD_THR); gwp::mbar_init(bar_empty + i, NCONS); }
+      gwp::mbar_init(bar_g, gwp::NPROD_THR);
+      gwp::mbar_init(bar_phase, NCONS);
+    }
   }
   __syncthreads();
+  Ring ring; ring.full = bar_full; ring.empty = bar_empty; ring.nstage = NSTAGE; ring.it = 0;
+  unsigned gpar = 0, ppar = 0;
+  const int nmain = (naux + KC - 1) / KC;
 
-  for (;;) {
-    if (threadIdx.x == 0) s_item = (int)atomicAdd(P.counter, 1u);
-    __syncthreads();
-    const int item = s_item;
-    __syncthreads();
-    if (item >= P.nitems) break;
-    const int t = item % d.ntau, k = item / d.ntau;
-
-    double sgr[NCT][2], sgi[NCT][2];
-#pragma unroll
-    for (int i = 0; i < NCT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
-
-    for (int ql = 0; ql < d.nq; ql++) {
-      const int q = d.q0 + ql, kp = gw_ksub(d, k, q);
-      const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
-      const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
-      const c128 *Gp = P.G + ((size_t)t * d.nk + kp) * n2;
-      const c128 *Wq = P.Wt + ((size_t)t * d.nq + ql) * naux * naux;
-      __syncthreads();
-      for (int i = threadIdx.x; i < n2; i += NTHR) { const int r = i / nao, cc = i - r * nao; sG[r * ldp + cc] = Gp[i]; }
-
-      for (int qt = 0; qt < P.nqt; qt++) {
-        const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
-        const c128 *W = Wq + (size_t)Q0 * naux;
-        const int nmain = (naux + KC - 1) / KC;
-        // ---- main GEMM, N chunk by N chunk; U^T written to slabU as [(Q,j)][b] ----
-        for (int ch = 0; ch < P.nchunk; ch++) {
-          const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);     // n-tiles of this chunk
-          const int n0 = nt0 * 8, ncols = ntc * 8;
-          const int noff = ((w & 3) - mh + 4) & 3;
-          const int njm = (ntc > noff) ? (ntc - noff + 3) / 4 : 0;
-          double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
-#pragma unroll
-          for (int i = 0; i < MT_W; i++)
-#pragma unroll
-            for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
-          int issued = 0;
-          for (; issued < NSTAGE - 1; issued++) {
-            if (issued < nmain) issue_main_job(sStage + (issued % NSTAGE) * P.stage_units, W, tm_rows, naux, V2, n2, n0, ncols, P.ldb, issued * KC);
-            cp_async_commit();
-          }
-          for (int jb = 0; jb < nmain; jb++) {
-            cp_async_wait<NSTAGE - 2>();
-            __syncthreads();
-            const int nx = jb + NSTAGE - 1;
-            if (nx < nmain) issue_main_job(sStage + (nx % NSTAGE) * P.stage_units, W, tm_rows, naux, V2, n2, n0, ncols, P.ldb, nx * KC);
-            cp_async_commit();
-            const c128 *sA = sStage + (jb % NSTAGE) * P.stage_units;
-            const c128 *sB = sA + TM * KC;
-            if (mh * MT_W < mtc) {
-#pragma unroll
-              for (int ks = 0; ks < KC / 4; ks++) {
-                const int u = (4 * ks + c) ^ sw;
-                c128 a[MT_W];
-#pragma unroll
-                for (int i = 0; i < MT_W; i++) a[i] = sA[(8 * (mh * MT_W + i) + g) * KC + u];
-                const c128 *brow = sB + (4 * ks + c) * P.ldb + g;
-#pragma unroll
-                for (int jn = 0; jn < NJ; jn++) {
-                  if (jn < njm) {
-                    const c128 b = brow[8 * (noff + 4 * jn)];
-#pragma unroll
-                    for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
-                  }
-                }
-              }
+  if (w >= NCONS) {
+    // =============================== producer warpgroup ===============================
+    gwp::reg_dec<40>();
+    for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+      const int t = item % d.ntau, k = item / d.ntau;
+      for (int ql = 0; ql < d.nq; ql++) {
+        const int q = d.q0 + ql, kp = gw_ksub(d, k, q);
+        const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
+        const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
+        const c128 *Wq = P.Wt + ((size_t)t * d.nq + ql) * naux * naux;
+        gwp::ws_issue_matrix<false>(sG, P.G + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
+        gwp::cp_async_arrive_noinc(bar_g);
+        for (int qt = 0; qt < P.nqt; qt++) {
+          const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0);
+          const c128 *W = Wq + (size_t)Q0 * naux;
+          for (int ch = 0; ch < P.nchunk; ch++) {
+            const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
+            for (int j = 0; j < nmain; j++) {
+              const int s = ring.acquire();
+              ws_issue_main(sStage + s * P.stage_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC);
+              ring.commit();
             }
           }
-          cp_async_wait<0>();
-          // store U^T: element (Q, n=(b,j)) -> slabU[(Q*nao + j)*nao + b]
-#pragma unroll
-          for (int i = 0; i < MT_W; i++) {
-            const int Ql = 8 * (mh * MT_W + i) + g;
-#pragma unroll
-            for (int jn = 0; jn < NJ; jn++) {
-              if (jn < njm && Ql < tm_rows) {
-#pragma unroll
-                for (int e = 0; e < 2; e++) {
-                  const int n = n0 + 8 * (noff + 4 * jn) + 2 * c + e;
-                  if (n < n2) {
-                    const int b = n / nao, j = n - b * nao;
-                    slabU[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
-                  }
-                }
-              }
-            }
-          }
-          __syncthreads();
-        }
-        // ---- pass A: T[Q][a][j] = Σ_b G[a][b] U[Q][b][j] ----
-        {
           const int rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
-          int issued = 0;
-          for (; issued < NSTAGE - 1; issued++) {
-            if (issued < npass) issue_pass_job(sStage + (issued % NSTAGE) * P.stage_units, slabU, issued * PASS_ROWS, rows, nao, ldp);
-            cp_async_commit();
+          gwp::mbar_wait(bar_phase, ppar); ppar ^= 1u;          // U^T of this panel is in slabU
+          for (int j = 0; j < npass; j++) {
+            const int s = ring.acquire();
+            gwp::ws_issue_rows(sStage + s * P.stage_units, slabU, j * PASS_ROWS, rows, nao, ldp, P.fd_nao);
+            ring.commit();
           }
-          for (int jb = 0; jb < npass; jb++) {
-            cp_async_wait<NSTAGE - 2>();
-            __syncthreads();
-            const int nx = jb + NSTAGE - 1;
-            if (nx < npass) issue_pass_job(sStage + (nx % NSTAGE) * P.stage_units, slabU, nx * PASS_ROWS, rows, nao, ldp);
-            cp_async_commit();
-            gwp::pass_compute<KSP_MAX, true>(sStage + (jb % NSTAGE) * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
-          }
-          cp_async_wait<0>();
-          __syncthreads();
-        }
-        // ---- final: Sigma[i][j] += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; one job per Q ----
-        {
+          gwp::mbar_wait(bar_phase, ppar); ppar ^= 1u;          // T of this panel is in slabT
           const c128 *V1t = V1 + (size_t)Q0 * n2;
-          int issued = 0;
-          for (; issued < NSTAGE - 1; issued++) {
-            if (issued < tm_rows) issue_final_job(sStage + (issued % NSTAGE) * P.stage_units, V1t + (size_t)issued * n2, slabT + (size_t)issued * n2, nao, ldp, P.ldt, P.ksp, naop);
-            cp_async_commit();
+          for (int j = 0; j < tm_rows; j++) {
+            const int s = ring.acquire();
+            gwp::ws_issue_final(sStage + s * P.stage_units, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldp, P.ldt, P.ksp, naop, P.fd_nao);
+            ring.commit();
           }
-          for (int jb = 0; jb < tm_rows; jb++) {
-            cp_async_wait<NSTAGE - 2>();
-            __syncthreads();
-            const int nx = jb + NSTAGE - 1;
-            if (nx < tm_rows) issue_final_job(sStage + (nx % NSTAGE) * P.stage_units, V1t + (size_t)nx * n2, slabT + (size_t)nx * n2, nao, ldp, P.ldt, P.ksp, naop);
-            cp_async_commit();
-            gwp::final_compute<NCT>(sStage + (jb % NSTAGE) * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
-          }
-          cp_async_wait<0>();
-          __syncthreads();
         }
       }
     }
-    // ---- epilogue ----
-    const double pref = -1.0 / (double)d.nk;
-    c128 *out = P.Sigma + ((size_t)t * d.nk + k) * n2;
-    gwp::final_store<NCT>(out, sgr, sgi, pref, nao, ndt);
+    asm volatile("cp.async.wait_all;\n" ::: "memory");
+  } else {
+    // =============================== consumer warps ===============================
+    gwp::reg_inc<232>();
+    const int g = lane >> 2, c = lane & 3;
+    const int mh = w >> 2;                              // m-half: m-tiles 2*mh, 2*mh+1
+    const int sw = (g & 1) << 2;
+    const int noff = ((w & 3) - mh + 4) & 3;
+    for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+      const int t = item % d.ntau, k = item / d.ntau;
+      double sgr[NCT][2], sgi[NCT][2];
+#pragma unroll
+      for (int i = 0; i < NCT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+      for (int ql = 0; ql < d.nq; ql++) {
+        gwp::mbar_wait(bar_g, gpar); gpar ^= 1u;
+        for (int qt = 0; qt < P.nqt; qt++) {
+          const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
+          // ---- main GEMM, N chunk by N chunk; U^T written to slabU as [(Q,j)][b] ----
+          for (int ch = 0; ch < P.nchunk; ch++) {
+            const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
+            const int n0 = nt0 * 8;
+            const int njm = (ntc > noff) ? (ntc - noff + 3) / 4 : 0;
+            const bool active = (mh * MT_W < mtc) && njm > 0;
+            double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
+#pragma unroll
+            for (int i = 0; i < MT_W; i++)
+#pragma unroll
+              for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
+            for (int jb = 0; jb < nmain; jb++) {
+              const int s = ring.wait();
+              if (active) {
+                const c128 *sAw = sStage + s * P.stage_units + (8 * mh * MT_W + g) * KC;
+                const c128 *sBw = sStage + s * P.stage_units + TM * KC + 8 * noff + g;
+                if (njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else {
+#pragma unroll
+                  for (int ks = 0; ks < KC / 4; ks++) {
+                    const int u = (4 * ks + c) ^ sw;
+                    c128 a[MT_W];
+#pragma unroll
+                    for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
+                    const c128 *brow = sBw + (4 * ks + c) * P.ldb;
+#pragma unroll
+                    for (int jn = 0; jn < NJ; jn++) {
+                      if (jn < njm) {
+                        const c128 b = brow[32 * jn];
+#pragma unroll
+                        for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
+                      }
+                    }
+                  }
+                }
+              }
+              ring.release();
+            }
+            // store U^T: element (Q, n=(b,j)) -> slabU[(Q*nao + j)*nao + b]
+#pragma unroll
+            for (int i = 0; i < MT_W; i++) {
+              const int Ql = 8 * (mh * MT_W + i) + g;
+#pragma unroll
+              for (int jn = 0; jn < NJ; jn++) {
+                if (jn < njm && Ql < tm_rows) {
+#pragma unroll
+                  for (int e = 0; e < 2; e++) {
+                    const int n = n0 + 8 * (noff + 4 * jn) + 2 * c + e;
+                    if (n < n2) {
+                      const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
+                      slabU[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
+                    }
+                  }
+                }
+              }
+            }
+          }
+          __threadfence(); __syncwarp();
+          if (lane == 0) gwp::mbar_arrive(bar_phase);
+          // ---- pass A: T[Q][a][j] = Σ_b G[a][b] U[Q][b][j] ----
+          const int rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
+          for (int jb = 0; jb < npass; jb++) {
+            const int s = ring.wait();
+            gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
+            ring.release();
+          }
+          __threadfence(); __syncwarp();
+          if (lane == 0) gwp::mbar_arrive(bar_phase);
+          // ---- final: Sigma[i][j] += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; one job per Q ----
+          for (int jb = 0; jb < tm_rows; jb++) {
+            const int s = ring.wait();
+            gwp::final_compute<NCT>(sStage + s * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
+            ring.release();
+          }
+        }
+      }
+      gwp::final_store<NCT>(P.Sigma + ((size_t)t * d.nk + k) * n2, sgr, sgi, -1.0 / (double)d.nk, nao, ndt);
+    }
   }
 }
 
 struct Plan {
-  int ksp_max, nct, nqt, nitems, ldp, ksp, ndt, ldt, nnt, nchunk, cht, ldb, stage_units, grid;
+  int ksp_max, nct, nqt, nitems, ldp, ksp, ndt, ldt, nnt, nchunk, cht, ldb, stage_units, grid, nstage;
   size_t smem, slab_units, work_bytes;
   bool ok;
 };
@@ -235,13 +270,16 @@ static Plan make_plan(const gw_problem *p) {
   pl.stage_units = s_pass;
   if (s_main > pl.stage_units) pl.stage_units = s_main;
   if (s_fin > pl.stage_units) pl.stage_units = s_fin;
-  pl.smem = ((size_t)naop * pl.ldp + (size_t)NSTAGE * pl.stage_units) * sizeof(c128);
+  const size_t fixed = (size_t)naop * pl.ldp * sizeof(c128), per = (size_t)pl.stage_units * sizeof(c128);
+  pl.nstage = (int)((225 * 1024 - fixed) / per);
+  if (pl.nstage > 6) pl.nstage = 6;
+  pl.smem = fixed + (size_t)pl.nstage * per;
   int dev = 0, nsm = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
   if (nsm <= 0) nsm = 148;
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
   pl.work_bytes = 256 + (size_t)nsm * 2 * pl.slab_units * sizeof(c128);
-  pl.ok = pl.smem <= 227 * 1024;
+  pl.ok = pl.nstage >= 2;
   return pl;
 }
 
@@ -273,7 +311,7 @@ template <int KSP_MAX, int NCT>
 static int launch_sigma(const s3::Plan &pl, const s3::Params &P, cudaStream_t st) {
   cudaError_t e = cudaFuncSetAttribute(s3::sigma_kernel<KSP_MAX, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
-  s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR, pl.smem, st>>>(P);
+  s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR_WS, pl.smem, st>>>(P);
   return (int)cudaGetLastError();
 }
 
@@ -283,12 +321,10 @@ int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *S
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   s3::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
-  P.counter = (unsigned *)p->work;
   P.scratch = (c128 *)((char *)p->work + 256);
   P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt;
-  P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.slab_units = pl.slab_units;
-  cudaError_t e = cudaMemsetAsync(p->work, 0, 256, st);
-  if (e != cudaSuccess) return (int)e;
+  P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.slab_units = pl.slab_units;
+  P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
   if (pl.nct == 2) {
     if (pl.ksp_max == 7) return launch_sigma<7, 2>(pl, P, st);
     if (pl.ksp_max == 13) return launch_sigma<13, 2>(pl, P, st);
