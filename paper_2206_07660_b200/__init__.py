@@ -9,8 +9,8 @@ import os
 
 from .binding import (GWProblem, GWError, lib, lib_path, gw_polarization, gw_screened_interaction, gw_selfenergy,
                       gw_exchange, gw_workspace_bytes, gw_sigma_iteration, gw_sigma_iteration_host,
-                      gw_executed_flops, gw_launch_count, gw_fp64_peak, gw_strerror, gw_version, debug_set_naive)
+                      gw_executed_flops, gw_launch_count, gw_fp64_peak, gw_strerror, gw_version)
 
 __all__ = ["GWProblem", "GWError", "lib", "lib_path", "gw_polarization", "gw_screened_interaction", "gw_selfenergy",
            "gw_exchange", "gw_workspace_bytes", "gw_sigma_iteration", "gw_sigma_iteration_host", "gw_executed_flops",
-           "gw_launch_count", "gw_fp64_peak", "gw_strerror", "gw_version", "debug_set_naive"]
+           "gw_launch_count", "gw_fp64_peak", "gw_strerror", "gw_version"]

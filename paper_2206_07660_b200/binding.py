@@ -48,8 +48,6 @@ def lib():
         L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
-        L.gw_debug_set_naive.argtypes = [ctypes.c_int]
-        L.gw_debug_set_naive.restype = None
         for n in ("gw_polarization", "gw_screened_interaction", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_version"):
             getattr(L, n).restype = ctypes.c_int
@@ -63,10 +61,6 @@ def gw_strerror(code):
 
 def gw_version():
     return int(lib().gw_version())
-
-
-def debug_set_naive(on):
-    lib().gw_debug_set_naive(1 if on else 0)
 
 
 def _check(rc, what):

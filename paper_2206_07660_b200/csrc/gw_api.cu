@@ -5,13 +5,6 @@
 #include <string.h>
 #include "gw_common.cuh"
 
-static int g_naive = -1;
-static bool use_naive() {
-  if (g_naive < 0) { const char *e = getenv("GW_DEBUG_NAIVE"); g_naive = (e && e[0] == '1') ? 1 : 0; }
-  return g_naive == 1;
-}
-extern "C" void gw_debug_set_naive(int on) { g_naive = on ? 1 : 0; }
-
 static int check_arch() {
   static int cached = 0;
   if (cached) return cached == 1 ? GW_OK : GW_EARCH;
@@ -42,13 +35,13 @@ extern "C" int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P
   if (!aligned16(G) || !aligned16(P0t)) return GW_EINVAL;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  return use_naive() ? gw_naive_stage1(p, (const c128 *)G, (c128 *)P0t, st) : gw_launch_stage1(p, (const c128 *)G, (c128 *)P0t, st);
+  return gw_launch_stage1(p, (const c128 *)G, (c128 *)P0t, st);
 }
 
 extern "C" size_t gw_workspace_bytes(const gw_problem *p) {
   if (check_problem(p, false) != GW_OK) return 0;
   GwDims d = gw_dims(p);
-  size_t m = use_naive() ? 2 * (size_t)d.nw * d.nq * d.naux * d.naux * sizeof(c128) : 0;   // debug reference kernels only
+  size_t m = 0;
   size_t s;
   if ((s = gw_stage1_workspace(p)) > m) m = s;
   if ((s = gw_stage2_workspace(p)) > m) m = s;
@@ -63,8 +56,7 @@ extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, 
   if (!p->work || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  return use_naive() ? gw_naive_stage2(p, (const c128 *)P0t, (c128 *)Wt, p->work, p->work_bytes, info, st)
-                     : gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, st);
+  return gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, st);
 }
 
 extern "C" int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c128 *Sigma, void *stream) {
@@ -72,8 +64,7 @@ extern "C" int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c12
   if (!aligned16(G) || !aligned16(Wt) || !aligned16(Sigma)) return GW_EINVAL;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  return use_naive() ? gw_naive_stage3(p, (const c128 *)G, (const c128 *)Wt, (c128 *)Sigma, st)
-                     : gw_launch_stage3(p, (const c128 *)G, (const c128 *)Wt, (c128 *)Sigma, st);
+  return gw_launch_stage3(p, (const c128 *)G, (const c128 *)Wt, (c128 *)Sigma, st);
 }
 
 extern "C" int gw_exchange(const gw_problem *p, const gw_c128 *gamma, gw_c128 *K, void *stream) {
@@ -81,7 +72,7 @@ extern "C" int gw_exchange(const gw_problem *p, const gw_c128 *gamma, gw_c128 *K
   if (!aligned16(gamma) || !aligned16(K)) return GW_EINVAL;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  return use_naive() ? gw_naive_stage4(p, (const c128 *)gamma, (c128 *)K, st) : gw_launch_stage4(p, (const c128 *)gamma, (c128 *)K, st);
+  return gw_launch_stage4(p, (const c128 *)gamma, (c128 *)K, st);
 }
 
 extern "C" int gw_executed_flops(const gw_problem *p, double *out) {

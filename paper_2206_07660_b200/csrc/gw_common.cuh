@@ -79,9 +79,3 @@ double gw_stage3_flops(const gw_problem *p);
 double gw_stage4_flops(const gw_problem *p);
 void gw_stage_flops(const gw_problem *p, double *out4);
 int gw_stage_launches(const gw_problem *p);
-
-// debug reference kernels (tiny configs only; not on the product path)
-int gw_naive_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t st);
-int gw_naive_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, void *work, size_t work_bytes, int32_t *info, cudaStream_t st);
-int gw_naive_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st);
-int gw_naive_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st);
