@@ -52,9 +52,10 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
 // complex 8x8 (+)= complex 8x4 * complex 4x8 as four real DMMAs (the "4-real-GEMM" scheme).
 // cr/ci: real/imag accumulator fragments; a, b: this lane's complex A[g][c] and B[c][g] elements.
 __device__ __forceinline__ void cmma(double (&cr)[2], double (&ci)[2], c128 a, c128 b) {
+  // real and imaginary chains alternate, so consecutive DMMAs of one warp never depend on each other
   dmma884(cr[0], cr[1], a.x, b.x);
-  dmma884(cr[0], cr[1], -a.y, b.y);
   dmma884(ci[0], ci[1], a.x, b.y);
+  dmma884(cr[0], cr[1], -a.y, b.y);
   dmma884(ci[0], ci[1], a.y, b.x);
 }
 

@@ -61,6 +61,46 @@ __device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG,
   }
 }
 
+// Straight-line version of pass_compute for ksp == KSP exactly (the production shapes: nao = 26 -> 7, nao = 52 -> 13):
+// the (n-tile, k-step) loop nest is flattened and fully unrolled, every B fragment is loaded PF steps (4*PF DMMAs)
+// before its use, and no branch separates the DMMAs.  Same sums in the same order as pass_compute.
+template <int KSP, bool TRANSPOSED>
+__device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
+                                                   int nao, int ldp) {
+  constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 4, NB = PF + 1;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  if (row0 + 8 * w >= rows_total) return;   // whole m-tile beyond the panel (warp-uniform)
+  c128 a[KSP];
+  const c128 *ap = sStage + (8 * w + g) * ldp + c;
+#pragma unroll
+  for (int ks = 0; ks < KSP; ks++) a[ks] = ap[4 * ks];
+  const int row = row0 + 8 * w + g;
+  const bool rok = row < rows_total;
+  c128 *o0;
+  size_t ostride;                           // distance between consecutive output columns
+  if (TRANSPOSED) { const int Q = row / nao, x = row - Q * nao; o0 = out + (size_t)Q * nao * nao + x; ostride = (size_t)nao; }
+  else { o0 = out + (size_t)row * nao; ostride = 1; }
+  const c128 *bp = sG + g * ldp + c;
+  c128 b[NB];
+#pragma unroll
+  for (int s = 0; s < PF && s < S; s++) b[s % NB] = bp[(s / KSP) * 8 * ldp + 4 * (s % KSP)];
+  double cr[2] = {0.0, 0.0}, ci[2] = {0.0, 0.0};
+#pragma unroll
+  for (int s = 0; s < S; s++) {
+    const int nt = s / KSP, ks = s % KSP;
+    if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
+    cmma(cr, ci, a[ks], b[s % NB]);
+    if (ks == KSP - 1) {
+      const int col = 8 * nt + 2 * c;
+      if (rok) {
+        if (col < nao) o0[(size_t)col * ostride] = make_double2(cr[0], ci[0]);
+        if (col + 1 < nao) o0[(size_t)(col + 1) * ostride] = make_double2(cr[1], ci[1]);
+      }
+      cr[0] = cr[1] = 0.0; ci[0] = ci[1] = 0.0;
+    }
+  }
+}
+
 // "final" job for one Q: A = Aq (nao x nao, [i][a]) -> stage[i][ldp]; B = Bq (nao x nao, [a][j]) -> [a][ldt], rows a >= nao zero
 __device__ __forceinline__ void issue_final_job(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop) {
   const int n2 = nao * nao;
@@ -92,6 +132,42 @@ __device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[N
       const c128 *bp = sB + c * ldt + 8 * nj + g;
       for (int ks = 0; ks < ksp; ks++) cmma(sgr[ti], sgi[ti], ap[4 * ks], bp[4 * ks * ldt]);
     }
+  }
+}
+
+// Straight-line version of final_compute for ksp == KSP exactly: all fragments of a k-step group are loaded before
+// the DMMAs that use them, the NCT tiles of the warp are interleaved (2*NCT independent chains).
+template <int KSP, int NCT>
+__device__ __forceinline__ void final_compute_exact(const c128 *stage, double (&sgr)[NCT][2], double (&sgi)[NCT][2], int ldp, int ldt,
+                                                    int naop) {
+  constexpr int NDT = (KSP + 1) / 2;
+  if (NCT * 8 < NDT * NDT) return;          // never launched with such a pair (the plan picks NCT from ndt)
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  const c128 *sA = stage, *sB = stage + naop * ldp;
+  const c128 *ap[NCT], *bp[NCT];
+  bool on[NCT];
+#pragma unroll
+  for (int ti = 0; ti < NCT; ti++) {
+    const int tile = w + 8 * ti;
+    on[ti] = tile < NDT * NDT;
+    const int mi = on[ti] ? tile / NDT : 0, nj = on[ti] ? tile - mi * NDT : 0;
+    ap[ti] = sA + (8 * mi + g) * ldp + c;
+    bp[ti] = sB + c * ldt + 8 * nj + g;
+  }
+  constexpr int GK = 4;                     // k-steps per load group
+#pragma unroll
+  for (int k0 = 0; k0 < KSP; k0 += GK) {
+    c128 a[NCT][GK], b[NCT][GK];
+#pragma unroll
+    for (int ti = 0; ti < NCT; ti++)
+#pragma unroll
+      for (int kk = 0; kk < GK; kk++)
+        if (k0 + kk < KSP && on[ti]) { a[ti][kk] = ap[ti][4 * (k0 + kk)]; b[ti][kk] = bp[ti][4 * (k0 + kk) * ldt]; }
+#pragma unroll
+    for (int kk = 0; kk < GK; kk++)
+#pragma unroll
+      for (int ti = 0; ti < NCT; ti++)
+        if (k0 + kk < KSP && on[ti]) cmma(sgr[ti], sgi[ti], a[ti][kk], b[ti][kk]);
   }
 }
 

@@ -170,14 +170,16 @@ __global__ void __launch_bounds__(NTHR_WS, 1) p0_kernel(const Params P) {
         gwp::mbar_wait(bar_g, gpar); gpar ^= 1u;
         for (int j = 0; j < npass; j++) {
           const int s = ring.wait();
-          gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sGt, slab, j * PASS_ROWS, rows, nao, ldp, P.ksp, P.ndt);
+          if (P.ksp == KSP_MAX) gwp::pass_compute_exact<KSP_MAX, true>(sStage + s * P.stage_units, sGt, slab, j * PASS_ROWS, rows, nao, ldp);
+          else gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sGt, slab, j * PASS_ROWS, rows, nao, ldp, P.ksp, P.ndt);
           ring.release();
         }
         __threadfence(); __syncwarp();
         if (lane == 0) gwp::mbar_arrive(bar_phase);
         for (int j = 0; j < npass; j++) {
           const int s = ring.wait();
-          gwp::pass_compute<KSP_MAX, false>(sStage + s * P.stage_units, sGm, slab, j * PASS_ROWS, rows, nao, ldp, P.ksp, P.ndt);
+          if (P.ksp == KSP_MAX) gwp::pass_compute_exact<KSP_MAX, false>(sStage + s * P.stage_units, sGm, slab, j * PASS_ROWS, rows, nao, ldp);
+          else gwp::pass_compute<KSP_MAX, false>(sStage + s * P.stage_units, sGm, slab, j * PASS_ROWS, rows, nao, ldp, P.ksp, P.ndt);
           ring.release();
         }
         __threadfence(); __syncwarp();

@@ -224,7 +224,8 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
           const int rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
           for (int jb = 0; jb < npass; jb++) {
             const int s = ring.wait();
-            gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
+            if (P.ksp == KSP_MAX) gwp::pass_compute_exact<KSP_MAX, true>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp);
+            else gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
             ring.release();
           }
           __threadfence(); __syncwarp();
@@ -232,7 +233,8 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
           // ---- final: Sigma[i][j] += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; one job per Q ----
           for (int jb = 0; jb < tm_rows; jb++) {
             const int s = ring.wait();
-            gwp::final_compute<NCT>(sStage + s * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
+            if (P.ksp == KSP_MAX) gwp::final_compute_exact<KSP_MAX, NCT>(sStage + s * P.stage_units, sgr, sgi, ldp, P.ldt, naop);
+            else gwp::final_compute<NCT>(sStage + s * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
             ring.release();
           }
         }
