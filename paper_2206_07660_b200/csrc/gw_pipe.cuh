@@ -31,8 +31,9 @@ __device__ __forceinline__ void issue_pass_job(c128 *stage, const c128 *src, int
 //   TRANSPOSED = false: out[row*nao + n]
 template <int KSP_MAX, bool TRANSPOSED>
 __device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
-                                             int nao, int ldp, int ksp, int ndt) {
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+                                             int nao, int ldp, int ksp, int ndt, int w = -1) {
+  if (w < 0) w = threadIdx.x >> 5;          // m-tile of this warp within the job
+  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
   if (row0 + 8 * w >= rows_total) return;   // whole m-tile beyond the panel (warp-uniform)
   c128 a[KSP_MAX];
 #pragma unroll
@@ -66,9 +67,10 @@ __device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG,
 // before its use, and no branch separates the DMMAs.  Same sums in the same order as pass_compute.
 template <int KSP, bool TRANSPOSED>
 __device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
-                                                   int nao, int ldp) {
+                                                   int nao, int ldp, int w = -1) {
   constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 4, NB = PF + 1;
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  if (w < 0) w = threadIdx.x >> 5;          // m-tile of this warp within the job
+  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
   if (row0 + 8 * w >= rows_total) return;   // whole m-tile beyond the panel (warp-uniform)
   c128 a[KSP];
   const c128 *ap = sStage + (8 * w + g) * ldp + c;
@@ -101,19 +103,20 @@ __device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c12
   }
 }
 
-// "final" job for one Q: A = Aq (nao x nao, [i][a]) -> stage[i][ldp]; B = Bq (nao x nao, [a][j]) -> [a][ldt], rows a >= nao zero
-__device__ __forceinline__ void issue_final_job(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop) {
-  const int n2 = nao * nao;
-  for (int i = threadIdx.x; i < n2; i += NTHR) {
-    const int r = i / nao, a = i - r * nao;
-    cp_async16(stage + r * ldp + a, Aq + i);
+// "final" job for the K range [a0, a0 + 4*ksp) of one Q: A = Aq[i][a0..] (nao x nao, [i][a]) -> stage[i][ldp];
+// B = Bq[a0..][j] (nao x nao, [a][j]) -> [a - a0][ldt]; K beyond nao is zero filled
+__device__ __forceinline__ void issue_final_job(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop, int a0) {
+  const int kw = 4 * ksp;
+  for (int i = threadIdx.x; i < nao * kw; i += NTHR) {
+    const int r = i / kw, cc = i - r * kw;
+    const bool ok = a0 + cc < nao;
+    cp_async16_zfill(stage + r * ldp + cc, ok ? Aq + r * nao + a0 + cc : Aq, ok);
   }
   c128 *sB = stage + naop * ldp;
-  const int rowsB = 4 * ksp;
-  for (int i = threadIdx.x; i < rowsB * nao; i += NTHR) {
+  for (int i = threadIdx.x; i < kw * nao; i += NTHR) {
     const int r = i / nao;
-    const bool ok = r < nao;
-    cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + i : Bq, ok);
+    const bool ok = a0 + r < nao;
+    cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + (size_t)a0 * nao + i : Bq, ok);
   }
 }
 
@@ -135,12 +138,12 @@ __device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[N
   }
 }
 
-// Straight-line version of final_compute for ksp == KSP exactly: all fragments of a k-step group are loaded before
-// the DMMAs that use them, the NCT tiles of the warp are interleaved (2*NCT independent chains).
-template <int KSP, int NCT>
+// Straight-line version of final_compute for KS k-steps and an NDT x NDT tile grid known at compile time: all fragments
+// of a k-step group are loaded before the DMMAs that use them, the NCT tiles of the warp are interleaved (2*NCT
+// independent chains).
+template <int KS, int NDT, int NCT>
 __device__ __forceinline__ void final_compute_exact(const c128 *stage, double (&sgr)[NCT][2], double (&sgi)[NCT][2], int ldp, int ldt,
                                                     int naop) {
-  constexpr int NDT = (KSP + 1) / 2;
   if (NCT * 8 < NDT * NDT) return;          // never launched with such a pair (the plan picks NCT from ndt)
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
   const c128 *sA = stage, *sB = stage + naop * ldp;
@@ -154,20 +157,20 @@ __device__ __forceinline__ void final_compute_exact(const c128 *stage, double (&
     ap[ti] = sA + (8 * mi + g) * ldp + c;
     bp[ti] = sB + c * ldt + 8 * nj + g;
   }
-  constexpr int GK = 4;                     // k-steps per load group
+  constexpr int GK = (NCT <= 2) ? 4 : 1;    // k-steps per load group
 #pragma unroll
-  for (int k0 = 0; k0 < KSP; k0 += GK) {
+  for (int k0 = 0; k0 < KS; k0 += GK) {
     c128 a[NCT][GK], b[NCT][GK];
 #pragma unroll
     for (int ti = 0; ti < NCT; ti++)
 #pragma unroll
       for (int kk = 0; kk < GK; kk++)
-        if (k0 + kk < KSP && on[ti]) { a[ti][kk] = ap[ti][4 * (k0 + kk)]; b[ti][kk] = bp[ti][4 * (k0 + kk) * ldt]; }
+        if (k0 + kk < KS && on[ti]) { a[ti][kk] = ap[ti][4 * (k0 + kk)]; b[ti][kk] = bp[ti][4 * (k0 + kk) * ldt]; }
 #pragma unroll
     for (int kk = 0; kk < GK; kk++)
 #pragma unroll
       for (int ti = 0; ti < NCT; ti++)
-        if (k0 + kk < KSP && on[ti]) cmma(sgr[ti], sgi[ti], a[ti][kk], b[ti][kk]);
+        if (k0 + kk < KS && on[ti]) cmma(sgr[ti], sgi[ti], a[ti][kk], b[ti][kk]);
   }
 }
 
@@ -225,11 +228,36 @@ __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t *bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
 
+// ---- thread-block-cluster helpers (a kernel launched without cluster dimensions is a cluster of one) ----
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+// arrive (release at cluster scope) on the mbarrier at the same shared-memory offset in CTA `rank` of this cluster
+__device__ __forceinline__ void mbar_arrive_cluster(uint64_t *bar, unsigned rank) {
+  unsigned remote;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(remote) : "r"(smem_u32(bar)), "r"(rank));
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(remote) : "memory");
+}
+// wait with acquire at cluster scope (the arrivals may come from the peer CTA)
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAITC:\n"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONEC;\n"
+      "bra LAB_WAITC;\n"
+      "DONEC:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
 // exact n / d for n*d < 2^32 (d >= 1), without an integer divide in the inner loops
 struct FastDiv {
   unsigned d, m;
   __host__ __device__ FastDiv() : d(1), m(0) {}
-  __host__ explicit FastDiv(unsigned dd) : d(dd), m(dd <= 1 ? 0u : (unsigned)((1ull << 32) / dd + 1)) {}
+  __host__ __device__ explicit FastDiv(unsigned dd) : d(dd), m(dd <= 1 ? 0u : (unsigned)((1ull << 32) / dd + 1)) {}
   __device__ __forceinline__ unsigned div(unsigned n) const { return m ? __umulhi(n, m) : n; }
 };
 
@@ -257,19 +285,20 @@ __device__ __forceinline__ void ws_issue_rows(c128 *stage, const c128 *src, int 
     cp_async16(stage + r * ldp + a, s + i);
   }
 }
-__device__ __forceinline__ void ws_issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop, FastDiv fd) {
-  const int n2 = nao * nao;
+// K range [a0, a0 + 4*ksp) of one Q: A = Aq[i][a0..] -> stage[i][ldp]; B = Bq[a0..][j] -> [a - a0][ldt]; K beyond nao is zero filled
+__device__ __forceinline__ void ws_issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, int ksp, int naop, FastDiv fd, FastDiv fk, int a0) {
   const int lane = threadIdx.x - 32 * NCONS;
-  for (int i = lane; i < n2; i += NPROD_THR) {
-    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
-    cp_async16(stage + r * ldp + a, Aq + i);
+  const int kw = 4 * ksp;
+  for (int i = lane; i < nao * kw; i += NPROD_THR) {
+    const int r = (int)fk.div((unsigned)i), cc = i - r * kw;
+    const bool ok = a0 + cc < nao;
+    cp_async16_zfill(stage + r * ldp + cc, ok ? Aq + r * nao + a0 + cc : Aq, ok);
   }
   c128 *sB = stage + naop * ldp;
-  const int rowsB = 4 * ksp;
-  for (int i = lane; i < rowsB * nao; i += NPROD_THR) {
+  for (int i = lane; i < kw * nao; i += NPROD_THR) {
     const int r = (int)fd.div((unsigned)i);
-    const bool ok = r < nao;
-    cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + i : Bq, ok);
+    const bool ok = a0 + r < nao;
+    cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + (size_t)a0 * nao + i : Bq, ok);
   }
 }
 // nao x nao matrix -> sG[r][ldp] (TRANSPOSE: sG[c][ldp + r])

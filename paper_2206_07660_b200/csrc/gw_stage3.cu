@@ -24,6 +24,8 @@ struct Params {
   int nqt, nitems;
   int ldp, ksp, ndt;      // pass / G smem row stride, k-steps over nao, tiles over nao
   int ldt;                // row stride of the T block in the final jobs
+  int kh, kspf, ldpf;     // final jobs: K splits per Q, k-steps per split, row stride of the V1 part
+  FastDiv fd_kw;          // divide by 4*kspf
   int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
   int ldb;                // row stride of the main-job B part
   int stage_units, nstage;
@@ -134,9 +136,11 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
           }
           gwp::mbar_wait(bar_phase, ppar); ppar ^= 1u;          // T of this panel is in slabT
           const c128 *V1t = V1 + (size_t)Q0 * n2;
-          for (int j = 0; j < tm_rows; j++) {
+          for (int j = 0; j < tm_rows * P.kh; j++) {
             const int s = ring.acquire();
-            gwp::ws_issue_final(sStage + s * P.stage_units, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldp, P.ldt, P.ksp, naop, P.fd_nao);
+            const int jq = j / P.kh, h = j - jq * P.kh;
+            gwp::ws_issue_final(sStage + s * P.stage_units, V1t + (size_t)jq * n2, slabT + (size_t)jq * n2, nao, P.ldpf, P.ldt, P.kspf, naop,
+                                P.fd_nao, P.fd_kw, 4 * P.kspf * h);
             ring.commit();
           }
         }
@@ -231,10 +235,11 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
           __threadfence(); __syncwarp();
           if (lane == 0) gwp::mbar_arrive(bar_phase);
           // ---- final: Sigma[i][j] += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; one job per Q ----
-          for (int jb = 0; jb < tm_rows; jb++) {
+          for (int jb = 0; jb < tm_rows * P.kh; jb++) {
             const int s = ring.wait();
-            if (P.ksp == KSP_MAX) gwp::final_compute_exact<KSP_MAX, NCT>(sStage + s * P.stage_units, sgr, sgi, ldp, P.ldt, naop);
-            else gwp::final_compute<NCT>(sStage + s * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
+            if (P.ksp == KSP_MAX && P.kh == 1) gwp::final_compute_exact<KSP_MAX, (KSP_MAX + 1) / 2, NCT>(sStage + s * P.stage_units, sgr, sgi, P.ldpf, P.ldt, naop);
+            else if (P.ksp == KSP_MAX && P.kh == 2) gwp::final_compute_exact<(KSP_MAX + 1) / 2, (KSP_MAX + 1) / 2, NCT>(sStage + s * P.stage_units, sgr, sgi, P.ldpf, P.ldt, naop);
+            else gwp::final_compute<NCT>(sStage + s * P.stage_units, sgr, sgi, P.ldpf, P.ldt, P.kspf, ndt, naop);
             ring.release();
           }
         }
@@ -245,7 +250,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
 }
 
 struct Plan {
-  int ksp_max, nct, nqt, nitems, ldp, ksp, ndt, ldt, nnt, nchunk, cht, ldb, stage_units, grid, nstage;
+  int ksp_max, nct, nqt, nitems, ldp, ksp, ndt, ldt, kh, kspf, ldpf, nnt, nchunk, cht, ldb, stage_units, grid, nstage;
   size_t smem, slab_units, work_bytes;
   bool ok;
 };
@@ -268,14 +273,24 @@ static Plan make_plan(const gw_problem *p) {
   pl.ldb = pl.cht * 8 + 2;
   pl.nqt = (d.naux + TM - 1) / TM;
   pl.nitems = d.ntau * d.nk;
-  int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + KC * pl.ldb, s_fin = naop * pl.ldp + 4 * pl.ksp * pl.ldt + 8;
-  pl.stage_units = s_pass;
-  if (s_main > pl.stage_units) pl.stage_units = s_main;
-  if (s_fin > pl.stage_units) pl.stage_units = s_fin;
-  const size_t fixed = (size_t)naop * pl.ldp * sizeof(c128), per = (size_t)pl.stage_units * sizeof(c128);
-  pl.nstage = (int)((225 * 1024 - fixed) / per);
-  if (pl.nstage > 6) pl.nstage = 6;
-  pl.smem = fixed + (size_t)pl.nstage * per;
+  const int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + KC * pl.ldb;
+  const size_t fixed = (size_t)naop * pl.ldp * sizeof(c128);
+  // final jobs cover one Q, or half of its K range when a whole Q would leave fewer than 3 ring stages
+  for (pl.kh = 1; pl.kh <= 2; pl.kh++) {
+    pl.kspf = (pl.ksp + pl.kh - 1) / pl.kh;
+    int f4 = pl.kspf * 4; if (f4 % 8 == 0) f4 += 4;
+    pl.ldpf = f4;
+    const int s_fin = naop * pl.ldpf + 4 * pl.kspf * pl.ldt + 8;
+    pl.stage_units = s_pass;
+    if (s_main > pl.stage_units) pl.stage_units = s_main;
+    if (s_fin > pl.stage_units) pl.stage_units = s_fin;
+    const size_t per = (size_t)pl.stage_units * sizeof(c128);
+    pl.nstage = (int)((225 * 1024 - fixed) / per);
+    if (pl.nstage > 6) pl.nstage = 6;
+    pl.smem = fixed + (size_t)pl.nstage * per;
+    if (pl.nstage >= 3) break;
+  }
+  if (pl.kh > 2) pl.kh = 2;
   int dev = 0, nsm = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
   if (nsm <= 0) nsm = 148;
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
@@ -304,7 +319,7 @@ double gw_stage3_flops(const gw_problem *p) {
     const double mtiles = (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
     tiles += mtiles * pl.nnt * (s3::KC / 4) * nmain;                         // main
     tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.ndt * pl.ksp;           // pass A
-    tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.ksp;                      // final
+    tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.kspf * pl.kh;             // final
   }
   return tiles * (double)d.nq * d.nk * d.ntau * 2048.0;
 }
@@ -324,7 +339,7 @@ int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *S
   s3::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt;
+  P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt; P.kh = pl.kh; P.kspf = pl.kspf; P.ldpf = pl.ldpf; P.fd_kw = gwp::FastDiv((unsigned)(4 * pl.kspf));
   P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
   if (pl.nct == 2) {

@@ -20,6 +20,7 @@ struct Params {
   c128 *part, *scratch;
   unsigned *counter;
   int nitems, ldp, ksp, ndt, ldt, stage_units;
+  int kh, kspf, ldpf;     // final jobs: K splits per Q, k-steps per split, row stride of the X part
   size_t slab_units;
 };
 
@@ -71,17 +72,22 @@ __global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
       }
       cp_async_wait<0>();
       __syncthreads();
+      const int nfin = tm_rows * P.kh;
+      auto issue_fin = [&](int j) {
+        const int jq = j / P.kh, h = j - jq * P.kh;
+        gwp::issue_final_job(sStage + (j % NSTAGE) * P.stage_units, slab + (size_t)jq * n2, V2t + (size_t)jq * n2, nao, P.ldpf, P.ldt, P.kspf, naop, 4 * P.kspf * h);
+      };
       for (issued = 0; issued < NSTAGE - 1; issued++) {
-        if (issued < tm_rows) gwp::issue_final_job(sStage + (issued % NSTAGE) * P.stage_units, slab + (size_t)issued * n2, V2t + (size_t)issued * n2, nao, ldp, P.ldt, P.ksp, naop);
+        if (issued < nfin) issue_fin(issued);
         cp_async_commit();
       }
-      for (int jb = 0; jb < tm_rows; jb++) {
+      for (int jb = 0; jb < nfin; jb++) {
         cp_async_wait<NSTAGE - 2>();
         __syncthreads();
         const int nx = jb + NSTAGE - 1;
-        if (nx < tm_rows) gwp::issue_final_job(sStage + (nx % NSTAGE) * P.stage_units, slab + (size_t)nx * n2, V2t + (size_t)nx * n2, nao, ldp, P.ldt, P.ksp, naop);
+        if (nx < nfin) issue_fin(nx);
         cp_async_commit();
-        gwp::final_compute<NCT>(sStage + (jb % NSTAGE) * P.stage_units, sgr, sgi, ldp, P.ldt, P.ksp, ndt, naop);
+        gwp::final_compute<NCT>(sStage + (jb % NSTAGE) * P.stage_units, sgr, sgi, P.ldpf, P.ldt, P.kspf, ndt, naop);
       }
       cp_async_wait<0>();
       __syncthreads();
@@ -101,7 +107,7 @@ __global__ void exchange_reduce_kernel(GwDims d, const c128 *__restrict__ part, 
   K[i] = make_double2(pref * re, pref * im);
 }
 
-struct Plan { gwp::PassGeom g; int nitems, stage_units, grid; size_t smem, slab_units, part_units, work_bytes; bool ok; };
+struct Plan { gwp::PassGeom g; int nitems, stage_units, grid, kh, kspf, ldpf; size_t smem, slab_units, part_units, work_bytes; bool ok; };
 
 static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
@@ -109,9 +115,17 @@ static Plan make_plan(const gw_problem *p) {
   pl.g = gwp::pass_geom(d.nao);
   if (!pl.g.ok) { pl.ok = false; return pl; }
   pl.nitems = d.nk * d.nq;
-  int s_pass = PASS_ROWS * pl.g.ldp, s_fin = pl.g.naop * pl.g.ldp + 4 * pl.g.ksp * pl.g.ldt + 8;
-  pl.stage_units = s_pass > s_fin ? s_pass : s_fin;
-  pl.smem = ((size_t)pl.g.naop * pl.g.ldp + (size_t)NSTAGE * pl.stage_units) * sizeof(c128);
+  const int s_pass = PASS_ROWS * pl.g.ldp;
+  for (pl.kh = 1; pl.kh <= 2; pl.kh++) {     // a final job covers one Q, or half of its K range if a whole Q does not fit
+    pl.kspf = (pl.g.ksp + pl.kh - 1) / pl.kh;
+    int f4 = pl.kspf * 4; if (f4 % 8 == 0) f4 += 4;
+    pl.ldpf = f4;
+    const int s_fin = pl.g.naop * pl.ldpf + 4 * pl.kspf * pl.g.ldt + 8;
+    pl.stage_units = s_pass > s_fin ? s_pass : s_fin;
+    pl.smem = ((size_t)pl.g.naop * pl.g.ldp + (size_t)NSTAGE * pl.stage_units) * sizeof(c128);
+    if (pl.smem <= 227 * 1024) break;
+  }
+  if (pl.kh > 2) pl.kh = 2;
   const int nsm = gwp::gw_num_sms();
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
@@ -135,7 +149,7 @@ double gw_stage4_flops(const gw_problem *p) {
   double tiles = 0.0;
   for (int Q0 = 0; Q0 < d.naux; Q0 += s4::TM) {
     const int tm_rows = (d.naux - Q0) < s4::TM ? (d.naux - Q0) : s4::TM;
-    tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.g.ndt * pl.g.ksp + (double)tm_rows * pl.g.ndt * pl.g.ndt * pl.g.ksp;
+    tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.g.ndt * pl.g.ksp + (double)tm_rows * pl.g.ndt * pl.g.ndt * pl.kspf * pl.kh;
   }
   return tiles * (double)d.nk * d.nq * 2048.0;
 }
@@ -157,7 +171,7 @@ int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream
   P.counter = (unsigned *)p->work;
   P.scratch = (c128 *)((char *)p->work + 256);
   P.part = P.scratch + (size_t)gwp::gw_num_sms() * pl.slab_units;
-  P.nitems = pl.nitems; P.ldp = pl.g.ldp; P.ksp = pl.g.ksp; P.ndt = pl.g.ndt; P.ldt = pl.g.ldt;
+  P.nitems = pl.nitems; P.ldp = pl.g.ldp; P.ksp = pl.g.ksp; P.ndt = pl.g.ndt; P.ldt = pl.g.ldt; P.kh = pl.kh; P.kspf = pl.kspf; P.ldpf = pl.ldpf;
   P.stage_units = pl.stage_units; P.slab_units = pl.slab_units;
   cudaError_t e = cudaMemsetAsync(p->work, 0, 256, st);
   if (e != cudaSuccess) return (int)e;
