@@ -8,6 +8,15 @@ namespace gwp {
 constexpr int NTHR = 256, NSTAGE = 3;
 constexpr int PASS_ROWS = 64;   // rows per pass job: one 8-row m-tile per warp
 
+// exact n / d for n*d < 2^32 (d >= 1), without an integer divide in the inner loops
+struct FastDiv {
+  unsigned d, m;
+  __host__ __device__ FastDiv() : d(1), m(0) {}
+  __host__ __device__ explicit FastDiv(unsigned dd) : d(dd), m(dd <= 1 ? 0u : (unsigned)((1ull << 32) / dd + 1)) {}
+  __device__ __forceinline__ unsigned div(unsigned n) const { return m ? __umulhi(n, m) : n; }
+};
+
+
 __device__ __forceinline__ void cp_async16_zfill(void *smem, const void *gmem, bool ok) {
   unsigned s = (unsigned)__cvta_generic_to_shared(smem);
   int n = ok ? 16 : 0;
@@ -68,7 +77,7 @@ __device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG,
 template <int KSP, bool TRANSPOSED>
 __device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
                                                    int nao, int ldp, int w = -1) {
-  constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 4, NB = PF + 1;
+  constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 3, NB = PF + 1;
   if (w < 0) w = threadIdx.x >> 5;          // m-tile of this warp within the job
   const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
   if (row0 + 8 * w >= rows_total) return;   // whole m-tile beyond the panel (warp-uniform)
@@ -78,10 +87,11 @@ __device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c12
   for (int ks = 0; ks < KSP; ks++) a[ks] = ap[4 * ks];
   const int row = row0 + 8 * w + g;
   const bool rok = row < rows_total;
-  c128 *o0;
-  size_t ostride;                           // distance between consecutive output columns
-  if (TRANSPOSED) { const int Q = row / nao, x = row - Q * nao; o0 = out + (size_t)Q * nao * nao + x; ostride = (size_t)nao; }
-  else { o0 = out + (size_t)row * nao; ostride = 1; }
+  // this lane's two output columns of n-tile nt are o[nt * 8 * ostride] and o[(nt * 8 + 1) * ostride]
+  c128 *o;
+  int ostride;
+  if (TRANSPOSED) { const int Q = row / nao, x = row - Q * nao; o = out + ((size_t)Q * nao + 2 * c) * nao + x; ostride = nao; }
+  else { o = out + (size_t)row * nao + 2 * c; ostride = 1; }
   const c128 *bp = sG + g * ldp + c;
   c128 b[NB];
 #pragma unroll
@@ -93,12 +103,62 @@ __device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c12
     if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
     cmma(cr, ci, a[ks], b[s % NB]);
     if (ks == KSP - 1) {
-      const int col = 8 * nt + 2 * c;
-      if (rok) {
-        if (col < nao) o0[(size_t)col * ostride] = make_double2(cr[0], ci[0]);
-        if (col + 1 < nao) o0[(size_t)(col + 1) * ostride] = make_double2(cr[1], ci[1]);
-      }
+      // only the last n-tile can reach beyond nao: 8*(NDT-1) <= 4*(KSP-1) < nao
+      if (rok && (nt < NDT - 1 || 8 * nt + 2 * c < nao)) o[0] = make_double2(cr[0], ci[0]);
+      if (rok && (nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao)) o[ostride] = make_double2(cr[1], ci[1]);
+      o += 8 * ostride;
       cr[0] = cr[1] = 0.0; ci[0] = ci[1] = 0.0;
+    }
+  }
+}
+
+// Multi-m-tile variant for dedicated pass warps: warp w owns the MT m-tiles 8*(MT*w + i) of a job; every B fragment is
+// loaded once and used by all MT tiles (2*MT independent accumulator chains).
+template <int KSP, bool TRANSPOSED, int MT>
+__device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
+                                                      int nao, int ldp, int w, FastDiv fd) {
+  constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 3, NB = PF + 1;
+  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
+  const int rbase = row0 + 8 * MT * w;
+  if (rbase >= rows_total) return;          // all m-tiles of this warp beyond the panel (warp-uniform)
+  c128 a[MT][KSP];
+  c128 *o[MT];
+  bool rok[MT];
+  int ostride;
+#pragma unroll
+  for (int i = 0; i < MT; i++) {
+    const c128 *ap = sStage + (8 * (MT * w + i) + g) * ldp + c;
+#pragma unroll
+    for (int ks = 0; ks < KSP; ks++) a[i][ks] = ap[4 * ks];
+    const int row = rbase + 8 * i + g;
+    rok[i] = row < rows_total;
+    if (TRANSPOSED) { const int Q = (int)fd.div((unsigned)row), x = row - Q * nao; o[i] = out + ((size_t)Q * nao + 2 * c) * nao + x; }
+    else o[i] = out + (size_t)row * nao + 2 * c;
+  }
+  ostride = TRANSPOSED ? nao : 1;
+  const c128 *bp = sG + g * ldp + c;
+  c128 b[NB];
+#pragma unroll
+  for (int s = 0; s < PF && s < S; s++) b[s % NB] = bp[(s / KSP) * 8 * ldp + 4 * (s % KSP)];
+  double cr[MT][2], ci[MT][2];
+#pragma unroll
+  for (int i = 0; i < MT; i++) { cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0; }
+#pragma unroll
+  for (int s = 0; s < S; s++) {
+    const int nt = s / KSP, ks = s % KSP;
+    if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
+#pragma unroll
+    for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][ks], b[s % NB]);
+    if (ks == KSP - 1) {
+      // only the last n-tile can reach beyond nao: 8*(NDT-1) <= 4*(KSP-1) < nao
+      const bool c0 = nt < NDT - 1 || 8 * nt + 2 * c < nao, c1 = nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao;
+#pragma unroll
+      for (int i = 0; i < MT; i++) {
+        if (rok[i] && c0) o[i][0] = make_double2(cr[i][0], ci[i][0]);
+        if (rok[i] && c1) o[i][ostride] = make_double2(cr[i][1], ci[i][1]);
+        o[i] += 8 * ostride;
+        cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0;
+      }
     }
   }
 }
@@ -252,14 +312,6 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, unsigned parity
       "DONEC:\n"
       "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-
-// exact n / d for n*d < 2^32 (d >= 1), without an integer divide in the inner loops
-struct FastDiv {
-  unsigned d, m;
-  __host__ __device__ FastDiv() : d(1), m(0) {}
-  __host__ __device__ explicit FastDiv(unsigned dd) : d(dd), m(dd <= 1 ? 0u : (unsigned)((1ull << 32) / dd + 1)) {}
-  __device__ __forceinline__ unsigned div(unsigned n) const { return m ? __umulhi(n, m) : n; }
-};
 
 struct Ring {
   uint64_t *full, *empty;   // [nstage] each

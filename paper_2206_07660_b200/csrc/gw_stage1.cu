@@ -7,57 +7,124 @@
 //   P0t[Q][Q']    = -(s/N_k) Σ_k Σ_(b,c) Z_k[Q][(b,c)] · V[k+q][k][Q'][(b,c)]            (one GEMM,  K = N_k·nao²)
 // so the second operand is the raw V block (rows Q', K contiguous), never transformed.
 //
-// Work decomposition: a persistent CTA owns a row panel [TM Q-rows] x [all naux Q'] of one (t,q) and keeps
-// it in registers over the whole k loop (the k-sum is inside the K loop; no cross-CTA reduction).  Because the
-// panel spans every Q', each Z row is produced exactly once (no recomputation of the V·G transforms across
-// column tiles).  Per k the CTA runs three phases, all on FP64 tensor cores (DMMA.8x8x4, 4-real-GEMM complex
-// scheme) fed by one cp.async stage pipeline:
-//   pass 1:  Xt[Q][b][d] = Σ_a V[k][k+q][Q][d][a] G[t][k+q][a][b]       rows (Q,d) are one flat M dimension
-//   pass 2:  Z [Q][b][c] = Σ_d Xt[Q][b][d] G[tbar][k][c][d]             rows (Q,b) flat; in place
-//   main  :  acc[Q][Q'] += Σ_K Z[Q][K] V[k+q][k][Q'][K],  K = (b,c) = nao² contiguous
-// Xt/Z live in a per-CTA slab of the workspace (TM·nao² complex, written and re-read within ~100 µs, i.e. L2
-// resident); they never exist as a full [t][q][k] tensor.
+// Work decomposition: a work item is a row panel [TM = 32 Q-rows] x [all naux Q'] of one (t,q); it is owned by one CTA
+// (naux <= 224) or by a cluster of two CTAs that split the Q' columns (naux <= 448), and its accumulators stay in
+// registers over the whole k loop (the k-sum is inside the K loop; no cross-CTA reduction, deterministic).
+// A CTA is warp specialised (16 warps, register budgets rebalanced with setmaxnreg):
+//   main warps 0-7   : acc[Q][Q'] += Σ_K Z[Q][K] V[k+q][k][Q'][K] on FP64 tensor cores (DMMA.8x8x4, 4-real-GEMM complex
+//                      scheme), operands streamed through an mbarrier-tracked cp.async ring
+//   pass warps 8-11  : produce Z for the NEXT k while the main warps consume the current one
+//                        pass 1:  Xt[Q][b][d] = Σ_a V[k][k+q][Q][d][a] G[t][k+q][a][b]      rows (Q,d) flat
+//                        pass 2:  Z [Q][b][c] = Σ_d Xt[Q][b][d] G[tbar][k][c][d]            rows (Q,b) flat; in place
+//                      (in a cluster each CTA transforms half of the panel rows)
+//   producer warps   : 12-14 feed the main ring, 15 feeds the pass ring and the G matrices
+// Xt/Z live in two per-cluster slabs of the workspace (TM·nao² complex each, double buffered over k, written and
+// re-read within ~100 µs, i.e. L2 resident); they never exist as a [t][q][k] tensor.
 #include "gw_pipe.cuh"
 
 namespace s1 {
 
-using gwp::NCONS; using gwp::NTHR_WS; using gwp::PASS_ROWS; using gwp::FastDiv; using gwp::Ring;
-constexpr int NSTAGE_MAX = 8;
+using gwp::FastDiv;
+constexpr int NMAINW = 8, NPASSW = 4;                 // main / pass warps; warps 12..15 are the producer warpgroup
+constexpr int NTHR1 = 32 * 16;
+constexpr int T_MPROD = 32 * 12, N_MPROD = 96;        // main-ring producer threads [384, 480)
+constexpr int T_PPROD = 32 * 15, N_PPROD = 32;        // pass-ring producer threads [480, 512)
+constexpr int NST_MAX = 8, PST_MAX = 4;
 constexpr int KC = 8;           // complex K per main job (one 128-byte row per operand row)
-constexpr int MT_W = 2;         // m-tiles per warp in the main GEMM
+constexpr int MT_W = 2;         // m-tiles per main warp
+constexpr int NJ = 7;           // n-tiles per main warp (4 column groups x 7 = 28 n-tiles = 224 columns per CTA)
+constexpr int TM = 32;          // panel rows
+constexpr int REG_MAIN = 176, REG_PASS = 120, REG_PROD = 40;   // 256*176 + 128*120 + 128*40 = 65536
 
 struct Params {
   GwDims d;
   const c128 *V, *G;
   c128 *P0t, *scratch;
+  int cs;                // CTAs per cluster = column splits of the panel
   int nqt, nitems;       // Q tiles per (t,q); total work items
   int ldp, ksp, ndt;     // pass smem row stride (complex), k-steps = ceil(nao/4), n-tiles over nao
-  int nt;                // n-tiles over naux
-  int stage_units;       // complex elements per stage buffer
-  int nstage;            // ring depth (fits shared memory)
-  size_t scratch_stride; // complex elements per CTA slab
+  int nt, ntc;           // n-tiles over naux; n-tiles per CTA
+  int main_units, pass_units;   // complex elements per main / pass stage buffer
+  int prows;                    // rows per pass job: 8 * (m-tiles per pass warp) * 4 pass warps
+  int nstage, pstage, ng;       // ring depths; number of G buffers (2: G[t] and G[tbar] side by side, 1: time shared)
+  size_t slab_units;     // complex elements per slab (two slabs per cluster)
   FastDiv fd_nao;
 };
 
-// main job (producer warp): A = Z[tm rows][k0..k0+8), B = Vb[naux rows][k0..k0+8); 16-byte units swizzled by row parity
-template <int TM>
-__device__ __forceinline__ void ws_issue_main(c128 *stage, const c128 *Z, int tm_rows, const c128 *Vb, int naux, int brows, int n2, int k0) {
-  const int pt = threadIdx.x - 32 * NCONS;
-  const int u = pt & 7, rsub = pt >> 3;                // 16 rows x 8 units per pass of the producer warpgroup
+// ring bookkeeping (same job sequence on the producer and the consumer side)
+struct Ring {
+  uint64_t *full, *empty;
+  int nstage; unsigned it;
+  __device__ __forceinline__ int stage() const { return (int)(it % (unsigned)nstage); }
+  __device__ __forceinline__ unsigned round() const { return it / (unsigned)nstage; }
+  __device__ __forceinline__ int acquire() { const int s = stage(); gwp::mbar_wait(empty + s, (round() & 1u) ^ 1u); return s; }
+  __device__ __forceinline__ void commit() { gwp::cp_async_arrive_noinc(full + stage()); ++it; }
+  __device__ __forceinline__ int wait() { const int s = stage(); gwp::mbar_wait(full + s, round() & 1u); return s; }
+  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); ++it; }
+};
+
+// main job: A = Z[TM rows][k0..k0+8), B = Vb[brows rows][k0..k0+8); 16-byte units swizzled by row parity.
+// Rows beyond the valid range re-read the last valid row (their products land in accumulators that are never stored);
+// only the K tail of the last job is zero filled.  Each thread owns one 16-byte unit column and walks the rows with
+// constant strides, so the loop body is one address add per copy.
+__device__ __forceinline__ void issue_main(c128 *stage, const c128 *Z, int tm_rows, const c128 *Vb, int ncols, int brows, int n2, int k0) {
+  constexpr int RS = N_MPROD / 8;                      // rows per sweep of the producer threads
+  const int pt = threadIdx.x - T_MPROD;
+  const int u = pt & 7, rsub = pt >> 3;
   const bool kok = k0 + u < n2;
-  for (int r = rsub; r < TM; r += 16) {
-    const bool ok = kok && (r < tm_rows);
-    gwp::cp_async16_zfill(stage + r * KC + (u ^ ((r & 1) << 2)), ok ? Z + (size_t)r * n2 + k0 + u : Z, ok);
+  const int nbytes = kok ? 16 : 0;
+  const int koff = kok ? k0 + u : 0;
+  const unsigned sbase = gwp::smem_u32(stage) + 16u * (unsigned)u;
+  {
+    const c128 *src = Z + koff;
+#pragma unroll
+    for (int r = rsub; r < TM; r += RS) {
+      const int rr = min(r, tm_rows - 1);
+      const unsigned dst = (sbase + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src + (size_t)rr * n2), "r"(nbytes));
+    }
   }
-  c128 *sB = stage + TM * KC;
-  for (int r = rsub; r < brows; r += 16) {
-    const bool ok = kok && (r < naux);
-    gwp::cp_async16_zfill(sB + r * KC + (u ^ ((r & 1) << 2)), ok ? Vb + (size_t)r * n2 + k0 + u : Vb, ok);
+  const unsigned sB = sbase + 16u * TM * KC;
+  const c128 *src = Vb + koff;
+  const size_t step = (size_t)RS * n2;
+  int r = rsub;
+  const c128 *sp = src + (size_t)r * n2;
+  for (; r + 3 * RS < ncols; r += 4 * RS, sp += 4 * step) {      // rows r, r+RS, r+2RS, r+3RS all valid (RS is even: same row parity)
+    const unsigned dst = (sB + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(sp), "r"(nbytes));
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst + RS * 16u * KC), "l"(sp + step), "r"(nbytes));
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst + 2 * RS * 16u * KC), "l"(sp + 2 * step), "r"(nbytes));
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst + 3 * RS * 16u * KC), "l"(sp + 3 * step), "r"(nbytes));
+  }
+  for (; r < brows; r += RS) {
+    const int rr = min(r, ncols - 1);
+    const unsigned dst = (sB + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src + (size_t)rr * n2), "r"(nbytes));
   }
 }
 
-// consumer: one main job (KC/4 k-steps) for this warp's MT_W x NJM tiles; all fragment loads hoisted per k-step
-template <int NJ, int NJM, int NSTRIDE>
+// rows [row0, row0+prows) of a dense (rows x nao) matrix -> stage[r][ldp]   (pass-ring producer warp)
+__device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd, int prows) {
+  const int nrow = min(prows, rows_total - row0);
+  const int total = nrow * nao;
+  const c128 *s = src + (size_t)row0 * nao;
+  for (int i = threadIdx.x - T_PPROD; i < total; i += N_PPROD) {
+    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
+    cp_async16(stage + r * ldp + a, s + i);
+  }
+}
+// nao x nao matrix -> sG[r][ldp] (TRANSPOSE: sG[c][ldp + r])
+template <bool TRANSPOSE>
+__device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao, int ldp, FastDiv fd) {
+  const int n2 = nao * nao;
+  for (int i = threadIdx.x - T_PPROD; i < n2; i += N_PPROD) {
+    const int r = (int)fd.div((unsigned)i), cc = i - r * nao;
+    cp_async16(TRANSPOSE ? sG + cc * ldp + r : sG + r * ldp + cc, src + i);
+  }
+}
+
+// main warps: one main job (KC/4 k-steps) for this warp's MT_W x NJM tiles; all fragment loads hoisted per k-step
+template <int NJM>
 __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
@@ -66,7 +133,7 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
 #pragma unroll
     for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++) b[jn] = sBw[jn * NSTRIDE * 8 * KC + u];
+    for (int jn = 0; jn < NJM; jn++) b[jn] = sBw[jn * 4 * 8 * KC + u];
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++)
 #pragma unroll
@@ -74,124 +141,193 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
   }
 }
 
-template <int NJ, int MH, int KSP_MAX>
-__global__ void __launch_bounds__(NTHR_WS, 1) p0_kernel(const Params P) {
-  constexpr int TM = 8 * MT_W * MH;
-  constexpr int NSTRIDE = 8 / MH;
+// decode a work item: Q-tile index slowest (the round-robin gives every cluster the same mix of full and ragged tiles),
+// then q, then t fastest (concurrent clusters share the V blocks of one q in L2)
+struct Item { int t, ql, Q0, tm_rows; };
+__device__ __forceinline__ Item decode_item(const GwDims &d, int item) {
+  Item it;
+  const int qt = item / (d.ntau * d.nq);
+  it.t = item % d.ntau; it.ql = (item / d.ntau) % d.nq; it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
+  return it;
+}
+
+template <int KSP_MAX>
+__global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   c128 *smem = reinterpret_cast<c128 *>(smem_raw);
   const GwDims d = P.d;
   const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, naop = 8 * P.ndt;
-  c128 *sGt = smem;                       // [naop][ldp]: sGt[b][a] = G[t][k+q][a][b]
-  c128 *sGm = sGt + naop * ldp;           // [naop][ldp]: sGm[c][d] = G[tbar][k][c][d]
-  c128 *sStage = sGm + naop * ldp;        // nstage x stage_units
-  const int NSTAGE = P.nstage;
-  __shared__ uint64_t bars[2 * NSTAGE_MAX + 2];
-  uint64_t *bar_full = bars, *bar_empty = bars + NSTAGE_MAX, *bar_g = bars + 2 * NSTAGE_MAX, *bar_phase = bars + 2 * NSTAGE_MAX + 1;
+  c128 *sG0 = smem;                                       // pass 1: sG0[b][a] = G[t][k+q][a][b]
+  c128 *sG1 = sG0 + (P.ng == 2 ? naop * ldp : 0);         // pass 2: sG1[c][d] = G[tbar][k][c][d]  (== sG0 when time shared)
+  c128 *sPass = smem + P.ng * naop * ldp;                 // pstage x pass_units
+  c128 *sMain = sPass + P.pstage * P.pass_units;          // nstage x main_units
+  __shared__ uint64_t bars[2 * NST_MAX + 2 * PST_MAX + 6];
+  uint64_t *full_m = bars, *empty_m = bars + NST_MAX, *full_p = bars + 2 * NST_MAX, *empty_p = full_p + PST_MAX;
+  uint64_t *bar_g = empty_p + PST_MAX, *bar_phase = bar_g + 1, *zready = bar_g + 2, *zfree = bar_g + 4;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  c128 *slab = P.scratch + (size_t)blockIdx.x * P.scratch_stride;
+  const int cs = P.cs;
+  const unsigned rank = cs > 1 ? gwp::cluster_ctarank() : 0u;
+  const int cid = blockIdx.x / cs, ncl = gridDim.x / cs;
+  c128 *slab0 = P.scratch + (size_t)cid * 2 * P.slab_units;
   const size_t vb = (size_t)naux * n2;
-  const int brows = 8 * P.nt;
+  const int nmain = (n2 + KC - 1) / KC;
+  const int rows_cta = TM / cs;                           // panel rows transformed by this CTA's pass warps
+  const int r0 = (int)rank * rows_cta;
+  const int col0 = 8 * (int)rank * P.ntc;                 // first Q' column of this CTA
+  const int ncols = max(0, min(naux - col0, 8 * P.ntc));
+  const int ntc_mine = (ncols + 7) / 8;
 
   // zero all dynamic smem once (pad rows/columns must hold finite values: they meet zero operands); init barriers
   {
-    const int tot = 2 * naop * ldp + NSTAGE * P.stage_units;
-    for (int i = threadIdx.x; i < tot; i += NTHR_WS) smem[i] = make_double2(0.0, 0.0);
+    const int tot = P.ng * naop * ldp + P.pstage * P.pass_units + P.nstage * P.main_units;
+    for (int i = threadIdx.x; i < tot; i += NTHR1) smem[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
-      for (int i = 0; i < NSTAGE; i++) { gwp::mbar_init(bar_full + i, gwp::NPROD_THR); gwp::mbar_init(bar_empty + i, NCONS); }
-      gwp::mbar_init(bar_g, gwp::NPROD_THR);
-      gwp::mbar_init(bar_phase, NCONS);
+      for (int i = 0; i < P.nstage; i++) { gwp::mbar_init(full_m + i, N_MPROD); gwp::mbar_init(empty_m + i, NMAINW); }
+      for (int i = 0; i < P.pstage; i++) { gwp::mbar_init(full_p + i, N_PPROD); gwp::mbar_init(empty_p + i, NPASSW); }
+      gwp::mbar_init(bar_g, N_PPROD);
+      gwp::mbar_init(bar_phase, NPASSW);
+      for (int i = 0; i < 2; i++) { gwp::mbar_init(zready + i, NPASSW * cs); gwp::mbar_init(zfree + i, NMAINW * cs); }
+      asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
   }
   __syncthreads();
-  Ring ring; ring.full = bar_full; ring.empty = bar_empty; ring.nstage = NSTAGE; ring.it = 0;
-  unsigned gpar = 0, ppar = 0;     // parities of bar_g / bar_phase (advance identically on both sides)
-  const int nmain = (n2 + KC - 1) / KC;
+  if (cs > 1) gwp::cluster_sync_all();
 
-  if (w >= NCONS) {
-    // =============================== producer warp ===============================
-    gwp::reg_dec<40>();
-    for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      // item order: Q-tile index slowest (so the round-robin gives every CTA the same mix of full and ragged tiles),
-      // then q, then t fastest (concurrent CTAs share the V blocks of one q in L2)
-      const int qt = item / (d.ntau * d.nq), t = item % d.ntau, ql = (item / d.ntau) % d.nq;
-      const int q = d.q0 + ql, Q0 = qt * TM;
-      const int tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
-      for (int k = 0; k < d.nk; k++) {
-        const int kq = gw_kadd(d, k, q);
-        const c128 *Vt = P.V + ((size_t)k * d.nk + kq) * vb + (size_t)Q0 * n2;
-        const c128 *Vb = P.V + ((size_t)kq * d.nk + k) * vb;
-        // G matrices of this k (consumers finished the passes of the previous k: see the phase wait below)
-        gwp::ws_issue_matrix<true>(sGt, P.G + ((size_t)t * d.nk + kq) * n2, nao, ldp, P.fd_nao);
-        gwp::ws_issue_matrix<false>(sGm, P.G + ((size_t)(d.ntau - 1 - t) * d.nk + k) * n2, nao, ldp, P.fd_nao);
-        gwp::cp_async_arrive_noinc(bar_g);
-        for (int j = 0; j < npass; j++) {
-          const int s = ring.acquire();
-          gwp::ws_issue_rows(sStage + s * P.stage_units, Vt, j * PASS_ROWS, rows, nao, ldp, P.fd_nao);
-          ring.commit();
-        }
-        gwp::mbar_wait(bar_phase, ppar); ppar ^= 1u;          // all Xt rows are in the slab
-        for (int j = 0; j < npass; j++) {
-          const int s = ring.acquire();
-          gwp::ws_issue_rows(sStage + s * P.stage_units, slab, j * PASS_ROWS, rows, nao, ldp, P.fd_nao);
-          ring.commit();
-        }
-        gwp::mbar_wait(bar_phase, ppar); ppar ^= 1u;          // Z complete; sGt/sGm free for the next k
-        for (int j = 0; j < nmain; j++) {
-          const int s = ring.acquire();
-          ws_issue_main<TM>(sStage + s * P.stage_units, slab, tm_rows, Vb, naux, brows, n2, j * KC);
-          ring.commit();
+  if (w >= NMAINW + NPASSW) {
+    // ====================================== producer warpgroup ======================================
+    gwp::reg_dec<REG_PROD>();
+    if (w < 15) {
+      // ---- main-ring producer (96 threads): Z of the current k and the raw V[k+q][k] rows of this CTA's columns ----
+      Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0;
+      unsigned kit = 0;
+      const int brows = 8 * ntc_mine;
+      for (int item = cid; item < P.nitems; item += ncl) {
+        const Item it = decode_item(d, item);
+        const int q = d.q0 + it.ql;
+        for (int k = 0; k < d.nk; k++, kit++) {
+          const int kq = gw_kadd(d, k, q);
+          const c128 *Vb = P.V + ((size_t)kq * d.nk + k) * vb + (size_t)col0 * n2;
+          const c128 *Z = slab0 + (size_t)(kit & 1u) * P.slab_units;
+          if (cs > 1) gwp::mbar_wait_cluster(zready + (kit & 1u), (kit >> 1) & 1u);
+          else gwp::mbar_wait(zready + (kit & 1u), (kit >> 1) & 1u);
+          for (int j = 0; j < nmain; j++) {
+            const int s = rm.acquire();
+            issue_main(sMain + s * P.main_units, Z, it.tm_rows, Vb, ncols, brows, n2, j * KC);
+            rm.commit();
+          }
         }
       }
+      asm volatile("cp.async.wait_all;\n" ::: "memory");
+    } else {
+      // ---- pass-ring producer (32 threads): G matrices, V[k][k+q] rows (pass 1), Xt rows from the slab (pass 2) ----
+      Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0;
+      unsigned kit = 0, ph = 0;
+      for (int item = cid; item < P.nitems; item += ncl) {
+        const Item it = decode_item(d, item);
+        const int q = d.q0 + it.ql;
+        const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
+        for (int k = 0; k < d.nk; k++, kit++) {
+          const int kq = gw_kadd(d, k, q);
+          const c128 *Vt = P.V + ((size_t)k * d.nk + kq) * vb + (size_t)(it.Q0 + r0) * n2;
+          const c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
+          const c128 *Gt = P.G + ((size_t)it.t * d.nk + kq) * n2, *Gm = P.G + ((size_t)(d.ntau - 1 - it.t) * d.nk + k) * n2;
+          // pass 1 (its G buffer was last read two phases ago; a time-shared buffer must wait for the previous phase)
+          if (P.ng == 2) issue_matrix<true>(sG0, Gt, nao, ldp, P.fd_nao);
+          if (ph > 0) gwp::mbar_wait(bar_phase, (ph - 1) & 1u);
+          if (P.ng == 1) issue_matrix<true>(sG0, Gt, nao, ldp, P.fd_nao);
+          gwp::cp_async_arrive_noinc(bar_g);
+          for (int j = 0; j < npass; j++) {
+            const int s = rp.acquire();
+            issue_rows(sPass + s * P.pass_units, Vt, j * P.prows, my_rows, nao, ldp, P.fd_nao, P.prows);
+            rp.commit();
+          }
+          ph++;
+          // pass 2: reads the Xt rows written by pass 1
+          if (P.ng == 2) issue_matrix<false>(sG1, Gm, nao, ldp, P.fd_nao);
+          gwp::mbar_wait(bar_phase, (ph - 1) & 1u);
+          if (P.ng == 1) issue_matrix<false>(sG1, Gm, nao, ldp, P.fd_nao);
+          gwp::cp_async_arrive_noinc(bar_g);
+          for (int j = 0; j < npass; j++) {
+            const int s = rp.acquire();
+            issue_rows(sPass + s * P.pass_units, Xs, j * P.prows, my_rows, nao, ldp, P.fd_nao, P.prows);
+            rp.commit();
+          }
+          ph++;
+        }
+      }
+      asm volatile("cp.async.wait_all;\n" ::: "memory");
     }
-    asm volatile("cp.async.wait_all;\n" ::: "memory");
+  } else if (w >= NMAINW) {
+    // ========================================= pass warps =========================================
+    if constexpr (REG_PASS > 65536 / NTHR1) gwp::reg_inc<REG_PASS>(); else gwp::reg_dec<REG_PASS>();
+    const int wp = w - NMAINW;
+    constexpr int PMT = 1;                             // m-tiles per pass warp (prows = 32*PMT); 2 measured slower (fewer main registers)
+    Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0;
+    unsigned kit = 0, ph = 0;
+    for (int item = cid; item < P.nitems; item += ncl) {
+      const Item it = decode_item(d, item);
+      const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
+      for (int k = 0; k < d.nk; k++, kit++) {
+        c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
+        // this slab was read by the main GEMM of iteration kit-2
+        if (kit >= 2) {
+          if (cs > 1) gwp::mbar_wait_cluster(zfree + (kit & 1u), ((kit >> 1) - 1u) & 1u);
+          else gwp::mbar_wait(zfree + (kit & 1u), ((kit >> 1) - 1u) & 1u);
+        }
+        gwp::mbar_wait(bar_g, ph & 1u);
+        for (int j = 0; j < npass; j++) {
+          const int s = rp.wait();
+          if (P.ksp == KSP_MAX) gwp::pass_compute_exact_mt<KSP_MAX, true, PMT>(sPass + s * P.pass_units, sG0, Xs, j * P.prows, my_rows, nao, ldp, wp, P.fd_nao);
+          else gwp::pass_compute<KSP_MAX, true>(sPass + s * P.pass_units, sG0, Xs, j * P.prows, my_rows, nao, ldp, P.ksp, P.ndt, wp);
+          rp.release();
+        }
+        __threadfence(); __syncwarp();
+        if (lane == 0) gwp::mbar_arrive(bar_phase);
+        ph++;
+        gwp::mbar_wait(bar_g, ph & 1u);
+        for (int j = 0; j < npass; j++) {
+          const int s = rp.wait();
+          if (P.ksp == KSP_MAX) gwp::pass_compute_exact_mt<KSP_MAX, false, PMT>(sPass + s * P.pass_units, sG1, Xs, j * P.prows, my_rows, nao, ldp, wp, P.fd_nao);
+          else gwp::pass_compute<KSP_MAX, false>(sPass + s * P.pass_units, sG1, Xs, j * P.prows, my_rows, nao, ldp, P.ksp, P.ndt, wp);
+          rp.release();
+        }
+        __threadfence(); __syncwarp();
+        if (lane == 0) {
+          gwp::mbar_arrive(bar_phase);
+          if (cs > 1) { for (int r = 0; r < cs; r++) gwp::mbar_arrive_cluster(zready + (kit & 1u), (unsigned)r); }
+          else gwp::mbar_arrive(zready + (kit & 1u));
+        }
+        ph++;
+      }
+    }
   } else {
-    // =============================== consumer warps ===============================
-    gwp::reg_inc<232>();
+    // ========================================= main warps =========================================
+    gwp::reg_inc<REG_MAIN>();
     const int g = lane >> 2, c = lane & 3;
-    const int mh = (MH == 2) ? (w >> 2) : 0;
-    const int noff = (MH == 2) ? (((w & 3) - mh + 4) & 3) : w;
-    const int njm = (P.nt > noff) ? (P.nt - noff + NSTRIDE - 1) / NSTRIDE : 0;   // n-tiles owned by this warp
+    const int mh = w >> 2;                               // m-half: m-tiles 2*mh, 2*mh+1
+    const int noff = ((w & 3) - mh + 4) & 3;             // first n-tile; n-tiles noff + 4*jn
+    const int njm = (ntc_mine > noff) ? (ntc_mine - noff + 3) / 4 : 0;
     const int sw = (g & 1) << 2;
-    for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      // item order: Q-tile index slowest (so the round-robin gives every CTA the same mix of full and ragged tiles),
-      // then q, then t fastest (concurrent CTAs share the V blocks of one q in L2)
-      const int qt = item / (d.ntau * d.nq), t = item % d.ntau, ql = (item / d.ntau) % d.nq;
-      const int Q0 = qt * TM;
-      const int tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
-      const int mtc = (tm_rows + 7) / 8;
+    Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0;
+    unsigned kit = 0;
+    for (int item = cid; item < P.nitems; item += ncl) {
+      const Item it = decode_item(d, item);
+      const int mtc = (it.tm_rows + 7) / 8;
+      const bool active = (mh * MT_W < mtc) && njm > 0;
       double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
 #pragma unroll
       for (int i = 0; i < MT_W; i++)
 #pragma unroll
         for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
 
-      for (int k = 0; k < d.nk; k++) {
-        gwp::mbar_wait(bar_g, gpar); gpar ^= 1u;
-        for (int j = 0; j < npass; j++) {
-          const int s = ring.wait();
-          if (P.ksp == KSP_MAX) gwp::pass_compute_exact<KSP_MAX, true>(sStage + s * P.stage_units, sGt, slab, j * PASS_ROWS, rows, nao, ldp);
-          else gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sGt, slab, j * PASS_ROWS, rows, nao, ldp, P.ksp, P.ndt);
-          ring.release();
-        }
-        __threadfence(); __syncwarp();
-        if (lane == 0) gwp::mbar_arrive(bar_phase);
-        for (int j = 0; j < npass; j++) {
-          const int s = ring.wait();
-          if (P.ksp == KSP_MAX) gwp::pass_compute_exact<KSP_MAX, false>(sStage + s * P.stage_units, sGm, slab, j * PASS_ROWS, rows, nao, ldp);
-          else gwp::pass_compute<KSP_MAX, false>(sStage + s * P.stage_units, sGm, slab, j * PASS_ROWS, rows, nao, ldp, P.ksp, P.ndt);
-          ring.release();
-        }
-        __threadfence(); __syncwarp();
-        if (lane == 0) gwp::mbar_arrive(bar_phase);
-        const bool active = (mh * MT_W < mtc) && njm > 0;
+      for (int k = 0; k < d.nk; k++, kit++) {
         for (int j = 0; j < nmain; j++) {
-          const int s = ring.wait();
+          const int s = rm.wait();
           if (active) {
-            const c128 *sAw = sStage + s * P.stage_units + (8 * mh * MT_W + g) * KC;
-            const c128 *sBw = sStage + s * P.stage_units + TM * KC + (8 * noff + g) * KC;
-            if (njm == NJ) main_compute<NJ, NJ, NSTRIDE>(sAw, sBw, accr, acci, c, sw);
-            else if (njm == NJ - 1) main_compute<NJ, NJ - 1, NSTRIDE>(sAw, sBw, accr, acci, c, sw);
+            const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + g) * KC;
+            const c128 *sBw = sMain + s * P.main_units + TM * KC + (8 * noff + g) * KC;
+            if (njm == NJ) main_compute<NJ>(sAw, sBw, accr, acci, c, sw);
+            else if (njm == NJ - 1) main_compute<NJ - 1>(sAw, sBw, accr, acci, c, sw);
             else {
 #pragma unroll
               for (int ks = 0; ks < KC / 4; ks++) {
@@ -202,7 +338,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) p0_kernel(const Params P) {
 #pragma unroll
                 for (int jn = 0; jn < NJ; jn++) {
                   if (jn < njm) {
-                    const c128 b = sBw[jn * NSTRIDE * 8 * KC + u];
+                    const c128 b = sBw[jn * 4 * 8 * KC + u];
 #pragma unroll
                     for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
                   }
@@ -210,31 +346,38 @@ __global__ void __launch_bounds__(NTHR_WS, 1) p0_kernel(const Params P) {
               }
             }
           }
-          ring.release();
+          rm.release();
+        }
+        // every cp.async read of this k's slab has landed: hand it back to the pass warps (of all CTAs in the cluster)
+        if (lane == 0) {
+          if (cs > 1) { for (int r = 0; r < cs; r++) gwp::mbar_arrive_cluster(zfree + (kit & 1u), (unsigned)r); }
+          else gwp::mbar_arrive(zfree + (kit & 1u));
         }
       }
-      // ---- epilogue: scale by -(s/N_k), store the panel ----
+      // ---- epilogue: scale by -(s/N_k), store this CTA's columns of the panel ----
       const double pref = -(double)d.s / (double)d.nk;
-      c128 *out = P.P0t + ((size_t)t * d.nq + ql) * naux * naux;
+      c128 *out = P.P0t + ((size_t)it.t * d.nq + it.ql) * naux * naux + col0;
 #pragma unroll
       for (int i = 0; i < MT_W; i++) {
-        const int Q = Q0 + 8 * (mh * MT_W + i) + g;
+        const int Q = it.Q0 + 8 * (mh * MT_W + i) + g;
 #pragma unroll
         for (int jn = 0; jn < NJ; jn++) {
           if (jn < njm && Q < naux) {
-            const int col = 8 * (noff + NSTRIDE * jn) + 2 * c;
-            if (col < naux) out[(size_t)Q * naux + col] = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
-            if (col + 1 < naux) out[(size_t)Q * naux + col + 1] = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
+            const int col = 8 * (noff + 4 * jn) + 2 * c;
+            if (col < ncols) out[(size_t)Q * naux + col] = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
+            if (col + 1 < ncols) out[(size_t)Q * naux + col + 1] = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
           }
         }
       }
     }
   }
+  // a CTA must not exit while its peer may still arrive on its barriers
+  if (cs > 1) gwp::cluster_sync_all();
 }
 
 struct Plan {
-  int mh, ksp_max, TM, nqt, nitems, ldp, ksp, ndt, nt, stage_units, grid, nstage;
-  size_t smem, scratch_stride, work_bytes;
+  int cs, ksp_max, nqt, nitems, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
+  size_t smem, slab_units, work_bytes;
   bool ok;
 };
 
@@ -242,27 +385,36 @@ static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
   GwDims d = gw_dims(p);
   pl.nt = (d.naux + 7) / 8;
-  if (pl.nt <= 28) pl.mh = 2; else if (pl.nt <= 56) pl.mh = 1; else { pl.ok = false; return pl; }
-  pl.TM = 8 * MT_W * pl.mh;
+  if (pl.nt <= 4 * NJ) pl.cs = 1; else if (pl.nt <= 8 * NJ) pl.cs = 2; else { pl.ok = false; return pl; }
+  pl.ntc = (pl.nt + pl.cs - 1) / pl.cs;
   pl.ksp = (d.nao + 3) / 4;
   pl.ksp_max = pl.ksp <= 7 ? 7 : (pl.ksp <= 13 ? 13 : 16);
   if (pl.ksp > 16) { pl.ok = false; return pl; }
   pl.ndt = (d.nao + 7) / 8;
   int r4 = pl.ksp * 4; if (r4 % 8 == 0) r4 += 4;
   pl.ldp = r4;
-  pl.nqt = (d.naux + pl.TM - 1) / pl.TM;
+  pl.nqt = (d.naux + TM - 1) / TM;
   pl.nitems = pl.nqt * d.ntau * d.nq;
-  int s_pass = PASS_ROWS * pl.ldp, s_main = (pl.TM + 8 * pl.nt) * KC;
-  pl.stage_units = s_pass > s_main ? s_pass : s_main;
-  const size_t fixed = (size_t)2 * 8 * pl.ndt * pl.ldp * sizeof(c128), per = (size_t)pl.stage_units * sizeof(c128);
-  pl.nstage = (int)((225 * 1024 - fixed) / per);
-  if (pl.nstage > 6) pl.nstage = 6;
-  pl.smem = fixed + (size_t)pl.nstage * per;
-  int dev = 0, nsm = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-  if (nsm <= 0) nsm = 148;
-  pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
-  pl.scratch_stride = (((size_t)pl.TM * d.nao * d.nao) + 15) / 16 * 16;
-  pl.work_bytes = 256 + (size_t)nsm * pl.scratch_stride * sizeof(c128);
+  pl.main_units = (TM + 8 * pl.ntc) * KC;
+  pl.prows = 32;
+  pl.pass_units = pl.prows * pl.ldp;
+  // shared memory: prefer both G matrices resident and a 3-deep pass ring; shrink them while the main ring has < 4 stages
+  const size_t gsz = (size_t)8 * pl.ndt * pl.ldp * sizeof(c128), psz = (size_t)pl.pass_units * sizeof(c128), msz = (size_t)pl.main_units * sizeof(c128);
+  const size_t cap = 226 * 1024;
+  const int tryng[4] = {2, 2, 1, 1}, tryps[4] = {3, 2, 3, 2};
+  for (int i = 0; i < 4; i++) {
+    pl.ng = tryng[i]; pl.pstage = tryps[i];
+    const size_t fixed = pl.ng * gsz + pl.pstage * psz;
+    pl.nstage = fixed < cap ? (int)((cap - fixed) / msz) : 0;
+    if (pl.nstage > 6) pl.nstage = 6;
+    pl.smem = fixed + (size_t)pl.nstage * msz;
+    if (pl.nstage >= 4) break;
+  }
+  const int nsm = gwp::gw_num_sms();
+  pl.nclusters = nsm / pl.cs;
+  if (pl.nclusters > pl.nitems) pl.nclusters = pl.nitems;
+  pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
+  pl.work_bytes = 256 + (size_t)nsm * 2 * pl.slab_units * sizeof(c128);
   pl.ok = pl.nstage >= 2;
   return pl;
 }
@@ -281,9 +433,14 @@ double gw_stage1_flops(const gw_problem *p) {
   GwDims d = gw_dims(p);
   double tiles = 0.0;
   for (int qt = 0; qt < pl.nqt; qt++) {
-    const int tm_rows = (d.naux - qt * pl.TM) < pl.TM ? (d.naux - qt * pl.TM) : pl.TM;
-    const int rows = tm_rows * d.nao;
-    const double mt_pass = (rows + 7) / 8;
+    const int tm_rows = (d.naux - qt * s1::TM) < s1::TM ? (d.naux - qt * s1::TM) : s1::TM;
+    double mt_pass = 0.0;                       // 8-row m-tiles of the two passes, per CTA of the cluster
+    for (int r = 0; r < pl.cs; r++) {
+      const int r0 = r * (s1::TM / pl.cs);
+      int rows = tm_rows < r0 + s1::TM / pl.cs ? tm_rows - r0 : s1::TM / pl.cs;
+      if (rows < 0) rows = 0;
+      mt_pass += (rows * d.nao + 7) / 8;
+    }
     const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp;
     const int mtc = (tm_rows + 7) / 8;
     // main: warps whose first m-tile is valid execute MT_W m-tiles x their n-tiles x 2 k-steps per job
@@ -295,12 +452,29 @@ double gw_stage1_flops(const gw_problem *p) {
   return tiles * (double)d.nk * d.ntau * d.nq * 2048.0;
 }
 
-template <int NJ, int MH, int KSP_MAX>
+template <int KSP_MAX>
 static int launch_p0(const s1::Plan &pl, const s1::Params &P, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(s1::p0_kernel<NJ, MH, KSP_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  cudaError_t e = cudaFuncSetAttribute(s1::p0_kernel<KSP_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
-  s1::p0_kernel<NJ, MH, KSP_MAX><<<pl.grid, s1::NTHR_WS, pl.smem, st>>>(P);
-  return (int)cudaGetLastError();
+  cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof(cfg));
+  cudaLaunchAttribute attr[1];
+  cfg.blockDim = dim3(s1::NTHR1, 1, 1);
+  cfg.dynamicSmemBytes = pl.smem;
+  cfg.stream = st;
+  int ncl = pl.nclusters;
+  if (pl.cs > 1) {
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = pl.cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    // co-resident clusters (a GPC with an odd number of free SMs leaves one unpaired)
+    cfg.gridDim = dim3(pl.cs * ncl, 1, 1);
+    int maxcl = 0;
+    if (cudaOccupancyMaxActiveClusters(&maxcl, s1::p0_kernel<KSP_MAX>, &cfg) == cudaSuccess && maxcl > 0 && maxcl < ncl) ncl = maxcl;
+    else cudaGetLastError();
+  }
+  cfg.gridDim = dim3(pl.cs * ncl, 1, 1);
+  e = cudaLaunchKernelEx(&cfg, s1::p0_kernel<KSP_MAX>, P);
+  return (int)e;
 }
 
 int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t st) {
@@ -310,16 +484,11 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   s1::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt;
-  P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.scratch_stride = pl.scratch_stride;
+  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
+  P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
+  P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
-  if (pl.mh == 2) {
-    if (pl.ksp_max == 7) return launch_p0<7, 2, 7>(pl, P, st);
-    if (pl.ksp_max == 13) return launch_p0<7, 2, 13>(pl, P, st);
-    return launch_p0<7, 2, 16>(pl, P, st);
-  } else {
-    if (pl.ksp_max == 7) return launch_p0<7, 1, 7>(pl, P, st);
-    if (pl.ksp_max == 13) return launch_p0<7, 1, 13>(pl, P, st);
-    return launch_p0<7, 1, 16>(pl, P, st);
-  }
+  if (pl.ksp_max == 7) return launch_p0<7>(pl, P, st);
+  if (pl.ksp_max == 13) return launch_p0<13>(pl, P, st);
+  return launch_p0<16>(pl, P, st);
 }
