@@ -316,15 +316,16 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, unsigned parity
 struct Ring {
   uint64_t *full, *empty;   // [nstage] each
   int nstage;
-  unsigned it;              // job counter (same sequence on both sides)
-  __device__ __forceinline__ int stage() const { return (int)(it % (unsigned)nstage); }
-  __device__ __forceinline__ unsigned round() const { return it / (unsigned)nstage; }
+  unsigned it;              // stage index of the next job (same sequence on both sides)
+  unsigned ph = 0;          // parity of the current round (no integer division per job)
+  __device__ __forceinline__ int stage() const { return (int)it; }
+  __device__ __forceinline__ void advance() { if (++it == (unsigned)nstage) { it = 0; ph ^= 1u; } }
   // producer side
-  __device__ __forceinline__ int acquire() { const int s = stage(); mbar_wait(empty + s, (round() & 1u) ^ 1u); return s; }
-  __device__ __forceinline__ void commit() { cp_async_arrive_noinc(full + stage()); ++it; }
+  __device__ __forceinline__ int acquire() { const int s = stage(); mbar_wait(empty + s, ph ^ 1u); return s; }
+  __device__ __forceinline__ void commit() { cp_async_arrive_noinc(full + stage()); advance(); }
   // consumer side
-  __device__ __forceinline__ int wait() { const int s = stage(); mbar_wait(full + s, round() & 1u); return s; }
-  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) mbar_arrive(empty + stage()); ++it; }
+  __device__ __forceinline__ int wait() { const int s = stage(); mbar_wait(full + s, ph); return s; }
+  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) mbar_arrive(empty + stage()); advance(); }
 };
 
 // producer-warpgroup versions of the job issue functions (128 threads: threadIdx.x - 32*NCONS)

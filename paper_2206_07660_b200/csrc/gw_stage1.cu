@@ -54,13 +54,14 @@ struct Params {
 // ring bookkeeping (same job sequence on the producer and the consumer side)
 struct Ring {
   uint64_t *full, *empty;
-  int nstage; unsigned it;
-  __device__ __forceinline__ int stage() const { return (int)(it % (unsigned)nstage); }
-  __device__ __forceinline__ unsigned round() const { return it / (unsigned)nstage; }
-  __device__ __forceinline__ int acquire() { const int s = stage(); gwp::mbar_wait(empty + s, (round() & 1u) ^ 1u); return s; }
-  __device__ __forceinline__ void commit() { gwp::cp_async_arrive_noinc(full + stage()); ++it; }
-  __device__ __forceinline__ int wait() { const int s = stage(); gwp::mbar_wait(full + s, round() & 1u); return s; }
-  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); ++it; }
+  int nstage; unsigned it;     // `it` = stage index, `ph` = parity of the current round (no integer division per job)
+  unsigned ph;
+  __device__ __forceinline__ int stage() const { return (int)it; }
+  __device__ __forceinline__ void advance() { if (++it == (unsigned)nstage) { it = 0; ph ^= 1u; } }
+  __device__ __forceinline__ int acquire() { const int s = stage(); gwp::mbar_wait(empty + s, ph ^ 1u); return s; }
+  __device__ __forceinline__ void commit() { gwp::cp_async_arrive_noinc(full + stage()); advance(); }
+  __device__ __forceinline__ int wait() { const int s = stage(); gwp::mbar_wait(full + s, ph); return s; }
+  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); advance(); }
 };
 
 // main job: A = Z[TM rows][k0..k0+8), B = Vb[brows rows][k0..k0+8); 16-byte units swizzled by row parity.
@@ -198,7 +199,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     gwp::reg_dec<REG_PROD>();
     if (w < 15) {
       // ---- main-ring producer (96 threads): Z of the current k and the raw V[k+q][k] rows of this CTA's columns ----
-      Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0;
+      Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
       unsigned kit = 0;
       const int brows = 8 * ntc_mine;
       for (int item = cid; item < P.nitems; item += ncl) {
@@ -220,7 +221,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       asm volatile("cp.async.wait_all;\n" ::: "memory");
     } else {
       // ---- pass-ring producer (32 threads): G matrices, V[k][k+q] rows (pass 1), Xt rows from the slab (pass 2) ----
-      Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0;
+      Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
       unsigned kit = 0, ph = 0;
       for (int item = cid; item < P.nitems; item += ncl) {
         const Item it = decode_item(d, item);
@@ -262,7 +263,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     if constexpr (REG_PASS > 65536 / NTHR1) gwp::reg_inc<REG_PASS>(); else gwp::reg_dec<REG_PASS>();
     const int wp = w - NMAINW;
     constexpr int PMT = 1;                             // m-tiles per pass warp (prows = 32*PMT); 2 measured slower (fewer main registers)
-    Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0;
+    Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
     unsigned kit = 0, ph = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
       const Item it = decode_item(d, item);
@@ -308,7 +309,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     const int noff = ((w & 3) - mh + 4) & 3;             // first n-tile; n-tiles noff + 4*jn
     const int njm = (ntc_mine > noff) ? (ntc_mine - noff + 3) / 4 : 0;
     const int sw = (g & 1) << 2;
-    Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0;
+    Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned kit = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
       const Item it = decode_item(d, item);

@@ -302,10 +302,6 @@ static Plan make_plan(const gw_problem *p) {
 
 }  // namespace s3
 
-size_t gw_stage3_workspace(const gw_problem *p) {
-  s3::Plan pl = s3::make_plan(p);
-  return pl.ok ? pl.work_bytes : 0;
-}
 
 double gw_stage3_flops(const gw_problem *p) {
   s3::Plan pl = s3::make_plan(p);
@@ -332,8 +328,9 @@ static int launch_sigma(const s3::Plan &pl, const s3::Params &P, cudaStream_t st
   return (int)cudaGetLastError();
 }
 
-int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
-  s3::Plan pl = s3::make_plan(p);
+namespace s3 {
+static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
+  Plan pl = make_plan(p);
   if (!pl.ok) return GW_ESHAPE;
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   s3::Params P;
@@ -351,4 +348,403 @@ int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *S
     if (pl.ksp_max == 13) return launch_sigma<13, 8>(pl, P, st);
     return launch_sigma<16, 8>(pl, P, st);
   }
+}
+}  // namespace s3
+
+// =====================================================================================================================
+// s3w — warp-specialised variant of the stage-3 kernel for the nao = 25..28 class (ksp = 7, 4 x 4 tiles over nao).
+// Same algebra as s3::sigma_kernel; the work of one (q, Q-panel) unit is split between warp roles that run concurrently:
+//   main warps 0-7  : U = W·V2 (N chunk by N chunk, accumulators in registers), U^T stored to slabU[unit & 1]
+//   aux warps 8-11  : for the PREVIOUS unit: pass A (T = G·U, slabU -> slabT) and the final contraction
+//                     Sigma += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; the nao x nao Sigma accumulator of the item lives in
+//                     their registers (warp w owns column tile w of all four row tiles)
+//   producer warps  : 12-14 feed the main ring (W panel + V2 chunk), 15 feeds the aux ring (G, slabU rows, V1 + slabT)
+// so the DMMA pipe never drains at a phase change and the small-K phases run beside the big GEMM.
+// =====================================================================================================================
+namespace s3w {
+
+using gwp::FastDiv;
+constexpr int NMAINW = 8, NAUXW = 4, NTHR = 512;
+constexpr int T_MPROD = 384, N_MPROD = 96, T_APROD = 480, N_APROD = 32;
+constexpr int KC = 8, MT_W = 2, NJ = 7, TM = 32, KSP = 7, NDT = 4, AROWS = 32;
+constexpr int NST_MAX = 8, AST_MAX = 4;
+constexpr int REG_MAIN = 176, REG_AUX = 120, REG_PROD = 40;
+
+struct Params {
+  GwDims d;
+  const c128 *V, *G, *Wt;
+  c128 *Sigma, *scratch;
+  int nqt, nitems;
+  int ldp, ldt;           // row strides: pass / G / V1 tiles (K contiguous), T tiles (K major)
+  int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
+  int ldb;                // row stride of the main-job B part
+  int main_units, aux_units, nstage, astage;
+  size_t slab_units;      // complex elements per slab (three slabs per CTA: U0, U1, T)
+  FastDiv fd_nao;
+};
+
+struct Ring {
+  uint64_t *full, *empty;
+  int nstage; unsigned it;     // `it` = stage index, `ph` = parity of the current round (no integer division per job)
+  unsigned ph;
+  __device__ __forceinline__ int stage() const { return (int)it; }
+  __device__ __forceinline__ void advance() { if (++it == (unsigned)nstage) { it = 0; ph ^= 1u; } }
+  __device__ __forceinline__ int acquire() { const int s = stage(); gwp::mbar_wait(empty + s, ph ^ 1u); return s; }
+  __device__ __forceinline__ void commit() { gwp::cp_async_arrive_noinc(full + stage()); advance(); }
+  __device__ __forceinline__ int wait() { const int s = stage(); gwp::mbar_wait(full + s, ph); return s; }
+  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); advance(); }
+};
+
+__device__ __forceinline__ void cpa(unsigned dst, const void *src, int nbytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(nbytes));
+}
+
+// main job: A = W[TM rows][k0..k0+8) swizzled by row parity (rows beyond tm_rows re-read the last valid row);
+// B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb] (K rows beyond naux and columns beyond nao² zero filled)
+__device__ __forceinline__ void issue_main(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
+                                           int n0, int ncols, int ldb, int k0) {
+  const int pt = threadIdx.x - T_MPROD;
+  const unsigned sA = gwp::smem_u32(stage);
+  {
+    const int u = pt & 7, rsub = pt >> 3;
+    const bool kok = k0 + u < naux;
+    const int nb = kok ? 16 : 0;
+    const c128 *src = W + (kok ? k0 + u : 0);
+#pragma unroll
+    for (int r = rsub; r < TM; r += N_MPROD / 8) {
+      const int rr = min(r, tm_rows - 1);
+      cpa((sA + 16u * (unsigned)(r * KC + u)) ^ ((unsigned)(r & 1) << 6), src + (size_t)rr * naux, nb);
+    }
+  }
+  const unsigned sB = sA + 16u * TM * KC;
+  for (int cc = pt; cc < ncols; cc += N_MPROD) {
+    const bool cok = n0 + cc < n2;
+    const c128 *src = V2 + (size_t)k0 * n2 + (cok ? n0 + cc : 0);
+    const unsigned dst = sB + 16u * (unsigned)cc;
+#pragma unroll
+    for (int r = 0; r < KC; r++) {
+      const bool ok = cok && (k0 + r < naux);
+      cpa(dst + 16u * (unsigned)(r * ldb), ok ? src + (size_t)r * n2 : V2, ok ? 16 : 0);
+    }
+  }
+}
+
+template <int NJM>
+__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, int ldb, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
+#pragma unroll
+  for (int ks = 0; ks < KC / 4; ks++) {
+    const int u = (4 * ks + c) ^ sw;
+    c128 a[MT_W], b[NJM];
+#pragma unroll
+    for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
+    const c128 *brow = sBw + (4 * ks + c) * ldb;
+#pragma unroll
+    for (int jn = 0; jn < NJM; jn++) b[jn] = brow[32 * jn];
+#pragma unroll
+    for (int jn = 0; jn < NJM; jn++)
+#pragma unroll
+      for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
+  }
+}
+
+// aux ring jobs (producer warp 15)
+__device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd) {
+  const int nrow = min(AROWS, rows_total - row0);
+  const int total = nrow * nao;
+  const c128 *s = src + (size_t)row0 * nao;
+  for (int i = threadIdx.x - T_APROD; i < total; i += N_APROD) {
+    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
+    cp_async16(stage + r * ldp + a, s + i);
+  }
+}
+// final job for one Q: A = V1[Q] (nao x nao, [i][a]) -> stage[i][ldp]; B = T[Q] ([a][j]) -> [a][ldt], K rows a >= nao zero filled
+__device__ __forceinline__ void issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, FastDiv fd) {
+  const int n2 = nao * nao, lane = threadIdx.x - T_APROD;
+  for (int i = lane; i < n2; i += N_APROD) {
+    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
+    cp_async16(stage + r * ldp + a, Aq + i);
+  }
+  c128 *sB = stage + 8 * NDT * ldp;
+  for (int i = lane; i < 4 * KSP * nao; i += N_APROD) {
+    const int r = (int)fd.div((unsigned)i);
+    const bool ok = r < nao;
+    gwp::cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + i : Bq, ok);
+  }
+}
+__device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao, int ldp, FastDiv fd) {
+  for (int i = threadIdx.x - T_APROD; i < nao * nao; i += N_APROD) {
+    const int r = (int)fd.div((unsigned)i), cc = i - r * nao;
+    cp_async16(sG + r * ldp + cc, src + i);
+  }
+}
+
+// aux warps: Sigma tiles (mi, nj = w), mi = 0..3:  acc[mi] += A[mi rows][K] · B[K][8 w ..]; one B fragment per k-step
+__device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[NDT][2], double (&sgi)[NDT][2], int ldp, int ldt, int w) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
+  const c128 *ap = stage + g * ldp + c;
+  const c128 *bp = stage + 8 * NDT * ldp + c * ldt + 8 * w + g;
+#pragma unroll
+  for (int ks = 0; ks < KSP; ks++) {
+    const c128 b = bp[4 * ks * ldt];
+    c128 a[NDT];
+#pragma unroll
+    for (int mi = 0; mi < NDT; mi++) a[mi] = ap[8 * mi * ldp + 4 * ks];
+#pragma unroll
+    for (int mi = 0; mi < NDT; mi++) cmma(sgr[mi], sgi[mi], a[mi], b);
+  }
+}
+
+__global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  c128 *smem = reinterpret_cast<c128 *>(smem_raw);
+  const GwDims d = P.d;
+  const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, ldt = P.ldt;
+  c128 *sG = smem;                                   // [32][ldp]: sG[a][b] = G[t][k-q][a][b]
+  c128 *sAux = sG + 8 * NDT * ldp;                   // astage x aux_units
+  c128 *sMain = sAux + P.astage * P.aux_units;       // nstage x main_units
+  __shared__ uint64_t bars[2 * NST_MAX + 2 * AST_MAX + 6];
+  uint64_t *full_m = bars, *empty_m = bars + NST_MAX, *full_a = bars + 2 * NST_MAX, *empty_a = full_a + AST_MAX;
+  uint64_t *bar_g = empty_a + AST_MAX, *bar_phase = bar_g + 1, *uready = bar_g + 2, *ufree = bar_g + 4;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  c128 *slabU = P.scratch + (size_t)blockIdx.x * 3 * P.slab_units;
+  c128 *slabT = slabU + 2 * P.slab_units;
+  const size_t vb = (size_t)naux * n2;
+  const int nmain = (naux + KC - 1) / KC;
+  {
+    const int tot = 8 * NDT * ldp + P.astage * P.aux_units + P.nstage * P.main_units;
+    for (int i = threadIdx.x; i < tot; i += NTHR) smem[i] = make_double2(0.0, 0.0);
+    if (threadIdx.x == 0) {
+      for (int i = 0; i < P.nstage; i++) { gwp::mbar_init(full_m + i, N_MPROD); gwp::mbar_init(empty_m + i, NMAINW); }
+      for (int i = 0; i < P.astage; i++) { gwp::mbar_init(full_a + i, N_APROD); gwp::mbar_init(empty_a + i, NAUXW); }
+      gwp::mbar_init(bar_g, N_APROD);
+      gwp::mbar_init(bar_phase, NAUXW);
+      for (int i = 0; i < 2; i++) { gwp::mbar_init(uready + i, NMAINW); gwp::mbar_init(ufree + i, NAUXW); }
+    }
+  }
+  __syncthreads();
+
+  if (w >= NMAINW + NAUXW) {
+    gwp::reg_dec<REG_PROD>();
+    if (w < 15) {
+      // ---- main-ring producer: W panel rows and V2 chunk rows ----
+      Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
+      for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+        const int t = item % d.ntau, k = item / d.ntau;
+        for (int ql = 0; ql < d.nq; ql++) {
+          const int kp = gw_ksub(d, k, d.q0 + ql);
+          const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
+          const c128 *Wq = P.Wt + ((size_t)t * d.nq + ql) * naux * naux;
+          for (int qt = 0; qt < P.nqt; qt++) {
+            const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0);
+            const c128 *W = Wq + (size_t)Q0 * naux;
+            for (int ch = 0; ch < P.nchunk; ch++) {
+              const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
+              for (int j = 0; j < nmain; j++) {
+                const int s = rm.acquire();
+                issue_main(sMain + s * P.main_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC);
+                rm.commit();
+              }
+            }
+          }
+        }
+      }
+      asm volatile("cp.async.wait_all;\n" ::: "memory");
+    } else {
+      // ---- aux-ring producer: G per q, U^T rows of the finished unit (pass A), then V1[Q] + T[Q] per Q (final) ----
+      Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
+      unsigned un = 0;
+      for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+        const int t = item % d.ntau, k = item / d.ntau;
+        for (int ql = 0; ql < d.nq; ql++) {
+          const int kp = gw_ksub(d, k, d.q0 + ql);
+          const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
+          for (int qt = 0; qt < P.nqt; qt++, un++) {
+            const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + AROWS - 1) / AROWS;
+            const c128 *U = slabU + (size_t)(un & 1u) * P.slab_units;
+            // sG is free: pass A of the previous unit completed before its final jobs were issued
+            if (qt == 0) issue_matrix(sG, P.G + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
+            gwp::cp_async_arrive_noinc(bar_g);
+            gwp::mbar_wait(uready + (un & 1u), (un >> 1) & 1u);
+            for (int j = 0; j < npass; j++) {
+              const int s = ra.acquire();
+              issue_rows(sAux + s * P.aux_units, U, j * AROWS, rows, nao, ldp, P.fd_nao);
+              ra.commit();
+            }
+            gwp::mbar_wait(bar_phase, un & 1u);                     // T of this unit is in slabT
+            const c128 *V1t = V1 + (size_t)Q0 * n2;
+            for (int j = 0; j < tm_rows; j++) {
+              const int s = ra.acquire();
+              issue_final(sAux + s * P.aux_units, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldp, ldt, P.fd_nao);
+              ra.commit();
+            }
+          }
+        }
+      }
+      asm volatile("cp.async.wait_all;\n" ::: "memory");
+    }
+  } else if (w >= NMAINW) {
+    // ============================================ aux warps ============================================
+    gwp::reg_dec<REG_AUX>();
+    const int wa = w - NMAINW, g = lane >> 2, c = lane & 3;
+    Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
+    unsigned un = 0;
+    for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+      const int t = item % d.ntau, k = item / d.ntau;
+      double sgr[NDT][2], sgi[NDT][2];
+#pragma unroll
+      for (int i = 0; i < NDT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+      for (int ql = 0; ql < d.nq; ql++) {
+        for (int qt = 0; qt < P.nqt; qt++, un++) {
+          const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + AROWS - 1) / AROWS;
+          gwp::mbar_wait(bar_g, un & 1u);
+          for (int j = 0; j < npass; j++) {
+            const int s = ra.wait();
+            gwp::pass_compute_exact_mt<KSP, true, 1>(sAux + s * P.aux_units, sG, slabT, j * AROWS, rows, nao, ldp, wa, P.fd_nao);
+            ra.release();
+          }
+          __threadfence(); __syncwarp();
+          if (lane == 0) { gwp::mbar_arrive(bar_phase); gwp::mbar_arrive(ufree + (un & 1u)); }
+          for (int j = 0; j < tm_rows; j++) {
+            const int s = ra.wait();
+            final_compute(sAux + s * P.aux_units, sgr, sgi, ldp, ldt, wa);
+            ra.release();
+          }
+        }
+      }
+      // Sigma[t][k] = -(1/N_k) acc: this warp's column tile of the four row tiles
+      const double pref = -1.0 / (double)d.nk;
+      c128 *out = P.Sigma + ((size_t)t * d.nk + k) * n2;
+      const int j0 = 8 * wa + 2 * c;
+#pragma unroll
+      for (int mi = 0; mi < NDT; mi++) {
+        const int i = 8 * mi + g;
+        if (i < nao) {
+          if (j0 < nao) out[i * nao + j0] = make_double2(pref * sgr[mi][0], pref * sgi[mi][0]);
+          if (j0 + 1 < nao) out[i * nao + j0 + 1] = make_double2(pref * sgr[mi][1], pref * sgi[mi][1]);
+        }
+      }
+    }
+  } else {
+    // ============================================ main warps ============================================
+    gwp::reg_inc<REG_MAIN>();
+    const int g = lane >> 2, c = lane & 3;
+    const int mh = w >> 2, sw = (g & 1) << 2, noff = ((w & 3) - mh + 4) & 3;
+    Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
+    unsigned un = 0;
+    for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+      for (int ql = 0; ql < d.nq; ql++) {
+        for (int qt = 0; qt < P.nqt; qt++, un++) {
+          const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
+          c128 *U = slabU + (size_t)(un & 1u) * P.slab_units;
+          for (int ch = 0; ch < P.nchunk; ch++) {
+            const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0), n0 = nt0 * 8;
+            const int njm = (ntc > noff) ? (ntc - noff + 3) / 4 : 0;
+            const bool active = (mh * MT_W < mtc) && njm > 0;
+            double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
+#pragma unroll
+            for (int i = 0; i < MT_W; i++)
+#pragma unroll
+              for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
+            for (int jb = 0; jb < nmain; jb++) {
+              const int s = rm.wait();
+              if (active) {
+                const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + g) * KC;
+                const c128 *sBw = sMain + s * P.main_units + TM * KC + 8 * noff + g;
+                if (njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 4) main_compute<4>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 3) main_compute<3>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 2) main_compute<2>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else main_compute<1>(sAw, sBw, P.ldb, accr, acci, c, sw);
+              }
+              rm.release();
+            }
+            // slabU[un & 1] was read by pass A of unit un-2
+            if (ch == 0 && un >= 2) gwp::mbar_wait(ufree + (un & 1u), ((un >> 1) - 1u) & 1u);
+            // store U^T: element (Q, n=(b,j)) -> U[(Q*nao + j)*nao + b]
+#pragma unroll
+            for (int i = 0; i < MT_W; i++) {
+              const int Ql = 8 * (mh * MT_W + i) + g;
+#pragma unroll
+              for (int jn = 0; jn < NJ; jn++) {
+                if (jn < njm && Ql < tm_rows) {
+#pragma unroll
+                  for (int e = 0; e < 2; e++) {
+                    const int n = n0 + 8 * (noff + 4 * jn) + 2 * c + e;
+                    if (n < n2) {
+                      const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
+                      U[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
+                    }
+                  }
+                }
+              }
+            }
+          }
+          __threadfence(); __syncwarp();
+          if (lane == 0) gwp::mbar_arrive(uready + (un & 1u));
+        }
+      }
+    }
+  }
+}
+
+struct Plan { int nqt, nitems, ldp, ldt, nnt, nchunk, cht, ldb, main_units, aux_units, nstage, astage, grid; size_t smem, slab_units, work_bytes; bool ok; };
+
+static Plan make_plan(const gw_problem *p) {
+  Plan pl; memset(&pl, 0, sizeof(pl));
+  GwDims d = gw_dims(p);
+  if ((d.nao + 3) / 4 != KSP) { pl.ok = false; return pl; }
+  pl.ldp = 4 * KSP;                         // 28 ≡ 4 (mod 8)
+  pl.ldt = 8 * NDT + 2;
+  pl.nnt = (d.nao * d.nao + 7) / 8;
+  pl.nchunk = (pl.nnt + 4 * NJ - 1) / (4 * NJ);
+  pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
+  pl.ldb = pl.cht * 8 + 2;
+  pl.nqt = (d.naux + TM - 1) / TM;
+  pl.nitems = d.ntau * d.nk;
+  pl.main_units = TM * KC + KC * pl.ldb;
+  const int s_pass = AROWS * pl.ldp, s_fin = 8 * NDT * pl.ldp + 4 * KSP * pl.ldt + 8;
+  pl.aux_units = s_pass > s_fin ? s_pass : s_fin;
+  pl.astage = 3;
+  const size_t cap = 226 * 1024, fixed = ((size_t)8 * NDT * pl.ldp + (size_t)pl.astage * pl.aux_units) * sizeof(c128);
+  pl.nstage = (int)((cap - fixed) / ((size_t)pl.main_units * sizeof(c128)));
+  if (pl.nstage > 6) pl.nstage = 6;
+  pl.smem = fixed + (size_t)pl.nstage * pl.main_units * sizeof(c128);
+  const int nsm = gwp::gw_num_sms();
+  pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
+  pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
+  pl.work_bytes = 256 + (size_t)nsm * 3 * pl.slab_units * sizeof(c128);
+  pl.ok = pl.nstage >= 3;
+  return pl;
+}
+
+static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
+  Plan pl = make_plan(p);
+  if (!pl.ok) return GW_ESHAPE;
+  if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
+  Params P;
+  P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
+  P.scratch = (c128 *)((char *)p->work + 256);
+  P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ldt = pl.ldt; P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb;
+  P.main_units = pl.main_units; P.aux_units = pl.aux_units; P.nstage = pl.nstage; P.astage = pl.astage; P.slab_units = pl.slab_units;
+  P.fd_nao = FastDiv((unsigned)P.d.nao);
+  cudaError_t e = cudaFuncSetAttribute(sigma_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  if (e != cudaSuccess) return (int)e;
+  sigma_ws_kernel<<<pl.grid, NTHR, pl.smem, st>>>(P);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace s3w
+
+size_t gw_stage3_workspace(const gw_problem *p) {
+  s3w::Plan pw = s3w::make_plan(p);
+  if (pw.ok) return pw.work_bytes;
+  s3::Plan pl = s3::make_plan(p);
+  return pl.ok ? pl.work_bytes : 0;
+}
+
+int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
+  if (s3w::make_plan(p).ok) return s3w::launch(p, G, Wt, Sigma, st);
+  return s3::launch(p, G, Wt, Sigma, st);
 }
