@@ -168,6 +168,7 @@ class ClockSampler:
 
 
 # dram traffic per launch of the dominant kernel from the committed ncu capture (profiles/), keyed by config; None = not captured
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu captures summarised in profiles/ (key: config, stage)
 NCU_TRAFFIC_BYTES = {}
 
 
@@ -277,18 +278,28 @@ def run_ours(args):
 
     if rank != 0:
         return 0
-    # ---- roofline of the dominant kernel (stage 3's sigma_kernel or stage 1's p0_kernel, whichever is longer) ----
+    # ---- roofline of the dominant kernel (stage 3's sigma kernel or stage 1's p0_kernel, whichever takes longer) ----
+    # achieved = ALGORITHMIC flops of the launch (8*(naux²nao² + 2 naux nao³) per (k,q,tau) unit x units)
+    # / the CUDA-event duration of that launch on the launching stream; peak = FP64 DMMA peak measured in this run.
+    names = {0: "s1::p0_kernel (stage 1, Eq. 28b)",
+             2: ("s3w::sigma_ws_kernel" if (cfg.nao + 3) // 4 == 7 else "s3::sigma_kernel") + " (stage 3, Eq. 31)"}
+    per_kernel = {}
+    for st in (0, 2):
+        alg = (nom["stage3"] if st == 2 else nom["stage1"]) * nq / cfg.nk
+        ach = alg / (stage_ms[st] * 1e-3) * 1e-12
+        per_kernel[names[st]] = {"ms": stage_ms[st], "achieved": ach, "frac": ach / peak,
+                                 "achieved_executed": executed[st] / (stage_ms[st] * 1e-3) * 1e-12,
+                                 "executed_over_algorithmic": executed[st] / alg,
+                                 "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, st))}
     dom = 2 if stage_ms[2] >= stage_ms[0] else 0
-    dom_name = {0: "s1::p0_kernel (stage 1, Eq. 28b)", 2: "s3::sigma_kernel (stage 3, Eq. 31)"}[dom]
-    alg_flops = (nom["stage3"] if dom == 2 else nom["stage1"]) * nq / cfg.nk
-    achieved = alg_flops / (stage_ms[dom] * 1e-3) * 1e-12
-    roof = {"bound": "tensor", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-            "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+    dk = per_kernel[names[dom]]
+    roof = {"bound": "tensor", "kernel": names[dom], "achieved": dk["achieved"], "peak": peak, "unit": "TFLOP/s",
+            "frac": dk["frac"], "traffic": dk["traffic"],
             "peak_source": "measured in this run: register-resident DMMA.8x8x4 loop on all SMs (gw_fp64_peak); "
                            "MEASURED_PEAKS.json has no FP64 entry",
             "flops": "algorithmic (Algorithm 1 literal, 8 flops per complex multiply-add); executed/algorithmic = %.3f"
-                     % (executed[dom] / alg_flops),
-            "achieved_executed": executed[dom] / (stage_ms[dom] * 1e-3) * 1e-12}
+                     % dk["executed_over_algorithmic"],
+            "achieved_executed": dk["achieved_executed"], "kernels": per_kernel}
     total_nom = nom["total"]
     out = {"metric": "sigma_build_seconds_per_iteration", "value": ms_per_step * 1e-3, "unit": "s", "n_gpus": world,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,

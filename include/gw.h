@@ -77,6 +77,14 @@ int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P0t, void *s
  *   info: device int32[2] or NULL.  Set to {-1,-1} on success, else {q, n} of one failing factorisation. */
 int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, void *stream);
 
+/* Stage 2 plus the integrand of the dynamical part of the GW Luttinger-Ward functional, Eq. 37:
+ *   phi[n][q-q_begin] = tr{ ln[I − P0w[n][q]] + P0w[n][q] }      (real; ln det from the Cholesky diagonal of stage 2b)
+ * so that  Φ̃_GW = (1/2N_k) Σ_q (1/β) Σ_n phi[n][q]; the Matsubara sum over the sparse grid needs the caller's
+ * quadrature weights (the paper gives none), so the summand is returned, not the sum.
+ *   phi : device double [nw][nq]   out (8-byte aligned, required).  Other arguments and errors as above;
+ *   an entry whose factorisation failed (see info) is unspecified. */
+int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, double *phi, void *stream);
+
 /* Stage 3 — Eq. 31, Algorithm 1 second k loop:
  *   Sigma[t][k][i][j] = -(1/N_k) Σ_{q in shard} Σ_QQ' Σ_ab V[k][k-q][Q][i][a] G[t][k-q][a][b] Wt[t][q-q_begin][Q][Q'] V[k-q][k][Q'][b][j]
  *   G     : device [ntau][nk][nao][nao]    in

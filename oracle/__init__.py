@@ -113,6 +113,15 @@ def dyson(P):
     return X
 
 
+def phi(P):
+    """Summand of Eq. 37 for one matrix: tr{ln[I - P] + P}."""
+    n = P.shape[0]
+    out = ctypes.c_double(0.0)
+    if lib().gwref_phi(n, _p(np.ascontiguousarray(P, dtype=np.complex128)), ctypes.byref(out)):
+        raise RuntimeError("oracle: zero pivot")
+    return out.value
+
+
 def screened_interaction_q(cfg, T_wt, T_tw, P0t_q, want_freq=False):
     """Stage 2 for one q.  P0t_q: packed [ntau][naux][naux]."""
     ps = cfg.naux * cfg.naux

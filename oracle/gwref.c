@@ -15,6 +15,7 @@
  *           Eq. 30                                       -> gwref_transform
  *           for k { read V(k,k-q); for tau: Eq. 31 } }   -> gwref_sigma_slice
  *   Eq. 22 (static exchange)                             -> gwref_exchange_slice
+ *   Eq. 37 summand tr{ln[I - P0(iOmega)] + P0(iOmega)}   -> gwref_phi
  *
  * No blocking, fusion or reordering beyond the temporaries A, B, X, Y named in
  * SURVEY.md §8(c); the linear solve is Gaussian elimination with partial pivoting
@@ -37,7 +38,8 @@
  *
  * Parity pins: tests/test_oracle_pins.py (closed form P1, Lindhard P2, invariants P3-P5,
  * brute-force Matsubara sum P6, trace identity P7, solve residual P8, exchange limit P9,
- * literal 4-index evaluation P10).  Nothing here is "parity unpinned".
+ * literal 4-index evaluation P10, scalar form / series / eigenvalue route of the Eq. 37 summand P11).
+ * Nothing here is "parity unpinned".
  */
 #include <complex.h>
 #include <math.h>
@@ -181,6 +183,40 @@ int gwref_dyson(int n, const c128 *P, c128 *X) {
       }
     }
   free(M);
+  return fail;
+}
+
+/* ---- Summand of Eq. 37: phi = tr{ ln[I - P] + P } for one matrix.
+ * tr ln M = ln det M, and det M is the product of the pivots of Gaussian elimination with partial pivoting (times the
+ * sign of the row permutation).  I - P0(iOmega) is Hermitian positive definite under reading R7, so det M > 0 and
+ * ln det M = Σ_c ln|u_cc|; the imaginary part of tr P (zero for Hermitian P) is dropped.  Returns 1 on a zero pivot. */
+int gwref_phi(int n, const c128 *P, double *phi) {
+  c128 *M = (c128 *)malloc(sizeof(c128) * n * n);
+  double tr = 0.0, lndet = 0.0;
+  for (int i = 0; i < n; i++) {
+    tr += creal(P[(size_t)i * n + i]);
+    for (int j = 0; j < n; j++) M[(size_t)i * n + j] = (i == j ? 1.0 : 0.0) - P[(size_t)i * n + j];
+  }
+  int fail = 0;
+  for (int c = 0; c < n; c++) {
+    int p = c;
+    double best = cabs(M[(size_t)c * n + c]);
+    for (int r = c + 1; r < n; r++) {
+      double v = cabs(M[(size_t)r * n + c]);
+      if (v > best) { best = v; p = r; }
+    }
+    if (best == 0.0) { fail = 1; break; }
+    if (p != c)
+      for (int j = 0; j < n; j++) { c128 tmp = M[(size_t)c * n + j]; M[(size_t)c * n + j] = M[(size_t)p * n + j]; M[(size_t)p * n + j] = tmp; }
+    lndet += log(best);
+    for (int r = c + 1; r < n; r++) {
+      c128 f = M[(size_t)r * n + c] / M[(size_t)c * n + c];
+      if (f == 0) continue;
+      for (int j = c; j < n; j++) M[(size_t)r * n + j] -= f * M[(size_t)c * n + j];
+    }
+  }
+  free(M);
+  *phi = lndet + tr;
   return fail;
 }
 

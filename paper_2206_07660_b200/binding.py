@@ -38,6 +38,7 @@ def lib():
         vp, sz = ctypes.c_void_p, ctypes.c_size_t
         L.gw_polarization.argtypes = [P, vp, vp, vp]
         L.gw_screened_interaction.argtypes = [P, vp, vp, vp, vp]
+        L.gw_screened_interaction_phi.argtypes = [P, vp, vp, vp, vp, vp]
         L.gw_selfenergy.argtypes = [P, vp, vp, vp, vp]
         L.gw_exchange.argtypes = [P, vp, vp, vp]
         L.gw_workspace_bytes.argtypes = [P]
@@ -48,7 +49,7 @@ def lib():
         L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
-        for n in ("gw_polarization", "gw_screened_interaction", "gw_selfenergy", "gw_exchange",
+        for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_version"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
@@ -149,6 +150,23 @@ def gw_screened_interaction(prob, P0t, Wt=None, info=None, stream=None):
     _check(lib().gw_screened_interaction(prob.ref(), _dev(P0t, shape, "P0t"), _dev(Wt, shape, "Wt"),
                                          ctypes.c_void_p(info.data_ptr()), _stream(stream)), "gw_screened_interaction")
     return Wt, info
+
+
+def gw_screened_interaction_phi(prob, P0t, Wt=None, info=None, phi=None, stream=None):
+    """Stage 2 plus phi[n][q] = tr{ln[I - P0w] + P0w}, the summand of Eq. 37."""
+    shape = (prob.ntau, prob.nq, prob.naux, prob.naux)
+    if Wt is None:
+        Wt = torch.empty(shape, dtype=torch.complex128, device=P0t.device)
+    if info is None:
+        info = torch.empty(2, dtype=torch.int32, device=P0t.device)
+    if phi is None:
+        phi = torch.empty((prob.nw, prob.nq), dtype=torch.float64, device=P0t.device)
+    if phi.dtype != torch.float64 or tuple(phi.shape) != (prob.nw, prob.nq) or not phi.is_contiguous():
+        raise GWError("phi must be a contiguous float64 tensor of shape (nw, nq)")
+    _check(lib().gw_screened_interaction_phi(prob.ref(), _dev(P0t, shape, "P0t"), _dev(Wt, shape, "Wt"),
+                                             ctypes.c_void_p(info.data_ptr()), ctypes.c_void_p(phi.data_ptr()),
+                                             _stream(stream)), "gw_screened_interaction_phi")
+    return Wt, info, phi
 
 
 def gw_selfenergy(prob, G, Wt, Sigma=None, stream=None):

@@ -56,7 +56,15 @@ extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, 
   if (!p->work || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  return gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, st);
+  return gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, NULL, st);
+}
+
+extern "C" int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, double *phi, void *stream) {
+  int rc = check_problem(p, true); if (rc) return rc;
+  if (!aligned16(P0t) || !aligned16(Wt) || !phi || (((uintptr_t)phi) & 7)) return GW_EINVAL;
+  if (!p->work || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
+  if ((rc = check_arch())) return rc;
+  return gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, phi, (cudaStream_t)stream);
 }
 
 extern "C" int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c128 *Sigma, void *stream) {

@@ -84,6 +84,7 @@ struct DysonParams {
   c128 *PW;                // batch matrices, n*n each (index = freq*nq + ql); overwritten by the solution
   c128 *slabs;             // per-CTA copy for A / L
   int32_t *info;
+  double *phi;        // optional [batch]: tr{ln[I - P0w] + P0w} (summand of Eq. 37), or NULL
 };
 
 // C[r][col] -= Σ_k Aop(r,k) * Bop(k,col) over a tile range; operands in shared memory.
@@ -147,15 +148,18 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
   c128 *sBlk = smem + pan_units;              // [nb][ldn]
   __shared__ int s_bad;
   __shared__ double s_piv;
+  __shared__ double s_red[NTHR];
   c128 *A = P.slabs + (size_t)blockIdx.x * n * n;
   const int kst = (nb + 3) / 4;
 
   for (int mi = blockIdx.x; mi < P.batch; mi += gridDim.x) {
     c128 *Pm = P.PW + (size_t)mi * n * n;
     if (threadIdx.x == 0) s_bad = 0;
+    double trp = 0.0;                                  // this thread's share of Re tr P0w (fixed order: deterministic)
     for (int e = threadIdx.x; e < n * n; e += NTHR) {
       const int i = e / n, j = e - i * n;
       const c128 v = Pm[e];
+      if (i == j) trp += v.x;
       A[e] = make_double2((i == j ? 1.0 : 0.0) - v.x, -v.y);
     }
     __syncthreads();
@@ -210,6 +214,18 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
       if (m > jb)
         update_tiles<false, true, true>(A + (size_t)(j0 + jb) * n + j0 + jb, n, m - jb, m - jb, sPan + jb * ldpan, ldpan, sPan + jb * ldpan, ldpan, kst);
       __syncthreads();
+    }
+    if (P.phi) {
+      // Eq. 37 summand: tr ln[I - P0w] + tr P0w = 2 Σ_i ln L_ii + tr P0w  (tree reduction in a fixed order)
+      double v = trp;
+      for (int i = threadIdx.x; i < n; i += NTHR) v += 2.0 * log(A[(size_t)i * n + i].x);
+      s_red[threadIdx.x] = v;
+      __syncthreads();
+      for (int h = NTHR / 2; h > 0; h >>= 1) {
+        if (threadIdx.x < h) s_red[threadIdx.x] += s_red[threadIdx.x + h];
+        __syncthreads();
+      }
+      if (threadIdx.x == 0) P.phi[mi] = s_red[0];
     }
     // ---------- forward solve L Y = P (in place on Pm) ----------
     for (int j0 = 0; j0 < n; j0 += nb) {
@@ -308,7 +324,7 @@ size_t gw_stage2_workspace(const gw_problem *p) {
   return pl.ok ? pl.work_bytes : 0;
 }
 
-int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *info, cudaStream_t st) {
+int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *info, double *phi, cudaStream_t st) {
   s2::Plan pl = s2::make_plan(p);
   if (!pl.ok) return GW_ESHAPE;
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
@@ -322,7 +338,7 @@ int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *in
   s2::transform_kernel<<<pl.grid_t, s2::NTHR, pl.smem_t, st>>>(d.nw, d.ntau, (const c128 *)p->T_wt, P0t, Wt, len, pl.nblocks);
   s2::DysonParams D;
   D.n = d.naux; D.nb = pl.nb; D.batch = d.nw * d.nq; D.nq = d.nq; D.q0 = d.q0; D.ldpan = pl.ldpan; D.ldn = pl.ldn;
-  D.PW = Wt; D.slabs = (c128 *)((char *)p->work + 256); D.info = info;
+  D.PW = Wt; D.slabs = (c128 *)((char *)p->work + 256); D.info = info; D.phi = phi;
   s2::dyson_kernel<<<pl.grid_d, s2::NTHR, pl.smem_d, st>>>(D);
   s2::transform_kernel<<<pl.grid_t, s2::NTHR, pl.smem_t, st>>>(d.ntau, d.nw, (const c128 *)p->T_tw, Wt, Wt, len, pl.nblocks);
   return (int)cudaGetLastError();

@@ -706,7 +706,7 @@ static Plan make_plan(const gw_problem *p) {
   pl.main_units = TM * KC + KC * pl.ldb;
   const int s_pass = AROWS * pl.ldp, s_fin = 8 * NDT * pl.ldp + 4 * KSP * pl.ldt + 8;
   pl.aux_units = s_pass > s_fin ? s_pass : s_fin;
-  pl.astage = 3;
+  pl.astage = 2;
   const size_t cap = 226 * 1024, fixed = ((size_t)8 * NDT * pl.ldp + (size_t)pl.astage * pl.aux_units) * sizeof(c128);
   pl.nstage = (int)((cap - fixed) / ((size_t)pl.main_units * sizeof(c128)));
   if (pl.nstage > 6) pl.nstage = 6;

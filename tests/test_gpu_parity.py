@@ -108,11 +108,16 @@ def _sampled_parity(name, oracle_lib, n_q=2, n_t=2, n_k=2):
             e.append(relerr(Sigma[t, k].cpu().numpy(), ref))
         e4.append(relerr(K[k].cpu().numpy(), oracle_lib.exchange_slice(cfg, vb, p.gamma, k)))
     errs["Sigma"], errs["K"] = max(e), max(e4)
-    # invariants on the FULL outputs (hold at any size)
-    lhs = torch.einsum("tkij,tkji->t", Sigma, G.flip(0))
-    rhs = torch.einsum("tqab,tqba->t", Wt, P0t.flip(0)) / cfg.spin_deg
+    # invariants on the FULL outputs (hold at any size); evaluated one tau node at a time to bound temporaries
+    N = cfg.ntau
+    tr = lambda A, B: (A * B.transpose(-1, -2)).sum()                         # Σ tr(A_x B_x) over the leading index
+    lhs = torch.stack([tr(Sigma[t], G[N - 1 - t]) for t in range(N)])
+    rhs = torch.stack([tr(Wt[t], P0t[N - 1 - t]) for t in range(N)]) / cfg.spin_deg
     errs["P7_trace"] = float((lhs - rhs).abs().max() / rhs.abs().max())
-    herm = lambda A: float((A - A.transpose(-1, -2).conj()).abs().max() / A.abs().max())
+
+    def herm(A):
+        num = max(float((A[t] - A[t].transpose(-1, -2).conj()).abs().max()) for t in range(A.shape[0]))
+        return num / max(float(A[t].abs().max()) for t in range(A.shape[0]))
     errs["herm_P0t"], errs["herm_Wt"], errs["herm_Sigma"] = herm(P0t), herm(Wt), herm(Sigma)
     neg = torch.from_numpy(p.mesh.neg().astype(np.int64)).cuda()
     errs["TR_Sigma"] = float((Sigma[:, neg] - Sigma.conj()).abs().max() / Sigma.abs().max())
@@ -205,3 +210,22 @@ def test_host_buffer_iteration_matches(problems, oracle_results):
     ref = oracle_results("R")
     for key in ("P0t", "Wt", "Sigma", "K"):
         assert relerr(r[key].numpy(), ref[key]) <= TOL, key
+
+
+@pytest.mark.parametrize("name", ["T", "R", "L"])
+def test_phi_parity(problems, oracle_results, oracle_lib, name):
+    """gw_screened_interaction_phi: phi[n][q] = tr{ln[I - P0w] + P0w} (Eq. 37 summand) against the oracle's LU route,
+    Wt identical to the plain call."""
+    import paper_2206_07660_b200 as gw
+    p = problems(name)
+    ref = oracle_results(name)
+    cfg = p.cfg
+    prob, G, gamma = device_problem(p)
+    P0t = torch.from_numpy(ref["P0t"]).cuda()
+    W0, _ = gw.gw_screened_interaction(prob, P0t)
+    W1, info, phi = gw.gw_screened_interaction_phi(prob, P0t)
+    torch.cuda.synchronize()
+    assert torch.equal(W0, W1) and info.cpu().tolist() == [-1, -1]
+    want = np.array([[oracle_lib.phi(ref["P0w"][n, q]) for q in range(cfg.nk)] for n in range(cfg.nw)])
+    got = phi.cpu().numpy()
+    assert np.max(np.abs(got - want) / np.maximum(1.0, np.abs(want))) <= 1e-10

@@ -295,3 +295,36 @@ def test_P10_literal_einsum(problems, oracle_results, name):
                 lit[t, q] += np.einsum("Qda,cd,ab,Pbc->QP", V[k, kq], p.G[N - 1 - t, k], p.G[t, kq], V[kq, k])
     lit *= -cfg.spin_deg / nk
     assert relerr(r["P0t"], lit) < 1e-13
+
+
+# ---- P11: summand of Eq. 37, phi = tr{ln[I - P] + P} ----
+def test_P11_phi_scalar_and_series(oracle_lib):
+    """Closed form for a 1x1 matrix, and the paper's own expansion (first line of Eq. 37):
+    tr{ln[I-P]+P} = -Σ_{m>=2} tr(P^m)/m, evaluated by explicit matrix powers for a small-norm Hermitian P."""
+    for pval in (-3.7, -0.2, 0.5):
+        got = oracle_lib.phi(np.array([[pval]], dtype=np.complex128))
+        assert abs(got - (np.log(1.0 - pval) + pval)) <= 1e-14 * max(1.0, abs(pval))
+    rng = np.random.default_rng(5)
+    n = 9
+    A = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    P = -(A @ A.conj().T)
+    P *= 0.3 / np.linalg.norm(P, 2)                       # spectral radius 0.3: the series converges fast
+    series, Pm = 0.0, P.copy()
+    for m in range(2, 80):
+        Pm = Pm @ P
+        series -= np.trace(Pm).real / m
+    assert abs(oracle_lib.phi(P) - series) <= 1e-13
+
+
+def test_P11_phi_matches_eigenvalues(problems, oracle_results, oracle_lib):
+    """On real stage-2 data (config T): tr ln[I-P0w] + tr P0w = Σ_i ln(1-λ_i) + λ_i over the eigenvalues of the
+    Hermitian P0w (a different route than the oracle's LU pivots); the (I-P)^2 term of Eq. 36 bounds it from below."""
+    P0w = oracle_results("T")["P0w"]
+    for n in (0, 3, 17):
+        for q in (0, 4):
+            P = P0w[n, q]
+            lam = np.linalg.eigvalsh(0.5 * (P + P.conj().T))
+            ref = float(np.sum(np.log1p(-lam) + lam))
+            got = oracle_lib.phi(P)
+            assert abs(got - ref) <= 1e-12 * max(1.0, abs(ref))
+            assert got <= 1e-14 and got >= -0.5 * np.sum(lam ** 2) - 1e-12     # ln(1-x)+x in [-x²/2, 0] for x <= 0
