@@ -118,18 +118,23 @@ template <int KSP, bool TRANSPOSED, int MT>
 __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
                                                       int nao, int ldp, int w, FastDiv fd) {
   constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 3, NB = PF + 1;
+  constexpr bool CACHE_A = KSP * MT <= 8;   // keep the A fragments of the m-tile(s) in registers, else stream them like B
+  constexpr int NA = CACHE_A ? KSP : NB;
   const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
   const int rbase = row0 + 8 * MT * w;
   if (rbase >= rows_total) return;          // all m-tiles of this warp beyond the panel (warp-uniform)
-  c128 a[MT][KSP];
+  c128 a[MT][NA];
+  const c128 *ap[MT];
   c128 *o[MT];
   bool rok[MT];
   int ostride;
 #pragma unroll
   for (int i = 0; i < MT; i++) {
-    const c128 *ap = sStage + (8 * (MT * w + i) + g) * ldp + c;
+    ap[i] = sStage + (8 * (MT * w + i) + g) * ldp + c;
+    if (CACHE_A) {
 #pragma unroll
-    for (int ks = 0; ks < KSP; ks++) a[i][ks] = ap[4 * ks];
+      for (int ks = 0; ks < KSP; ks++) a[i][ks] = ap[i][4 * ks];
+    }
     const int row = rbase + 8 * i + g;
     rok[i] = row < rows_total;
     if (TRANSPOSED) { const int Q = (int)fd.div((unsigned)row), x = row - Q * nao; o[i] = out + ((size_t)Q * nao + 2 * c) * nao + x; }
@@ -137,27 +142,62 @@ __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const 
   }
   ostride = TRANSPOSED ? nao : 1;
   const c128 *bp = sG + g * ldp + c;
-  c128 b[NB];
-#pragma unroll
-  for (int s = 0; s < PF && s < S; s++) b[s % NB] = bp[(s / KSP) * 8 * ldp + 4 * (s % KSP)];
   double cr[MT][2], ci[MT][2];
+  if (CACHE_A) {
+    // short K: one flat, fully unrolled (n-tile, k-step) sequence with the B fragments PF steps ahead
+    c128 b[NB];
 #pragma unroll
-  for (int i = 0; i < MT; i++) { cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0; }
+    for (int s = 0; s < PF && s < S; s++) b[s % NB] = bp[(s / KSP) * 8 * ldp + 4 * (s % KSP)];
 #pragma unroll
-  for (int s = 0; s < S; s++) {
-    const int nt = s / KSP, ks = s % KSP;
-    if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
+    for (int i = 0; i < MT; i++) { cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0; }
 #pragma unroll
-    for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][ks], b[s % NB]);
-    if (ks == KSP - 1) {
-      // only the last n-tile can reach beyond nao: 8*(NDT-1) <= 4*(KSP-1) < nao
+    for (int s = 0; s < S; s++) {
+      const int nt = s / KSP, ks = s % KSP;
+      if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
+#pragma unroll
+      for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][ks], b[s % NB]);
+      if (ks == KSP - 1) {
+        // only the last n-tile can reach beyond nao: 8*(NDT-1) <= 4*(KSP-1) < nao
+        const bool c0 = nt < NDT - 1 || 8 * nt + 2 * c < nao, c1 = nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao;
+#pragma unroll
+        for (int i = 0; i < MT; i++) {
+          if (rok[i] && c0) o[i][0] = make_double2(cr[i][0], ci[i][0]);
+          if (rok[i] && c1) o[i][ostride] = make_double2(cr[i][1], ci[i][1]);
+          o[i] += 8 * ostride;
+          cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0;
+        }
+      }
+    }
+  } else {
+    // long K: a real loop over the n-tiles (bounded register pressure), A and B fragments streamed PF k-steps ahead
+#pragma unroll 1
+    for (int nt = 0; nt < NDT; nt++) {
+      const c128 *bq = bp + nt * 8 * ldp;
+      c128 b[NB];
+#pragma unroll
+      for (int ks = 0; ks < PF && ks < KSP; ks++) {
+        b[ks % NB] = bq[4 * ks];
+#pragma unroll
+        for (int i = 0; i < MT; i++) a[i][ks % NB] = ap[i][4 * ks];
+      }
+#pragma unroll
+      for (int i = 0; i < MT; i++) { cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0; }
+#pragma unroll
+      for (int ks = 0; ks < KSP; ks++) {
+        if (ks + PF < KSP) {
+          b[(ks + PF) % NB] = bq[4 * (ks + PF)];
+#pragma unroll
+          for (int i = 0; i < MT; i++) a[i][(ks + PF) % NB] = ap[i][4 * (ks + PF)];
+        }
+#pragma unroll
+        for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][ks % NB], b[ks % NB]);
+      }
       const bool c0 = nt < NDT - 1 || 8 * nt + 2 * c < nao, c1 = nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao;
 #pragma unroll
       for (int i = 0; i < MT; i++) {
         if (rok[i] && c0) o[i][0] = make_double2(cr[i][0], ci[i][0]);
         if (rok[i] && c1) o[i][ostride] = make_double2(cr[i][1], ci[i][1]);
         o[i] += 8 * ostride;
-        cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0;
       }
     }
   }
