@@ -143,33 +143,9 @@ __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const 
   ostride = TRANSPOSED ? nao : 1;
   const c128 *bp = sG + g * ldp + c;
   double cr[MT][2], ci[MT][2];
-  if (CACHE_A) {
-    // short K: one flat, fully unrolled (n-tile, k-step) sequence with the B fragments PF steps ahead
-    c128 b[NB];
-#pragma unroll
-    for (int s = 0; s < PF && s < S; s++) b[s % NB] = bp[(s / KSP) * 8 * ldp + 4 * (s % KSP)];
-#pragma unroll
-    for (int i = 0; i < MT; i++) { cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0; }
-#pragma unroll
-    for (int s = 0; s < S; s++) {
-      const int nt = s / KSP, ks = s % KSP;
-      if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
-#pragma unroll
-      for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][ks], b[s % NB]);
-      if (ks == KSP - 1) {
-        // only the last n-tile can reach beyond nao: 8*(NDT-1) <= 4*(KSP-1) < nao
-        const bool c0 = nt < NDT - 1 || 8 * nt + 2 * c < nao, c1 = nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao;
-#pragma unroll
-        for (int i = 0; i < MT; i++) {
-          if (rok[i] && c0) o[i][0] = make_double2(cr[i][0], ci[i][0]);
-          if (rok[i] && c1) o[i][ostride] = make_double2(cr[i][1], ci[i][1]);
-          o[i] += 8 * ostride;
-          cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0;
-        }
-      }
-    }
-  } else {
-    // long K: a real loop over the n-tiles (bounded register pressure), A and B fragments streamed PF k-steps ahead
+  {
+    // a real loop over the n-tiles (bounded register pressure); B fragments (and, for long K, A fragments) are streamed
+    // PF k-steps ahead
 #pragma unroll 1
     for (int nt = 0; nt < NDT; nt++) {
       const c128 *bq = bp + nt * 8 * ldp;
@@ -177,8 +153,10 @@ __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const 
 #pragma unroll
       for (int ks = 0; ks < PF && ks < KSP; ks++) {
         b[ks % NB] = bq[4 * ks];
+        if (!CACHE_A) {
 #pragma unroll
-        for (int i = 0; i < MT; i++) a[i][ks % NB] = ap[i][4 * ks];
+          for (int i = 0; i < MT; i++) a[i][ks % NB] = ap[i][4 * ks];
+        }
       }
 #pragma unroll
       for (int i = 0; i < MT; i++) { cr[i][0] = cr[i][1] = 0.0; ci[i][0] = ci[i][1] = 0.0; }
@@ -186,11 +164,13 @@ __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const 
       for (int ks = 0; ks < KSP; ks++) {
         if (ks + PF < KSP) {
           b[(ks + PF) % NB] = bq[4 * (ks + PF)];
+          if (!CACHE_A) {
 #pragma unroll
-          for (int i = 0; i < MT; i++) a[i][(ks + PF) % NB] = ap[i][4 * (ks + PF)];
+            for (int i = 0; i < MT; i++) a[i][(ks + PF) % NB] = ap[i][4 * (ks + PF)];
+          }
         }
 #pragma unroll
-        for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][ks % NB], b[ks % NB]);
+        for (int i = 0; i < MT; i++) cmma(cr[i], ci[i], a[i][CACHE_A ? ks : ks % NB], b[ks % NB]);
       }
       const bool c0 = nt < NDT - 1 || 8 * nt + 2 * c < nao, c1 = nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao;
 #pragma unroll
