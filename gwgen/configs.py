@@ -51,6 +51,8 @@ CONFIGS = {
     "P": GWConfig("cfgP", (4, 4, 4), 26, 200, 8, 8, 700.0, -2.0, 3.0, 0.04, BASE_SEED + 97),
     # mid-size ragged config for parity tests: sizes that are not multiples of any tile
     "R": GWConfig("cfgR", (3, 2, 2), 7, 37, 18, 18, 30.0, -1.5, 2.0, 0.04, BASE_SEED + 98),
+    # small problem with the production basis size (nao=26: the straight-line / warp-specialised kernel variants), ragged naux
+    "S": GWConfig("cfgS", (2, 1, 2), 26, 44, 8, 8, 40.0, -2.0, 3.0, 0.04, BASE_SEED + 94),
     # config-4-shaped problem with a short tau grid (same per-CTA behaviour, 15x less work)
     "Q": GWConfig("cfgQ", (4, 4, 4), 52, 400, 8, 8, 1000.0, -3.0, 5.0, 0.04, BASE_SEED + 95),
     # config-4-shaped basis (nao=52, naux > 224: the wide-panel / split-K kernel variants) at a size the oracle does in full

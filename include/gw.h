@@ -61,7 +61,18 @@ typedef struct {
   const gw_c128 *T_tw;     /* device [ntau][nw]: bosonic iΩ→τ transform matrix, Eq. 30 */
   void *work;              /* device scratch shared by the four calls (L2-resident intermediates, solver copies), */
   size_t work_bytes;       /*   at least gw_workspace_bytes(p) bytes, 256-byte aligned; contents are don't-care    */
+  int32_t symmetry;        /* 0 = evaluate Algorithm 1 literally (default); GW_SYM_TR = the caller asserts time-reversal   */
+  int32_t reserved;        /*   symmetric inputs (see GW_SYM_TR below); must be 0                                          */
 } gw_problem;
+
+/* gw_problem.symmetry flag.  Time reversal: G[t][−k] = conj(G[t][k]) and V[−k1][−k2] = conj(V[k1][k2]) element-wise (the same
+ * property that makes I − P̃0(iΩ) Hermitian for the Cholesky solve; the paper exploits k ↔ −k too).  Then
+ * P̃0^q(β−τ) = P̃0^q(τ) and Σ^{−k}(τ) = conj Σ^{k}(τ), and the library evaluates only the irreducible half and copies the rest:
+ *   gw_polarization : tau nodes t <= ntau-1-t are computed, P0t[ntau-1-t] is a copy of P0t[t];
+ *   gw_selfenergy   : k <= −k are computed, Sigma[t][−k] = conj(Sigma[t][k])  (only for the full q range and nk <= 128);
+ * the other calls ignore the flag.  Computed elements are bit-identical to the literal evaluation.  If the inputs do not
+ * have the symmetry the copied elements are wrong — nothing checks it. */
+enum { GW_SYM_TR = 1 };
 
 /* Stage 1 — Eq. 28b, Algorithm 1 first k loop:
  *   P0t[t][q-q_begin][Q][Q'] = -(s/N_k) Σ_k Σ_abcd V[k][k+q][Q][d][a] G[t][k+q][a][b] V[k+q][k][Q'][b][c] G[ntau-1-t][k][c][d]

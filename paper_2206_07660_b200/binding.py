@@ -13,13 +13,17 @@ class GWError(RuntimeError):
     pass
 
 
+GW_SYM_TR = 1   # gw_problem.symmetry flag (include/gw.h)
+
+
 class _CProblem(ctypes.Structure):
     _fields_ = [("nk1", ctypes.c_int32), ("nk2", ctypes.c_int32), ("nk3", ctypes.c_int32),
                 ("nao", ctypes.c_int32), ("naux", ctypes.c_int32), ("ntau", ctypes.c_int32), ("nw", ctypes.c_int32),
                 ("spin_deg", ctypes.c_int32), ("q_begin", ctypes.c_int32), ("q_end", ctypes.c_int32),
                 ("beta", ctypes.c_double),
                 ("V", ctypes.c_void_p), ("T_wt", ctypes.c_void_p), ("T_tw", ctypes.c_void_p),
-                ("work", ctypes.c_void_p), ("work_bytes", ctypes.c_size_t)]
+                ("work", ctypes.c_void_p), ("work_bytes", ctypes.c_size_t),
+                ("symmetry", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 def lib_path():
@@ -88,7 +92,8 @@ class GWProblem:
 
     V, T_wt, T_tw: CUDA complex128 tensors for the device calls, or CPU tensors for gw_sigma_iteration_host."""
 
-    def __init__(self, mesh, nao, naux, ntau, nw, beta, V, T_wt, T_tw, spin_deg=2, q_begin=0, q_end=None):
+    def __init__(self, mesh, nao, naux, ntau, nw, beta, V, T_wt, T_tw, spin_deg=2, q_begin=0, q_end=None, symmetry=0):
+        self.symmetry = int(symmetry)      # 0 = literal Algorithm 1; GW_SYM_TR = time-reversal symmetric inputs (gw.h)
         self.mesh = tuple(int(m) for m in mesh)
         self.nk = self.mesh[0] * self.mesh[1] * self.mesh[2]
         self.nao, self.naux, self.ntau, self.nw = int(nao), int(naux), int(ntau), int(nw)
@@ -103,7 +108,7 @@ class GWProblem:
                 raise GWError(f"{name}: need contiguous complex128 of shape {shape}, got {tuple(t.shape)} {t.dtype}")
         self.c = _CProblem(self.mesh[0], self.mesh[1], self.mesh[2], self.nao, self.naux, self.ntau, self.nw,
                            self.spin_deg, self.q_begin, self.q_end, self.beta,
-                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr(), None, 0)
+                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr(), None, 0, self.symmetry, 0)
         self.work = None
         if V.is_cuda:
             self.set_work(torch.empty(int(lib().gw_workspace_bytes(ctypes.byref(self.c))), dtype=torch.uint8, device=V.device))
@@ -120,7 +125,7 @@ class GWProblem:
 
     def shard(self, q_begin, q_end):
         return GWProblem(self.mesh, self.nao, self.naux, self.ntau, self.nw, self.beta, self.V, self.T_wt, self.T_tw,
-                         self.spin_deg, q_begin, q_end)
+                         self.spin_deg, q_begin, q_end, self.symmetry)
 
     def ref(self):
         return ctypes.byref(self.c)

@@ -13,13 +13,14 @@ struct GwDims {
   int nao, naux, ntau, nw;
   int s;            // spin_deg
   int q0, nq;       // q shard
+  int sym;          // gw_problem.symmetry
 };
 
 static inline GwDims gw_dims(const gw_problem *p) {
   GwDims d;
   d.nk1 = p->nk1; d.nk2 = p->nk2; d.nk3 = p->nk3; d.nk = p->nk1 * p->nk2 * p->nk3;
   d.nao = p->nao; d.naux = p->naux; d.ntau = p->ntau; d.nw = p->nw; d.s = p->spin_deg;
-  d.q0 = p->q_begin; d.nq = p->q_end - p->q_begin;
+  d.q0 = p->q_begin; d.nq = p->q_end - p->q_begin; d.sym = p->symmetry;
   return d;
 }
 

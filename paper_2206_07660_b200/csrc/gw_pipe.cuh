@@ -117,7 +117,7 @@ __device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c12
 template <int KSP, bool TRANSPOSED, int MT>
 __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
                                                       int nao, int ldp, int w, FastDiv fd) {
-  constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 3, NB = PF + 1;
+  constexpr int NDT = (KSP + 1) / 2, PF = 3, NB = PF + 1;
   constexpr bool CACHE_A = KSP * MT <= 8;   // keep the A fragments of the m-tile(s) in registers, else stream them like B
   constexpr int NA = CACHE_A ? KSP : NB;
   const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
@@ -256,8 +256,10 @@ __device__ __forceinline__ void final_compute_exact(const c128 *stage, double (&
 
 // store the warp-owned tiles of an nao x nao result, scaled
 template <int NCT>
-__device__ __forceinline__ void final_store(c128 *out, const double (&sgr)[NCT][2], const double (&sgi)[NCT][2], double pref, int nao, int ndt) {
+__device__ __forceinline__ void final_store(c128 *out, const double (&sgr)[NCT][2], const double (&sgi)[NCT][2], double pref, int nao, int ndt,
+                                            bool conj = false) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+  const double prefi = conj ? -pref : pref;
 #pragma unroll
   for (int ti = 0; ti < NCT; ti++) {
     const int tile = w + 8 * ti;
@@ -265,8 +267,8 @@ __device__ __forceinline__ void final_store(c128 *out, const double (&sgr)[NCT][
       const int mi = tile / ndt, nj = tile - mi * ndt;
       const int i = 8 * mi + g, j = 8 * nj + 2 * c;
       if (i < nao) {
-        if (j < nao) out[i * nao + j] = make_double2(pref * sgr[ti][0], pref * sgi[ti][0]);
-        if (j + 1 < nao) out[i * nao + j + 1] = make_double2(pref * sgr[ti][1], pref * sgi[ti][1]);
+        if (j < nao) out[i * nao + j] = make_double2(pref * sgr[ti][0], prefi * sgi[ti][0]);
+        if (j + 1 < nao) out[i * nao + j + 1] = make_double2(pref * sgr[ti][1], prefi * sgi[ti][1]);
       }
     }
   }

@@ -42,6 +42,7 @@ struct Params {
   c128 *P0t, *scratch;
   int cs;                // CTAs per cluster = column splits of the panel
   int nqt, nitems;       // Q tiles per (t,q); total work items
+  int nteff;             // tau nodes evaluated: ntau, or ceil(ntau/2) under GW_SYM_TR (the rest is mirrored)
   int ldp, ksp, ndt;     // pass smem row stride (complex), k-steps = ceil(nao/4), n-tiles over nao
   int nt, ntc;           // n-tiles over naux; n-tiles per CTA
   int main_units, pass_units;   // complex elements per main / pass stage buffer
@@ -64,11 +65,20 @@ struct Ring {
   __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); advance(); }
 };
 
+// L2 eviction policies: the slabs are read exactly once after they are written (evict first), the V blocks are shared by
+// every CTA working on the same q (evict last)
+__device__ __forceinline__ uint64_t policy_evict_first() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p)); return p; }
+__device__ __forceinline__ uint64_t policy_evict_last() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p)); return p; }
+__device__ __forceinline__ void cpa_hint(unsigned dst, const void *src, int nbytes, uint64_t pol) {
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst), "l"(src), "r"(nbytes), "l"(pol));
+}
+
 // main job: A = Z[TM rows][k0..k0+8), B = Vb[brows rows][k0..k0+8); 16-byte units swizzled by row parity.
 // Rows beyond the valid range re-read the last valid row (their products land in accumulators that are never stored);
 // only the K tail of the last job is zero filled.  Each thread owns one 16-byte unit column and walks the rows with
 // constant strides, so the loop body is one address add per copy.
-__device__ __forceinline__ void issue_main(c128 *stage, const c128 *Z, int tm_rows, const c128 *Vb, int ncols, int brows, int n2, int k0) {
+__device__ __forceinline__ void issue_main(c128 *stage, const c128 *Z, int tm_rows, const c128 *Vb, int ncols, int brows, int n2, int k0,
+                                           uint64_t polA, uint64_t polB) {
   constexpr int RS = N_MPROD / 8;                      // rows per sweep of the producer threads
   const int pt = threadIdx.x - T_MPROD;
   const int u = pt & 7, rsub = pt >> 3;
@@ -82,7 +92,7 @@ __device__ __forceinline__ void issue_main(c128 *stage, const c128 *Z, int tm_ro
     for (int r = rsub; r < TM; r += RS) {
       const int rr = min(r, tm_rows - 1);
       const unsigned dst = (sbase + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src + (size_t)rr * n2), "r"(nbytes));
+      cpa_hint(dst, src + (size_t)rr * n2, nbytes, polA);
     }
   }
   const unsigned sB = sbase + 16u * TM * KC;
@@ -92,15 +102,15 @@ __device__ __forceinline__ void issue_main(c128 *stage, const c128 *Z, int tm_ro
   const c128 *sp = src + (size_t)r * n2;
   for (; r + 3 * RS < ncols; r += 4 * RS, sp += 4 * step) {      // rows r, r+RS, r+2RS, r+3RS all valid (RS is even: same row parity)
     const unsigned dst = (sB + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(sp), "r"(nbytes));
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst + RS * 16u * KC), "l"(sp + step), "r"(nbytes));
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst + 2 * RS * 16u * KC), "l"(sp + 2 * step), "r"(nbytes));
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst + 3 * RS * 16u * KC), "l"(sp + 3 * step), "r"(nbytes));
+    cpa_hint(dst, sp, nbytes, polB);
+    cpa_hint(dst + RS * 16u * KC, sp + step, nbytes, polB);
+    cpa_hint(dst + 2 * RS * 16u * KC, sp + 2 * step, nbytes, polB);
+    cpa_hint(dst + 3 * RS * 16u * KC, sp + 3 * step, nbytes, polB);
   }
   for (; r < brows; r += RS) {
     const int rr = min(r, ncols - 1);
     const unsigned dst = (sB + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src + (size_t)rr * n2), "r"(nbytes));
+    cpa_hint(dst, src + (size_t)rr * n2, nbytes, polB);
   }
 }
 
@@ -145,10 +155,10 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
 // decode a work item: Q-tile index slowest (the round-robin gives every cluster the same mix of full and ragged tiles),
 // then q, then t fastest (concurrent clusters share the V blocks of one q in L2)
 struct Item { int t, ql, Q0, tm_rows; };
-__device__ __forceinline__ Item decode_item(const GwDims &d, int item) {
+__device__ __forceinline__ Item decode_item(const GwDims &d, int nteff, int item) {
   Item it;
-  const int qt = item / (d.ntau * d.nq);
-  it.t = item % d.ntau; it.ql = (item / d.ntau) % d.nq; it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
+  const int qt = item / (nteff * d.nq);
+  it.t = item % nteff; it.ql = (item / nteff) % d.nq; it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
   return it;
 }
 
@@ -202,8 +212,9 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
       unsigned kit = 0;
       const int brows = 8 * ntc_mine;
+      const uint64_t polA = policy_evict_first(), polB = policy_evict_last();
       for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(d, item);
+        const Item it = decode_item(d, P.nteff, item);
         const int q = d.q0 + it.ql;
         for (int k = 0; k < d.nk; k++, kit++) {
           const int kq = gw_kadd(d, k, q);
@@ -213,7 +224,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
           else gwp::mbar_wait(zready + (kit & 1u), (kit >> 1) & 1u);
           for (int j = 0; j < nmain; j++) {
             const int s = rm.acquire();
-            issue_main(sMain + s * P.main_units, Z, it.tm_rows, Vb, ncols, brows, n2, j * KC);
+            issue_main(sMain + s * P.main_units, Z, it.tm_rows, Vb, ncols, brows, n2, j * KC, polA, polB);
             rm.commit();
           }
         }
@@ -224,7 +235,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
       unsigned kit = 0, ph = 0;
       for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(d, item);
+        const Item it = decode_item(d, P.nteff, item);
         const int q = d.q0 + it.ql;
         const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
         for (int k = 0; k < d.nk; k++, kit++) {
@@ -266,7 +277,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
     unsigned kit = 0, ph = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
-      const Item it = decode_item(d, item);
+      const Item it = decode_item(d, P.nteff, item);
       const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
       for (int k = 0; k < d.nk; k++, kit++) {
         c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
@@ -312,7 +323,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned kit = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
-      const Item it = decode_item(d, item);
+      const Item it = decode_item(d, P.nteff, item);
       const int mtc = (it.tm_rows + 7) / 8;
       const bool active = (mh * MT_W < mtc) && njm > 0;
       double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
@@ -357,16 +368,21 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       }
       // ---- epilogue: scale by -(s/N_k), store this CTA's columns of the panel ----
       const double pref = -(double)d.s / (double)d.nk;
-      c128 *out = P.P0t + ((size_t)it.t * d.nq + it.ql) * naux * naux + col0;
+      // under GW_SYM_TR the mirrored tau node receives a copy: P0^q(beta - tau) = P0^q(tau)
+      const int tbar = d.ntau - 1 - it.t;
+      const int ncopy = (P.nteff < d.ntau && tbar != it.t) ? 2 : 1;
+      for (int cp = 0; cp < ncopy; cp++) {
+        c128 *out = P.P0t + ((size_t)(cp ? tbar : it.t) * d.nq + it.ql) * naux * naux + col0;
 #pragma unroll
-      for (int i = 0; i < MT_W; i++) {
-        const int Q = it.Q0 + 8 * (mh * MT_W + i) + g;
+        for (int i = 0; i < MT_W; i++) {
+          const int Q = it.Q0 + 8 * (mh * MT_W + i) + g;
 #pragma unroll
-        for (int jn = 0; jn < NJ; jn++) {
-          if (jn < njm && Q < naux) {
-            const int col = 8 * (noff + 4 * jn) + 2 * c;
-            if (col < ncols) out[(size_t)Q * naux + col] = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
-            if (col + 1 < ncols) out[(size_t)Q * naux + col + 1] = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
+          for (int jn = 0; jn < NJ; jn++) {
+            if (jn < njm && Q < naux) {
+              const int col = 8 * (noff + 4 * jn) + 2 * c;
+              if (col < ncols) out[(size_t)Q * naux + col] = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
+              if (col + 1 < ncols) out[(size_t)Q * naux + col + 1] = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
+            }
           }
         }
       }
@@ -377,7 +393,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
 }
 
 struct Plan {
-  int cs, ksp_max, nqt, nitems, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
+  int cs, ksp_max, nqt, nitems, nteff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
   size_t smem, slab_units, work_bytes;
   bool ok;
 };
@@ -395,7 +411,8 @@ static Plan make_plan(const gw_problem *p) {
   int r4 = pl.ksp * 4; if (r4 % 8 == 0) r4 += 4;
   pl.ldp = r4;
   pl.nqt = (d.naux + TM - 1) / TM;
-  pl.nitems = pl.nqt * d.ntau * d.nq;
+  pl.nteff = (d.sym & GW_SYM_TR) ? (d.ntau + 1) / 2 : d.ntau;
+  pl.nitems = pl.nqt * pl.nteff * d.nq;
   pl.main_units = (TM + 8 * pl.ntc) * KC;
   pl.prows = 32;
   pl.pass_units = pl.prows * pl.ldp;
@@ -450,7 +467,7 @@ double gw_stage1_flops(const gw_problem *p) {
     const double mainv = mtiles * pl.nt * (s1::KC / 4) * nmain;
     tiles += pass + mainv;
   }
-  return tiles * (double)d.nk * d.ntau * d.nq * 2048.0;
+  return tiles * (double)d.nk * pl.nteff * d.nq * 2048.0;
 }
 
 template <int KSP_MAX>
@@ -485,7 +502,7 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   s1::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
+  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
   P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);

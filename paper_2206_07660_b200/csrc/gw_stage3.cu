@@ -11,6 +11,14 @@
 // U and T live in two per-CTA slabs of the workspace (L2 resident); the raw V2 block is the only big stream.
 #include "gw_pipe.cuh"
 
+// GW_SYM_TR bookkeeping shared by both stage-3 kernels: the k <= -k half of the mesh (only for the full q range, nk <= 128)
+static int fill_kirr(const GwDims &d, short *kirr) {
+  if (!(d.sym & GW_SYM_TR) || d.nk > 128 || d.q0 != 0 || d.nq != d.nk) return d.nk;
+  int n = 0;
+  for (int k = 0; k < d.nk; k++) if (k <= gw_ksub(d, 0, k)) kirr[n++] = (short)k;
+  return n;
+}
+
 namespace s3 {
 
 using gwp::NCONS; using gwp::NTHR_WS; using gwp::PASS_ROWS; using gwp::FastDiv; using gwp::Ring;
@@ -30,6 +38,9 @@ struct Params {
   int ldb;                // row stride of the main-job B part
   int stage_units, nstage;
   size_t slab_units;      // complex elements per slab (two slabs per CTA)
+  int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
+  short kirr[128];        // the evaluated k points when nkeff < nk
+  __device__ __forceinline__ int kof(int i) const { return nkeff < d.nk ? (int)kirr[i] : i; }
   FastDiv fd_nao;
 };
 
@@ -108,7 +119,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
     // =============================== producer warpgroup ===============================
     gwp::reg_dec<40>();
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      const int t = item % d.ntau, k = item / d.ntau;
+      const int t = item % d.ntau, k = P.kof(item / d.ntau);
       for (int ql = 0; ql < d.nq; ql++) {
         const int q = d.q0 + ql, kp = gw_ksub(d, k, q);
         const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
@@ -155,7 +166,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
     const int sw = (g & 1) << 2;
     const int noff = ((w & 3) - mh + 4) & 3;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      const int t = item % d.ntau, k = item / d.ntau;
+      const int t = item % d.ntau, k = P.kof(item / d.ntau);
       double sgr[NCT][2], sgi[NCT][2];
 #pragma unroll
       for (int i = 0; i < NCT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
@@ -228,7 +239,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
           const int rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
           for (int jb = 0; jb < npass; jb++) {
             const int s = ring.wait();
-            if (P.ksp == KSP_MAX) gwp::pass_compute_exact<KSP_MAX, true>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp);
+            if (P.ksp == KSP_MAX) gwp::pass_compute_exact_mt<KSP_MAX, true, 1>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, w, P.fd_nao);
             else gwp::pass_compute<KSP_MAX, true>(sStage + s * P.stage_units, sG, slabT, jb * PASS_ROWS, rows, nao, ldp, P.ksp, ndt);
             ring.release();
           }
@@ -245,6 +256,10 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
         }
       }
       gwp::final_store<NCT>(P.Sigma + ((size_t)t * d.nk + k) * n2, sgr, sgi, -1.0 / (double)d.nk, nao, ndt);
+      if (P.nkeff < d.nk) {                                   // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
+        const int kn = gw_ksub(d, 0, k);
+        if (kn != k) gwp::final_store<NCT>(P.Sigma + ((size_t)t * d.nk + kn) * n2, sgr, sgi, -1.0 / (double)d.nk, nao, ndt, true);
+      }
     }
   }
 }
@@ -272,7 +287,7 @@ static Plan make_plan(const gw_problem *p) {
   pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
   pl.ldb = pl.cht * 8 + 2;
   pl.nqt = (d.naux + TM - 1) / TM;
-  pl.nitems = d.ntau * d.nk;
+  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
   const int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + KC * pl.ldb;
   const size_t fixed = (size_t)naop * pl.ldp * sizeof(c128);
   // final jobs cover one Q, or half of its K range when a whole Q would leave fewer than 3 ring stages
@@ -317,7 +332,8 @@ double gw_stage3_flops(const gw_problem *p) {
     tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.ndt * pl.ksp;           // pass A
     tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.kspf * pl.kh;             // final
   }
-  return tiles * (double)d.nq * d.nk * d.ntau * 2048.0;
+  short tmp[128];
+  return tiles * (double)d.nq * fill_kirr(d, tmp) * d.ntau * 2048.0;
 }
 
 template <int KSP_MAX, int NCT>
@@ -339,6 +355,7 @@ static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigm
   P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt; P.kh = pl.kh; P.kspf = pl.kspf; P.ldpf = pl.ldpf; P.fd_kw = gwp::FastDiv((unsigned)(4 * pl.kspf));
   P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
+  P.nkeff = fill_kirr(P.d, P.kirr);
   if (pl.nct == 2) {
     if (pl.ksp_max == 7) return launch_sigma<7, 2>(pl, P, st);
     if (pl.ksp_max == 13) return launch_sigma<13, 2>(pl, P, st);
@@ -380,6 +397,9 @@ struct Params {
   int ldb;                // row stride of the main-job B part
   int main_units, aux_units, nstage, astage;
   size_t slab_units;      // complex elements per slab (three slabs per CTA: U0, U1, T)
+  int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
+  short kirr[128];        // the evaluated k points when nkeff < nk
+  __device__ __forceinline__ int kof(int i) const { return nkeff < d.nk ? (int)kirr[i] : i; }
   FastDiv fd_nao;
 };
 
@@ -398,11 +418,16 @@ struct Ring {
 __device__ __forceinline__ void cpa(unsigned dst, const void *src, int nbytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(nbytes));
 }
+// with an L2 eviction policy: the V blocks are shared by the ~100 CTAs that work on the same k (evict last)
+__device__ __forceinline__ void cpa_hint(unsigned dst, const void *src, int nbytes, uint64_t pol) {
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst), "l"(src), "r"(nbytes), "l"(pol));
+}
+__device__ __forceinline__ uint64_t policy_evict_last() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p)); return p; }
 
 // main job: A = W[TM rows][k0..k0+8) swizzled by row parity (rows beyond tm_rows re-read the last valid row);
 // B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb] (K rows beyond naux and columns beyond nao² zero filled)
 __device__ __forceinline__ void issue_main(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
-                                           int n0, int ncols, int ldb, int k0) {
+                                           int n0, int ncols, int ldb, int k0, uint64_t polB) {
   const int pt = threadIdx.x - T_MPROD;
   const unsigned sA = gwp::smem_u32(stage);
   {
@@ -424,7 +449,7 @@ __device__ __forceinline__ void issue_main(c128 *stage, const c128 *W, int tm_ro
 #pragma unroll
     for (int r = 0; r < KC; r++) {
       const bool ok = cok && (k0 + r < naux);
-      cpa(dst + 16u * (unsigned)(r * ldb), ok ? src + (size_t)r * n2 : V2, ok ? 16 : 0);
+      cpa_hint(dst + 16u * (unsigned)(r * ldb), ok ? src + (size_t)r * n2 : V2, ok ? 16 : 0, polB);
     }
   }
 }
@@ -528,8 +553,9 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
     if (w < 15) {
       // ---- main-ring producer: W panel rows and V2 chunk rows ----
       Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
+      const uint64_t polB = policy_evict_last();
       for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-        const int t = item % d.ntau, k = item / d.ntau;
+        const int t = item % d.ntau, k = P.kof(item / d.ntau);
         for (int ql = 0; ql < d.nq; ql++) {
           const int kp = gw_ksub(d, k, d.q0 + ql);
           const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
@@ -541,7 +567,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
               const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
               for (int j = 0; j < nmain; j++) {
                 const int s = rm.acquire();
-                issue_main(sMain + s * P.main_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC);
+                issue_main(sMain + s * P.main_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC, polB);
                 rm.commit();
               }
             }
@@ -554,7 +580,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
       Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
       unsigned un = 0;
       for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-        const int t = item % d.ntau, k = item / d.ntau;
+        const int t = item % d.ntau, k = P.kof(item / d.ntau);
         for (int ql = 0; ql < d.nq; ql++) {
           const int kp = gw_ksub(d, k, d.q0 + ql);
           const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
@@ -589,7 +615,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
     Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
     unsigned un = 0;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      const int t = item % d.ntau, k = item / d.ntau;
+      const int t = item % d.ntau, k = P.kof(item / d.ntau);
       double sgr[NDT][2], sgi[NDT][2];
 #pragma unroll
       for (int i = 0; i < NDT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
@@ -613,14 +639,19 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
       }
       // Sigma[t][k] = -(1/N_k) acc: this warp's column tile of the four row tiles
       const double pref = -1.0 / (double)d.nk;
-      c128 *out = P.Sigma + ((size_t)t * d.nk + k) * n2;
+      const int kn = gw_ksub(d, 0, k);
+      const int ncopy = (P.nkeff < d.nk && kn != k) ? 2 : 1;  // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
       const int j0 = 8 * wa + 2 * c;
+      for (int cp = 0; cp < ncopy; cp++) {
+        c128 *out = P.Sigma + ((size_t)t * d.nk + (cp ? kn : k)) * n2;
+        const double prefi = cp ? -pref : pref;
 #pragma unroll
-      for (int mi = 0; mi < NDT; mi++) {
-        const int i = 8 * mi + g;
-        if (i < nao) {
-          if (j0 < nao) out[i * nao + j0] = make_double2(pref * sgr[mi][0], pref * sgi[mi][0]);
-          if (j0 + 1 < nao) out[i * nao + j0 + 1] = make_double2(pref * sgr[mi][1], pref * sgi[mi][1]);
+        for (int mi = 0; mi < NDT; mi++) {
+          const int i = 8 * mi + g;
+          if (i < nao) {
+            if (j0 < nao) out[i * nao + j0] = make_double2(pref * sgr[mi][0], prefi * sgi[mi][0]);
+            if (j0 + 1 < nao) out[i * nao + j0 + 1] = make_double2(pref * sgr[mi][1], prefi * sgi[mi][1]);
+          }
         }
       }
     }
@@ -702,7 +733,7 @@ static Plan make_plan(const gw_problem *p) {
   pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
   pl.ldb = pl.cht * 8 + 2;
   pl.nqt = (d.naux + TM - 1) / TM;
-  pl.nitems = d.ntau * d.nk;
+  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
   pl.main_units = TM * KC + KC * pl.ldb;
   const int s_pass = AROWS * pl.ldp, s_fin = 8 * NDT * pl.ldp + 4 * KSP * pl.ldt + 8;
   pl.aux_units = s_pass > s_fin ? s_pass : s_fin;
@@ -729,6 +760,7 @@ static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigm
   P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ldt = pl.ldt; P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb;
   P.main_units = pl.main_units; P.aux_units = pl.aux_units; P.nstage = pl.nstage; P.astage = pl.astage; P.slab_units = pl.slab_units;
   P.fd_nao = FastDiv((unsigned)P.d.nao);
+  P.nkeff = fill_kirr(P.d, P.kirr);
   cudaError_t e = cudaFuncSetAttribute(sigma_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
   sigma_ws_kernel<<<pl.grid, NTHR, pl.smem, st>>>(P);

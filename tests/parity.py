@@ -16,13 +16,13 @@ def worst_slice(a, b, lead=2):
     return float(np.max(num / np.maximum(den, 1e-300)))
 
 
-def device_problem(p, q_begin=0, q_end=None, device="cuda"):
+def device_problem(p, q_begin=0, q_end=None, device="cuda", symmetry=0):
     import paper_2206_07660_b200 as gw
     cfg = p.cfg
     V = p.V.to(device) if isinstance(p.V, torch.Tensor) else torch.from_numpy(p.V).to(device)
     prob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, V,
                         torch.from_numpy(p.T_wt).to(device), torch.from_numpy(p.T_tw).to(device),
-                        cfg.spin_deg, q_begin, q_end)
+                        cfg.spin_deg, q_begin, q_end, symmetry)
     G = torch.from_numpy(p.G).to(device)
     gamma = torch.from_numpy(p.gamma).to(device)
     return prob, G, gamma

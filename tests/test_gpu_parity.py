@@ -22,7 +22,7 @@ def run_gpu(p, **kw):
     return {k: v.cpu().numpy() for k, v in out.items()}
 
 
-@pytest.mark.parametrize("name", ["0", "T", "R", "L"])
+@pytest.mark.parametrize("name", ["0", "T", "R", "S", "L"])
 def test_full_parity_small(problems, oracle_results, name):
     p = problems(name)
     ref = oracle_results(name)
@@ -229,3 +229,34 @@ def test_phi_parity(problems, oracle_results, oracle_lib, name):
     want = np.array([[oracle_lib.phi(ref["P0w"][n, q]) for q in range(cfg.nk)] for n in range(cfg.nw)])
     got = phi.cpu().numpy()
     assert np.max(np.abs(got - want) / np.maximum(1.0, np.abs(want))) <= 1e-10
+
+
+@pytest.mark.parametrize("name", ["T", "R", "S", "L", "1"])
+def test_time_reversal_mode_parity(problems, oracle_results, oracle_lib, name):
+    """gw_problem.symmetry = GW_SYM_TR (irreducible tau / k halves computed, the rest copied) against the oracle, which
+    uses no symmetry: every element of P0t, Wt, Sigma, K to 1e-10; the computed half is bit-identical to the literal run."""
+    import gwgen
+    import paper_2206_07660_b200 as gw
+    if name == "1":
+        p = gwgen.make_problem("1")
+        cfg = p.cfg
+        vb = oracle_lib.VBlocks(cfg, p.V.numpy())
+        ref = {"P0t": oracle_lib.polarization(cfg, vb, p.G)}
+        ref["Wt"] = oracle_lib.screened_interaction(cfg, p.T_wt, p.T_tw, ref["P0t"])
+        ref["Sigma"] = oracle_lib.selfenergy(cfg, vb, p.G, ref["Wt"])
+        ref["K"] = oracle_lib.exchange(cfg, vb, p.gamma)
+    else:
+        p = problems(name); ref = oracle_results(name); cfg = p.cfg
+    got = run_gpu(p, symmetry=gw.GW_SYM_TR)
+    lit = run_gpu(p)
+    for key in ("P0t", "Wt", "Sigma", "K"):
+        assert relerr(got[key], ref[key]) <= TOL, (name, key)
+    half_t = (cfg.ntau + 1) // 2
+    assert np.array_equal(got["P0t"][:half_t], lit["P0t"][:half_t])
+    k0 = 0                                                # Gamma is its own partner: always in the computed half
+    assert relerr(got["Sigma"][:, k0], lit["Sigma"][:, k0]) <= 1e-12
+    # executed-work accounting follows the mode
+    prob_tr, _, _ = device_problem(p, symmetry=gw.GW_SYM_TR)
+    prob_li, _, _ = device_problem(p)
+    f_tr, f_li = gw.gw_executed_flops(prob_tr), gw.gw_executed_flops(prob_li)
+    assert f_tr[0] < 0.76 * f_li[0] and f_tr[2] <= f_li[2]
