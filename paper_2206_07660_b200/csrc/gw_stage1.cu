@@ -134,31 +134,33 @@ __device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao,
   }
 }
 
-// main warps: one main job (KC/4 k-steps) for this warp's MT_W x NJM tiles; all fragment loads hoisted per k-step
-template <int NJM>
+// main warps: one main job (KC/4 k-steps) for this warp's MTW x NJM tiles (n-tiles NSTRIDE apart); all fragment loads
+// hoisted per k-step
+template <int NJM, int NSTRIDE, int MTW>
 __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
     const int u = (4 * ks + c) ^ sw;
-    c128 a[MT_W], b[NJM];
+    c128 a[MTW], b[NJM];
 #pragma unroll
-    for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
+    for (int i = 0; i < MTW; i++) a[i] = sAw[i * 8 * KC + u];
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++) b[jn] = sBw[jn * 4 * 8 * KC + u];
+    for (int jn = 0; jn < NJM; jn++) b[jn] = sBw[jn * NSTRIDE * 8 * KC + u];
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++)
 #pragma unroll
-      for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
+      for (int i = 0; i < MTW; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
   }
 }
 
-// decode a work item: Q-tile index slowest (the round-robin gives every cluster the same mix of full and ragged tiles),
-// then q, then t fastest (concurrent clusters share the V blocks of one q in L2)
+// decode a work item: Q-tile index fastest (a cluster's item sequence cycles through full and ragged panels, so the short,
+// bandwidth-hungry ragged panels are spread over the whole run), then t, then q slowest (concurrent clusters share the V
+// blocks of one q in L2)
 struct Item { int t, ql, Q0, tm_rows; };
-__device__ __forceinline__ Item decode_item(const GwDims &d, int nteff, int item) {
+__device__ __forceinline__ Item decode_item(const GwDims &d, int nteff, int nqt, int item) {
   Item it;
-  const int qt = item / (nteff * d.nq);
-  it.t = item % nteff; it.ql = (item / nteff) % d.nq; it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
+  const int qt = item % nqt, r = item / nqt;
+  it.t = r % nteff; it.ql = r / nteff; it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
   return it;
 }
 
@@ -214,7 +216,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       const int brows = 8 * ntc_mine;
       const uint64_t polA = policy_evict_first(), polB = policy_evict_last();
       for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(d, P.nteff, item);
+        const Item it = decode_item(d, P.nteff, P.nqt, item);
         const int q = d.q0 + it.ql;
         for (int k = 0; k < d.nk; k++, kit++) {
           const int kq = gw_kadd(d, k, q);
@@ -235,7 +237,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
       unsigned kit = 0, ph = 0;
       for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(d, P.nteff, item);
+        const Item it = decode_item(d, P.nteff, P.nqt, item);
         const int q = d.q0 + it.ql;
         const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
         for (int k = 0; k < d.nk; k++, kit++) {
@@ -277,7 +279,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
     unsigned kit = 0, ph = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
-      const Item it = decode_item(d, P.nteff, item);
+      const Item it = decode_item(d, P.nteff, P.nqt, item);
       const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
       for (int k = 0; k < d.nk; k++, kit++) {
         c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
@@ -316,15 +318,21 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     // ========================================= main warps =========================================
     gwp::reg_inc<REG_MAIN>();
     const int g = lane >> 2, c = lane & 3;
-    const int mh = w >> 2;                               // m-half: m-tiles 2*mh, 2*mh+1
-    const int noff = ((w & 3) - mh + 4) & 3;             // first n-tile; n-tiles noff + 4*jn
-    const int njm = (ntc_mine > noff) ? (ntc_mine - noff + 3) / 4 : 0;
     const int sw = (g & 1) << 2;
     Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned kit = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
-      const Item it = decode_item(d, P.nteff, item);
+      const Item it = decode_item(d, P.nteff, P.nqt, item);
       const int mtc = (it.tm_rows + 7) / 8;
+      // tile ownership.  Full panels: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile.  Ragged last panel
+      // (<= 16 rows): all eight warps share m-tiles 0 (and 1), every 8th n-tile each, so the panel costs time in proportion
+      // to its rows instead of a full panel's.
+      const bool narrow = mtc <= 2;
+      const int mh = narrow ? 0 : (w >> 2);
+      const int noff = narrow ? w : (((w & 3) - mh + 4) & 3);
+      const int nstride = narrow ? 8 : 4;
+      const int mtw = (narrow && mtc == 1) ? 1 : MT_W;
+      const int njm = (ntc_mine > noff) ? (ntc_mine - noff + nstride - 1) / nstride : 0;
       const bool active = (mh * MT_W < mtc) && njm > 0;
       double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
 #pragma unroll
@@ -338,8 +346,12 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
           if (active) {
             const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + g) * KC;
             const c128 *sBw = sMain + s * P.main_units + TM * KC + (8 * noff + g) * KC;
-            if (njm == NJ) main_compute<NJ>(sAw, sBw, accr, acci, c, sw);
-            else if (njm == NJ - 1) main_compute<NJ - 1>(sAw, sBw, accr, acci, c, sw);
+            if (!narrow && njm == NJ) main_compute<NJ, 4, MT_W>(sAw, sBw, accr, acci, c, sw);
+            else if (!narrow && njm == NJ - 1) main_compute<NJ - 1, 4, MT_W>(sAw, sBw, accr, acci, c, sw);
+            else if (narrow && mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, accr, acci, c, sw);
+            else if (narrow && mtw == 1 && njm == 3) main_compute<3, 8, 1>(sAw, sBw, accr, acci, c, sw);
+            else if (narrow && mtw == 2 && njm == 4) main_compute<4, 8, 2>(sAw, sBw, accr, acci, c, sw);
+            else if (narrow && mtw == 2 && njm == 3) main_compute<3, 8, 2>(sAw, sBw, accr, acci, c, sw);
             else {
 #pragma unroll
               for (int ks = 0; ks < KC / 4; ks++) {
@@ -350,7 +362,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
 #pragma unroll
                 for (int jn = 0; jn < NJ; jn++) {
                   if (jn < njm) {
-                    const c128 b = sBw[jn * 4 * 8 * KC + u];
+                    const c128 b = sBw[jn * nstride * 8 * KC + u];
 #pragma unroll
                     for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
                   }
@@ -379,7 +391,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
 #pragma unroll
           for (int jn = 0; jn < NJ; jn++) {
             if (jn < njm && Q < naux) {
-              const int col = 8 * (noff + 4 * jn) + 2 * c;
+              const int col = 8 * (noff + nstride * jn) + 2 * c;
               if (col < ncols) out[(size_t)Q * naux + col] = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
               if (col + 1 < ncols) out[(size_t)Q * naux + col + 1] = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
             }
@@ -462,7 +474,7 @@ double gw_stage1_flops(const gw_problem *p) {
     const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp;
     const int mtc = (tm_rows + 7) / 8;
     // main: warps whose first m-tile is valid execute MT_W m-tiles x their n-tiles x 2 k-steps per job
-    const double mtiles = (double)((mtc + s1::MT_W - 1) / s1::MT_W) * s1::MT_W;
+    const double mtiles = mtc <= 2 ? (double)mtc : (double)((mtc + s1::MT_W - 1) / s1::MT_W) * s1::MT_W;   // ragged panel: narrow ownership
     const double nmain = (d.nao * d.nao + s1::KC - 1) / s1::KC;
     const double mainv = mtiles * pl.nt * (s1::KC / 4) * nmain;
     tiles += pass + mainv;

@@ -327,7 +327,7 @@ double gw_stage3_flops(const gw_problem *p) {
   for (int qt = 0; qt < pl.nqt; qt++) {
     const int tm_rows = (d.naux - qt * s3::TM) < s3::TM ? (d.naux - qt * s3::TM) : s3::TM;
     const int mtc = (tm_rows + 7) / 8;
-    const double mtiles = (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
+    const double mtiles = (((d.nao + 3) / 4 == 7) /* s3w kernel: narrow ragged panel */ && mtc <= 2) ? (double)mtc : (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
     tiles += mtiles * pl.nnt * (s3::KC / 4) * nmain;                         // main
     tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.ndt * pl.ksp;           // pass A
     tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.kspf * pl.kh;             // final
@@ -454,21 +454,21 @@ __device__ __forceinline__ void issue_main(c128 *stage, const c128 *W, int tm_ro
   }
 }
 
-template <int NJM>
+template <int NJM, int NSTRIDE = 4, int MTW = MT_W>
 __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, int ldb, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
     const int u = (4 * ks + c) ^ sw;
-    c128 a[MT_W], b[NJM];
+    c128 a[MTW], b[NJM];
 #pragma unroll
-    for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
+    for (int i = 0; i < MTW; i++) a[i] = sAw[i * 8 * KC + u];
     const c128 *brow = sBw + (4 * ks + c) * ldb;
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++) b[jn] = brow[32 * jn];
+    for (int jn = 0; jn < NJM; jn++) b[jn] = brow[8 * NSTRIDE * jn];
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++)
 #pragma unroll
-      for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
+      for (int i = 0; i < MTW; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
   }
 }
 
@@ -659,7 +659,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
     // ============================================ main warps ============================================
     gwp::reg_inc<REG_MAIN>();
     const int g = lane >> 2, c = lane & 3;
-    const int mh = w >> 2, sw = (g & 1) << 2, noff = ((w & 3) - mh + 4) & 3;
+    const int sw = (g & 1) << 2;
     Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned un = 0;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
@@ -667,9 +667,16 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
         for (int qt = 0; qt < P.nqt; qt++, un++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
           c128 *U = slabU + (size_t)(un & 1u) * P.slab_units;
+          // tile ownership: full panels as in s3::sigma_kernel; the ragged last panel (<= 16 rows) is shared by all eight
+          // warps (m-tiles 0 (and 1), every 8th n-tile each), so it costs time in proportion to its rows
+          const bool narrow = mtc <= 2;
+          const int mh = narrow ? 0 : (w >> 2);
+          const int noff = narrow ? w : (((w & 3) - mh + 4) & 3);
+          const int nstride = narrow ? 8 : 4;
+          const int mtw = (narrow && mtc == 1) ? 1 : MT_W;
           for (int ch = 0; ch < P.nchunk; ch++) {
             const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0), n0 = nt0 * 8;
-            const int njm = (ntc > noff) ? (ntc - noff + 3) / 4 : 0;
+            const int njm = (ntc > noff) ? (ntc - noff + nstride - 1) / nstride : 0;
             const bool active = (mh * MT_W < mtc) && njm > 0;
             double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
 #pragma unroll
@@ -681,7 +688,16 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
               if (active) {
                 const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + g) * KC;
                 const c128 *sBw = sMain + s * P.main_units + TM * KC + 8 * noff + g;
-                if (njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                if (narrow) {
+                  if (mtw == 1 && njm == 3) main_compute<3, 8, 1>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  else if (mtw == 1 && njm == 2) main_compute<2, 8, 1>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  else if (mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  else if (njm == 4) main_compute<4, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  else if (njm == 3) main_compute<3, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  else if (njm == 2) main_compute<2, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  else main_compute<1, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                }
+                else if (njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
                 else if (njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
                 else if (njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
                 else if (njm == 4) main_compute<4>(sAw, sBw, P.ldb, accr, acci, c, sw);
@@ -702,7 +718,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
                 if (jn < njm && Ql < tm_rows) {
 #pragma unroll
                   for (int e = 0; e < 2; e++) {
-                    const int n = n0 + 8 * (noff + 4 * jn) + 2 * c + e;
+                    const int n = n0 + 8 * (noff + nstride * jn) + 2 * c + e;
                     if (n < n2) {
                       const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
                       U[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
