@@ -170,7 +170,8 @@ class ClockSampler:
 
 # dram traffic per launch of the dominant kernel from the committed ncu capture (profiles/), keyed by config; None = not captured
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu captures summarised in profiles/ (key: config, stage)
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {("cfg2", 0): 4802780972032 + 1769176705024,      # profiles/r01_dram_cfg2.csv, s1::p0_kernel<7>
+                     ("cfg2", 2): 5304567847168 + 1975679740672}      # s3w::sigma_ws_kernel
 
 
 def run_ours(args):
@@ -249,6 +250,7 @@ def run_ours(args):
         total_ms, stage_ms = float(tt[0]), [float(x) for x in tt[1:]]
     ms_per_step = total_ms / args.steps
     info_host = info.cpu().tolist()
+    Sig_dev_check = Sigma.cpu()          # result of the literal device-resident run (the e2e leg must reproduce it bit for bit)
 
     # ---- the same iteration in the documented time-reversal mode (gw.h GW_SYM_TR): reported beside, never as `value` ----
     tr_mode = None
@@ -287,7 +289,6 @@ def run_ours(args):
         hTw = torch.from_numpy(p.T_wt).pin_memory(); hTt = torch.from_numpy(p.T_tw).pin_memory()
         hS = torch.empty(G.shape, dtype=torch.complex128, pin_memory=True)
         hK = torch.empty(gamma.shape, dtype=torch.complex128, pin_memory=True)
-        Sig_dev_check = Sigma.cpu()
         del P, Sigma, K, prob, G, gamma
         p.V = None
         torch.cuda.empty_cache()
