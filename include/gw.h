@@ -68,7 +68,8 @@ typedef struct {
 /* gw_problem.symmetry flag.  Time reversal: G[t][−k] = conj(G[t][k]) and V[−k1][−k2] = conj(V[k1][k2]) element-wise (the same
  * property that makes I − P̃0(iΩ) Hermitian for the Cholesky solve; the paper exploits k ↔ −k too).  Then
  * P̃0^q(β−τ) = P̃0^q(τ) and Σ^{−k}(τ) = conj Σ^{k}(τ), and the library evaluates only the irreducible half and copies the rest:
- *   gw_polarization : tau nodes t <= ntau-1-t are computed, P0t[ntau-1-t] is a copy of P0t[t];
+ *   gw_polarization : tau nodes t <= ntau-1-t are computed, P0t[ntau-1-t] is a copy of P0t[t]; for the full q range and
+ *                     nk <= 128 also only q <= −q, and P0t[t][−q] = transpose(P0t[t][q])  (216 -> 112 q points);
  *   gw_selfenergy   : k <= −k are computed, Sigma[t][−k] = conj(Sigma[t][k])  (only for the full q range and nk <= 128);
  * the other calls ignore the flag.  Computed elements are bit-identical to the literal evaluation.  If the inputs do not
  * have the symmetry the copied elements are wrong — nothing checks it. */

@@ -43,6 +43,9 @@ struct Params {
   int cs;                // CTAs per cluster = column splits of the panel
   int nqt, nitems;       // Q tiles per (t,q); total work items
   int nteff;             // tau nodes evaluated: ntau, or ceil(ntau/2) under GW_SYM_TR (the rest is mirrored)
+  int nqeff;             // q points evaluated: nq, or the q <= -q half under GW_SYM_TR (P0[-q] = P0[q]^T is copied)
+  short qirr[128];       // the evaluated q points when nqeff < nq
+  __device__ __forceinline__ int qof(int i) const { return nqeff < d.nq ? (int)qirr[i] : i; }
   int ldp, ksp, ndt;     // pass smem row stride (complex), k-steps = ceil(nao/4), n-tiles over nao
   int nt, ntc;           // n-tiles over naux; n-tiles per CTA
   int main_units, pass_units;   // complex elements per main / pass stage buffer
@@ -157,10 +160,11 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
 // bandwidth-hungry ragged panels are spread over the whole run), then t, then q slowest (concurrent clusters share the V
 // blocks of one q in L2)
 struct Item { int t, ql, Q0, tm_rows; };
-__device__ __forceinline__ Item decode_item(const GwDims &d, int nteff, int nqt, int item) {
+__device__ __forceinline__ Item decode_item(const Params &P, int item) {
+  const GwDims &d = P.d;
   Item it;
-  const int qt = item % nqt, r = item / nqt;
-  it.t = r % nteff; it.ql = r / nteff; it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
+  const int qt = item % P.nqt, r = item / P.nqt;
+  it.t = r % P.nteff; it.ql = P.qof(r / P.nteff); it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
   return it;
 }
 
@@ -216,7 +220,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       const int brows = 8 * ntc_mine;
       const uint64_t polA = policy_evict_first(), polB = policy_evict_last();
       for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(d, P.nteff, P.nqt, item);
+        const Item it = decode_item(P, item);
         const int q = d.q0 + it.ql;
         for (int k = 0; k < d.nk; k++, kit++) {
           const int kq = gw_kadd(d, k, q);
@@ -237,7 +241,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
       unsigned kit = 0, ph = 0;
       for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(d, P.nteff, P.nqt, item);
+        const Item it = decode_item(P, item);
         const int q = d.q0 + it.ql;
         const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
         for (int k = 0; k < d.nk; k++, kit++) {
@@ -279,7 +283,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
     unsigned kit = 0, ph = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
-      const Item it = decode_item(d, P.nteff, P.nqt, item);
+      const Item it = decode_item(P, item);
       const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
       for (int k = 0; k < d.nk; k++, kit++) {
         c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
@@ -322,7 +326,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned kit = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
-      const Item it = decode_item(d, P.nteff, P.nqt, item);
+      const Item it = decode_item(P, item);
       const int mtc = (it.tm_rows + 7) / 8;
       // tile ownership.  Full panels: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile.  Ragged last panel
       // (<= 16 rows): all eight warps share m-tiles 0 (and 1), every 8th n-tile each, so the panel costs time in proportion
@@ -381,10 +385,15 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
       // ---- epilogue: scale by -(s/N_k), store this CTA's columns of the panel ----
       const double pref = -(double)d.s / (double)d.nk;
       // under GW_SYM_TR the mirrored tau node receives a copy: P0^q(beta - tau) = P0^q(tau)
+      // and (full q range) the partner q receives the transpose: P0^{-q}_{Q'Q}(tau) = P0^{q}_{QQ'}(beta - tau) = P0^{q}_{QQ'}(tau)
       const int tbar = d.ntau - 1 - it.t;
-      const int ncopy = (P.nteff < d.ntau && tbar != it.t) ? 2 : 1;
-      for (int cp = 0; cp < ncopy; cp++) {
-        c128 *out = P.P0t + ((size_t)(cp ? tbar : it.t) * d.nq + it.ql) * naux * naux + col0;
+      const int nct = (P.nteff < d.ntau && tbar != it.t) ? 2 : 1;
+      const int qn = (P.nqeff < d.nq) ? gw_ksub(d, 0, it.ql) : it.ql;
+      const int ncq = (qn != it.ql) ? 2 : 1;
+      for (int cp = 0; cp < nct * ncq; cp++) {
+        const int tt = (cp & 1) && nct == 2 ? tbar : it.t;
+        const bool tr = cp >= nct;
+        c128 *out = P.P0t + ((size_t)tt * d.nq + (tr ? qn : it.ql)) * naux * naux;
 #pragma unroll
         for (int i = 0; i < MT_W; i++) {
           const int Q = it.Q0 + 8 * (mh * MT_W + i) + g;
@@ -392,8 +401,15 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
           for (int jn = 0; jn < NJ; jn++) {
             if (jn < njm && Q < naux) {
               const int col = 8 * (noff + nstride * jn) + 2 * c;
-              if (col < ncols) out[(size_t)Q * naux + col] = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
-              if (col + 1 < ncols) out[(size_t)Q * naux + col + 1] = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
+              const c128 v0 = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
+              const c128 v1 = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
+              if (!tr) {
+                if (col < ncols) out[(size_t)Q * naux + col0 + col] = v0;
+                if (col + 1 < ncols) out[(size_t)Q * naux + col0 + col + 1] = v1;
+              } else {
+                if (col < ncols) out[(size_t)(col0 + col) * naux + Q] = v0;
+                if (col + 1 < ncols) out[(size_t)(col0 + col + 1) * naux + Q] = v1;
+              }
             }
           }
         }
@@ -404,8 +420,16 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
   if (cs > 1) gwp::cluster_sync_all();
 }
 
+// GW_SYM_TR: the q <= -q half of the mesh (only for the full q range and nk <= 128)
+static int fill_qirr(const GwDims &d, short *qirr) {
+  if (!(d.sym & GW_SYM_TR) || d.nk > 128 || d.q0 != 0 || d.nq != d.nk) return d.nq;
+  int n = 0;
+  for (int q = 0; q < d.nk; q++) if (q <= gw_ksub(d, 0, q)) qirr[n++] = (short)q;
+  return n;
+}
+
 struct Plan {
-  int cs, ksp_max, nqt, nitems, nteff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
+  int cs, ksp_max, nqt, nitems, nteff, nqeff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
   size_t smem, slab_units, work_bytes;
   bool ok;
 };
@@ -424,7 +448,8 @@ static Plan make_plan(const gw_problem *p) {
   pl.ldp = r4;
   pl.nqt = (d.naux + TM - 1) / TM;
   pl.nteff = (d.sym & GW_SYM_TR) ? (d.ntau + 1) / 2 : d.ntau;
-  pl.nitems = pl.nqt * pl.nteff * d.nq;
+  { short tmp[128]; pl.nqeff = fill_qirr(d, tmp); }
+  pl.nitems = pl.nqt * pl.nteff * pl.nqeff;
   pl.main_units = (TM + 8 * pl.ntc) * KC;
   pl.prows = 32;
   pl.pass_units = pl.prows * pl.ldp;
@@ -479,7 +504,7 @@ double gw_stage1_flops(const gw_problem *p) {
     const double mainv = mtiles * pl.nt * (s1::KC / 4) * nmain;
     tiles += pass + mainv;
   }
-  return tiles * (double)d.nk * pl.nteff * d.nq * 2048.0;
+  return tiles * (double)d.nk * pl.nteff * pl.nqeff * 2048.0;
 }
 
 template <int KSP_MAX>
@@ -514,7 +539,7 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   s1::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
+  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
   P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
