@@ -63,3 +63,28 @@ def make_grids(ntau, nw, beta):
         raise RuntimeError(f"ill-conditioned sampling set: cond={cond:.3e}")
     return {"tau": tau, "nbos": S, "T_wt": np.ascontiguousarray(T_wt.astype(np.complex128)),
             "T_tw": np.ascontiguousarray(T_tw.astype(np.complex128)), "cond": cond}
+
+
+def make_fermionic_transform(ntau, beta, nw=None):
+    """tau -> i omega_n matrix for FERMIONIC functions on the same Chebyshev-Gauss tau nodes (Eq. 13, PAPER.md:110-116:
+    G(i omega_n) = int_0^beta G(tau) e^{i omega_n tau} dtau, omega_n = (2n+1) pi / beta): an *input* of gw_transform, the
+    next step of the workflow after the hot path (Sigma(tau) -> Sigma(i omega_n), Fig. 4 / PAPER.md:320).
+
+    All N Chebyshev polynomials are used (fermionic functions have no tau <-> beta - tau symmetry):
+      T_f = I_f . C,  C[j][t] = (2 - delta_j0)/N T_j(x_t),  I_f[n][j] = (beta/2) int_-1^1 T_j(x) e^{i omega_n beta (1+x)/2} dx
+    (Gauss-Legendre).  Returns dict(nfer[nw], T_wt_f[nw][ntau] complex128)."""
+    N = ntau
+    nw = N if nw is None else nw
+    S = bosonic_set(N)[:nw]                       # the same index pattern, read as fermionic indices n >= 0
+    t = np.arange(N)
+    x = -np.cos(np.pi * (2 * t + 1) / (2 * N))
+    j = np.arange(N)
+    Tt = np.cos(np.outer(j, np.arccos(x)))
+    C = Tt * (2.0 / N)
+    C[0] *= 0.5
+    M = 2 * N + 2 * int(S.max()) + 300
+    xg, wg = np.polynomial.legendre.leggauss(M)
+    Tg = np.cos(np.outer(j, np.arccos(xg)))
+    om = (2 * S + 1) * np.pi / beta
+    If = np.array([(beta / 2) * (Tg * (wg * np.exp(1j * w * beta * (1.0 + xg) / 2))).sum(1) for w in om])
+    return {"nfer": S, "omega": om, "T_wt_f": np.ascontiguousarray((If @ C).astype(np.complex128))}

@@ -97,6 +97,13 @@ int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt
  *   an entry whose factorisation failed (see info) is unspecified. */
 int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, double *phi, void *stream);
 
+/* Generic imaginary-axis grid transform — the kernel of Eq. 28a / Eq. 30 exposed for the next workflow step, the fermionic
+ * τ→iω_n transform of Σ̃ (Eq. 13; Fig. 4 step after the hot path):
+ *   Y[o][m] = Σ_i T[o][i] X[i][m],   o < n_out, i < n_in, m < len      (complex T; n_out, n_in <= 128)
+ *   T : device [n_out][n_in];  X : device [n_in][len];  Y : device [n_out][len], may alias X (each column block is read
+ *   completely before it is written).  Returns GW_EINVAL / GW_ESHAPE / GW_EARCH or a launch error. */
+int gw_transform(int32_t n_out, int32_t n_in, const gw_c128 *T, const gw_c128 *X, gw_c128 *Y, size_t len, void *stream);
+
 /* Stage 3 — Eq. 31, Algorithm 1 second k loop:
  *   Sigma[t][k][i][j] = -(1/N_k) Σ_{q in shard} Σ_QQ' Σ_ab V[k][k-q][Q][i][a] G[t][k-q][a][b] Wt[t][q-q_begin][Q][Q'] V[k-q][k][Q'][b][j]
  *   G     : device [ntau][nk][nao][nao]    in

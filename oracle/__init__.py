@@ -113,6 +113,18 @@ def dyson(P):
     return X
 
 
+def transform(T, X):
+    """Eq. 13 / 28a / 30 as a plain matrix application along the leading axis: Y[o][...] = sum_i T[o][i] X[i][...]."""
+    T = np.ascontiguousarray(T, dtype=np.complex128); X = np.ascontiguousarray(X, dtype=np.complex128)
+    n_out, n_in = T.shape
+    assert X.shape[0] == n_in
+    ln = int(np.prod(X.shape[1:]))
+    Y = np.empty((n_out,) + X.shape[1:], np.complex128)
+    lib().gwref_transform(ctypes.c_int(n_out), ctypes.c_int(n_in), _p(T), _p(X), ctypes.c_size_t(ln), _p(Y), ctypes.c_size_t(ln),
+                          ctypes.c_size_t(ln))
+    return Y
+
+
 def phi(P):
     """Summand of Eq. 37 for one matrix: tr{ln[I - P] + P}."""
     n = P.shape[0]

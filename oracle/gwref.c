@@ -38,7 +38,8 @@
  *
  * Parity pins: tests/test_oracle_pins.py (closed form P1, Lindhard P2, invariants P3-P5,
  * brute-force Matsubara sum P6, trace identity P7, solve residual P8, exchange limit P9,
- * literal 4-index evaluation P10, scalar form / series / eigenvalue route of the Eq. 37 summand P11).
+ * literal 4-index evaluation P10, scalar form / series / eigenvalue route of the Eq. 37 summand P11, fermionic
+ * transform of a single pole P12).
  * Nothing here is "parity unpinned".
  */
 #include <complex.h>

@@ -44,6 +44,7 @@ def lib():
         L.gw_screened_interaction.argtypes = [P, vp, vp, vp, vp]
         L.gw_screened_interaction_phi.argtypes = [P, vp, vp, vp, vp, vp]
         L.gw_selfenergy.argtypes = [P, vp, vp, vp, vp]
+        L.gw_transform.argtypes = [ctypes.c_int32, ctypes.c_int32, vp, vp, vp, ctypes.c_size_t, vp]
         L.gw_exchange.argtypes = [P, vp, vp, vp]
         L.gw_workspace_bytes.argtypes = [P]
         L.gw_workspace_bytes.restype = sz
@@ -53,7 +54,7 @@ def lib():
         L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
-        for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_selfenergy", "gw_exchange",
+        for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_version"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
@@ -172,6 +173,23 @@ def gw_screened_interaction_phi(prob, P0t, Wt=None, info=None, phi=None, stream=
                                              ctypes.c_void_p(info.data_ptr()), ctypes.c_void_p(phi.data_ptr()),
                                              _stream(stream)), "gw_screened_interaction_phi")
     return Wt, info, phi
+
+
+def gw_transform(T, X, Y=None, stream=None):
+    """Y[o][...] = sum_i T[o][i] X[i][...] along the leading axis (Eq. 13 / 28a / 30); Y may be X when the shapes agree."""
+    if T.dtype != torch.complex128 or X.dtype != torch.complex128 or not T.is_cuda or not X.is_cuda:
+        raise GWError("gw_transform: need CUDA complex128 tensors")
+    if not T.is_contiguous() or not X.is_contiguous() or T.dim() != 2 or X.shape[0] != T.shape[1]:
+        raise GWError("gw_transform: need contiguous T [n_out][n_in] and X [n_in][...]")
+    n_out, n_in = int(T.shape[0]), int(T.shape[1])
+    if Y is None:
+        Y = torch.empty((n_out,) + tuple(X.shape[1:]), dtype=torch.complex128, device=X.device)
+    if tuple(Y.shape) != (n_out,) + tuple(X.shape[1:]) or not Y.is_contiguous() or Y.dtype != torch.complex128:
+        raise GWError("gw_transform: Y must be contiguous complex128 of shape (n_out,) + X.shape[1:]")
+    ln = X.numel() // n_in
+    _check(lib().gw_transform(n_out, n_in, ctypes.c_void_p(T.data_ptr()), ctypes.c_void_p(X.data_ptr()),
+                              ctypes.c_void_p(Y.data_ptr()), ctypes.c_size_t(ln), _stream(stream)), "gw_transform")
+    return Y
 
 
 def gw_selfenergy(prob, G, Wt, Sigma=None, stream=None):

@@ -68,6 +68,12 @@ extern "C" int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P
   return gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, phi, (cudaStream_t)stream);
 }
 
+extern "C" int gw_transform(int32_t n_out, int32_t n_in, const gw_c128 *T, const gw_c128 *X, gw_c128 *Y, size_t len, void *stream) {
+  if (!aligned16(T) || !aligned16(X) || !aligned16(Y) || n_out <= 0 || n_in <= 0) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  return gw_launch_transform(n_out, n_in, (const c128 *)T, (const c128 *)X, (c128 *)Y, len, (cudaStream_t)stream);
+}
+
 extern "C" int gw_selfenergy(const gw_problem *p, const gw_c128 *G, const gw_c128 *Wt, gw_c128 *Sigma, void *stream) {
   int rc = check_problem(p, false); if (rc) return rc;
   if (!aligned16(G) || !aligned16(Wt) || !aligned16(Sigma)) return GW_EINVAL;

@@ -70,6 +70,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // kernel launchers implemented per stage
 int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t st);
 int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *info, double *phi, cudaStream_t st);
+int gw_launch_transform(int n_out, int n_in, const c128 *T, const c128 *X, c128 *Y, size_t len, cudaStream_t st);
 int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st);
 int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st);
 size_t gw_stage1_workspace(const gw_problem *p);

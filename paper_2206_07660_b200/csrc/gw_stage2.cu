@@ -343,3 +343,17 @@ int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *in
   s2::transform_kernel<<<pl.grid_t, s2::NTHR, pl.smem_t, st>>>(d.ntau, d.nw, (const c128 *)p->T_tw, Wt, Wt, len, pl.nblocks);
   return (int)cudaGetLastError();
 }
+
+int gw_launch_transform(int n_out, int n_in, const c128 *T, const c128 *X, c128 *Y, size_t len, cudaStream_t st) {
+  if (n_out <= 0 || n_in <= 0 || n_out > 128 || n_in > 128) return GW_ESHAPE;
+  const int nsm = gwp::gw_num_sms();
+  const size_t nb = (len + s2::NC - 1) / s2::NC;
+  if (nb == 0) return GW_OK;
+  if (nb > 0x7fffffffu) return GW_ESHAPE;
+  const int grid = nb < (size_t)nsm ? (int)nb : nsm;
+  const size_t smem = (size_t)((n_in + 3) / 4 * 4) * (s2::NC + 2) * sizeof(c128);
+  cudaError_t e = cudaFuncSetAttribute(s2::transform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return (int)e;
+  s2::transform_kernel<<<grid, s2::NTHR, smem, st>>>(n_out, n_in, T, X, Y, len, (int)nb);
+  return (int)cudaGetLastError();
+}

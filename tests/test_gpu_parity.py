@@ -262,3 +262,28 @@ def test_time_reversal_mode_parity(problems, oracle_results, oracle_lib, name):
     assert f_tr[0] < 0.76 * f_li[0] and f_tr[2] <= f_li[2]
     if (p.mesh.neg() != np.arange(cfg.nk)).any():     # some q != -q: tau half x q half (self-conjugate q stay)
         assert f_tr[0] < 0.45 * f_li[0]
+
+
+def test_transform_parity(problems, oracle_results, oracle_lib):
+    """gw_transform (generic grid transform; here the fermionic tau -> i omega_n transform of Sigma, Eq. 13) against the oracle:
+    a complex transform matrix, non-square shapes, ragged column counts and the in-place call."""
+    import gwgen
+    import paper_2206_07660_b200 as gw
+    p = problems("R"); cfg = p.cfg
+    Sg = oracle_results("R")["Sigma"]
+    f = gwgen.make_fermionic_transform(cfg.ntau, cfg.beta)
+    T = f["T_wt_f"]
+    want = oracle_lib.transform(T, Sg)
+    got = gw.gw_transform(torch.from_numpy(T).cuda(), torch.from_numpy(Sg).cuda())
+    assert relerr(got.cpu().numpy(), want) <= TOL
+    X = torch.from_numpy(Sg).cuda().clone()
+    gw.gw_transform(torch.from_numpy(T).cuda(), X, X)                     # in place (square)
+    assert relerr(X.cpu().numpy(), want) <= TOL
+    rng = np.random.default_rng(3)
+    for n_out, n_in, ln in ((5, 18, 77), (18, 7, 1), (128, 128, 130)):
+        Tr = rng.normal(size=(n_out, n_in)) + 1j * rng.normal(size=(n_out, n_in))
+        Xr = rng.normal(size=(n_in, ln)) + 1j * rng.normal(size=(n_in, ln))
+        g2 = gw.gw_transform(torch.from_numpy(Tr).cuda(), torch.from_numpy(Xr).cuda())
+        assert relerr(g2.cpu().numpy(), oracle_lib.transform(Tr, Xr)) <= TOL
+    with pytest.raises(gw.GWError):
+        gw.gw_transform(torch.zeros((129, 4), dtype=torch.complex128, device="cuda"), torch.zeros((4, 8), dtype=torch.complex128, device="cuda"))

@@ -328,3 +328,19 @@ def test_P11_phi_matches_eigenvalues(problems, oracle_results, oracle_lib):
             got = oracle_lib.phi(P)
             assert abs(got - ref) <= 1e-12 * max(1.0, abs(ref))
             assert got <= 1e-14 and got >= -0.5 * np.sum(lam ** 2) - 1e-12     # ln(1-x)+x in [-x²/2, 0] for x <= 0
+
+
+# ---- P12: fermionic tau -> i omega_n transform (Eq. 13), the step after the hot path ----
+def test_P12_fermionic_transform_closed_form(oracle_lib):
+    """G(tau) = -e^{-eps tau}/(1+e^{-beta eps}) transforms to 1/(i omega_n - eps): pins the generator's fermionic matrix and the
+    oracle's transform routine (sign of the exponent, omega_n = (2n+1) pi / beta, the beta/2 Jacobian) against a closed form."""
+    import gwgen
+    beta, N = 10.0, 32
+    g = gwgen.make_grids(N, N, beta)
+    f = gwgen.make_fermionic_transform(N, beta)
+    eps = np.array([0.7, -0.3, 0.05])
+    G = (-np.exp(-np.outer(g["tau"], eps)) / (1.0 + np.exp(-beta * eps))).astype(np.complex128)    # [ntau][3]
+    got = oracle_lib.transform(f["T_wt_f"], G)
+    ref = 1.0 / (1j * f["omega"][:, None] - eps[None, :])
+    assert np.max(np.abs(got - ref) / np.abs(ref)) < 1e-9
+    assert np.allclose(got, np.tensordot(f["T_wt_f"], G, axes=(1, 0)), rtol=1e-13, atol=0)
