@@ -162,9 +162,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
     // =============================== consumer warps ===============================
     gwp::reg_inc<232>();
     const int g = lane >> 2, c = lane & 3;
-    const int mh = w >> 2;                              // m-half: m-tiles 2*mh, 2*mh+1
     const int sw = (g & 1) << 2;
-    const int noff = ((w & 3) - mh + 4) & 3;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
       const int t = item % d.ntau, k = P.kof(item / d.ntau);
       double sgr[NCT][2], sgi[NCT][2];
@@ -174,11 +172,17 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
         gwp::mbar_wait(bar_g, gpar); gpar ^= 1u;
         for (int qt = 0; qt < P.nqt; qt++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
+          // tile ownership: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile; the ragged last panel
+          // (<= 16 rows) is shared by all eight warps (m-tiles 0, 1, every 8th n-tile each)
+          const bool narrow = mtc <= 2;
+          const int mh = narrow ? 0 : (w >> 2);
+          const int noff = narrow ? w : (((w & 3) - mh + 4) & 3);
+          const int nstride = narrow ? 8 : 4;
           // ---- main GEMM, N chunk by N chunk; U^T written to slabU as [(Q,j)][b] ----
           for (int ch = 0; ch < P.nchunk; ch++) {
             const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
             const int n0 = nt0 * 8;
-            const int njm = (ntc > noff) ? (ntc - noff + 3) / 4 : 0;
+            const int njm = (ntc > noff) ? (ntc - noff + nstride - 1) / nstride : 0;
             const bool active = (mh * MT_W < mtc) && njm > 0;
             double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
 #pragma unroll
@@ -190,9 +194,9 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
               if (active) {
                 const c128 *sAw = sStage + s * P.stage_units + (8 * mh * MT_W + g) * KC;
                 const c128 *sBw = sStage + s * P.stage_units + TM * KC + 8 * noff + g;
-                if (njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                if (!narrow && njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (!narrow && njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (!narrow && njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
                 else {
 #pragma unroll
                   for (int ks = 0; ks < KC / 4; ks++) {
@@ -204,7 +208,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
 #pragma unroll
                     for (int jn = 0; jn < NJ; jn++) {
                       if (jn < njm) {
-                        const c128 b = brow[32 * jn];
+                        const c128 b = brow[8 * nstride * jn];
 #pragma unroll
                         for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
                       }
@@ -223,7 +227,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
                 if (jn < njm && Ql < tm_rows) {
 #pragma unroll
                   for (int e = 0; e < 2; e++) {
-                    const int n = n0 + 8 * (noff + 4 * jn) + 2 * c + e;
+                    const int n = n0 + 8 * (noff + nstride * jn) + 2 * c + e;
                     if (n < n2) {
                       const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
                       slabU[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
@@ -327,7 +331,7 @@ double gw_stage3_flops(const gw_problem *p) {
   for (int qt = 0; qt < pl.nqt; qt++) {
     const int tm_rows = (d.naux - qt * s3::TM) < s3::TM ? (d.naux - qt * s3::TM) : s3::TM;
     const int mtc = (tm_rows + 7) / 8;
-    const double mtiles = (((d.nao + 3) / 4 == 7) /* s3w kernel: narrow ragged panel */ && mtc <= 2) ? (double)mtc : (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
+    const double mtiles = (mtc <= 2) ? (((d.nao + 3) / 4 == 7) ? (double)mtc : 2.0) /* ragged panel shared by all warps; s3 always runs 2 m-tiles */ : (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
     tiles += mtiles * pl.nnt * (s3::KC / 4) * nmain;                         // main
     tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.ndt * pl.ksp;           // pass A
     tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.kspf * pl.kh;             // final
