@@ -53,6 +53,9 @@ CONFIGS = {
     "R": GWConfig("cfgR", (3, 2, 2), 7, 37, 18, 18, 30.0, -1.5, 2.0, 0.04, BASE_SEED + 98),
     # small problem with the production basis size (nao=26: the straight-line / warp-specialised kernel variants), ragged naux
     "S": GWConfig("cfgS", (2, 1, 2), 26, 44, 8, 8, 40.0, -2.0, 3.0, 0.04, BASE_SEED + 94),
+    # odd sizes inside the compile-time k-step classes (nao = 25..28 -> 7 steps, 49..52 -> 13 steps), naux = one panel + 1 row
+    "U": GWConfig("cfgU", (1, 2, 1), 27, 33, 6, 6, 20.0, -2.0, 3.0, 0.04, BASE_SEED + 93),
+    "W": GWConfig("cfgW", (2, 1, 1), 49, 17, 6, 6, 20.0, -2.0, 3.0, 0.04, BASE_SEED + 92),
     # config-4-shaped problem with a short tau grid (same per-CTA behaviour, 15x less work)
     "Q": GWConfig("cfgQ", (4, 4, 4), 52, 400, 8, 8, 1000.0, -3.0, 5.0, 0.04, BASE_SEED + 95),
     # config-4-shaped basis (nao=52, naux > 224: the wide-panel / split-K kernel variants) at a size the oracle does in full

@@ -71,49 +71,11 @@ __device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG,
   }
 }
 
-// Straight-line version of pass_compute for ksp == KSP exactly (the production shapes: nao = 26 -> 7, nao = 52 -> 13):
-// the (n-tile, k-step) loop nest is flattened and fully unrolled, every B fragment is loaded PF steps (4*PF DMMAs)
-// before its use, and no branch separates the DMMAs.  Same sums in the same order as pass_compute.
-template <int KSP, bool TRANSPOSED>
-__device__ __forceinline__ void pass_compute_exact(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
-                                                   int nao, int ldp, int w = -1) {
-  constexpr int NDT = (KSP + 1) / 2, S = NDT * KSP, PF = 3, NB = PF + 1;
-  if (w < 0) w = threadIdx.x >> 5;          // m-tile of this warp within the job
-  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
-  if (row0 + 8 * w >= rows_total) return;   // whole m-tile beyond the panel (warp-uniform)
-  c128 a[KSP];
-  const c128 *ap = sStage + (8 * w + g) * ldp + c;
-#pragma unroll
-  for (int ks = 0; ks < KSP; ks++) a[ks] = ap[4 * ks];
-  const int row = row0 + 8 * w + g;
-  const bool rok = row < rows_total;
-  // this lane's two output columns of n-tile nt are o[nt * 8 * ostride] and o[(nt * 8 + 1) * ostride]
-  c128 *o;
-  int ostride;
-  if (TRANSPOSED) { const int Q = row / nao, x = row - Q * nao; o = out + ((size_t)Q * nao + 2 * c) * nao + x; ostride = nao; }
-  else { o = out + (size_t)row * nao + 2 * c; ostride = 1; }
-  const c128 *bp = sG + g * ldp + c;
-  c128 b[NB];
-#pragma unroll
-  for (int s = 0; s < PF && s < S; s++) b[s % NB] = bp[(s / KSP) * 8 * ldp + 4 * (s % KSP)];
-  double cr[2] = {0.0, 0.0}, ci[2] = {0.0, 0.0};
-#pragma unroll
-  for (int s = 0; s < S; s++) {
-    const int nt = s / KSP, ks = s % KSP;
-    if (s + PF < S) b[(s + PF) % NB] = bp[((s + PF) / KSP) * 8 * ldp + 4 * ((s + PF) % KSP)];
-    cmma(cr, ci, a[ks], b[s % NB]);
-    if (ks == KSP - 1) {
-      // only the last n-tile can reach beyond nao: 8*(NDT-1) <= 4*(KSP-1) < nao
-      if (rok && (nt < NDT - 1 || 8 * nt + 2 * c < nao)) o[0] = make_double2(cr[0], ci[0]);
-      if (rok && (nt < NDT - 1 || 8 * nt + 2 * c + 1 < nao)) o[ostride] = make_double2(cr[1], ci[1]);
-      o += 8 * ostride;
-      cr[0] = cr[1] = 0.0; ci[0] = ci[1] = 0.0;
-    }
-  }
-}
-
-// Multi-m-tile variant for dedicated pass warps: warp w owns the MT m-tiles 8*(MT*w + i) of a job; every B fragment is
-// loaded once and used by all MT tiles (2*MT independent accumulator chains).
+// pass_compute for ksp == KSP known at compile time (the production shapes: nao = 26 -> 7, nao = 52 -> 13): no branch between
+// the DMMAs of an n-tile, every B fragment loaded PF k-steps (4*PF DMMAs) before its use.  Same sums in the same order as
+// pass_compute.
+// Warp w owns the MT m-tiles 8*(MT*w + i) of a job; every B fragment is loaded once and used by all MT tiles
+// (2*MT independent accumulator chains).
 template <int KSP, bool TRANSPOSED, int MT>
 __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const c128 *sG, c128 *out, int row0, int rows_total,
                                                       int nao, int ldp, int w, FastDiv fd) {

@@ -22,7 +22,7 @@ def run_gpu(p, **kw):
     return {k: v.cpu().numpy() for k, v in out.items()}
 
 
-@pytest.mark.parametrize("name", ["0", "T", "R", "S", "L"])
+@pytest.mark.parametrize("name", ["0", "T", "R", "S", "U", "W", "L"])
 def test_full_parity_small(problems, oracle_results, name):
     p = problems(name)
     ref = oracle_results(name)
