@@ -44,26 +44,36 @@ struct Params {
   FastDiv fd_nao;
 };
 
-// main job (producer warpgroup): A = W[tm rows][k0..k0+8) swizzled; B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
+// main job (producer warpgroup): A = W[tm rows][k0..k0+8) swizzled by row parity (rows beyond tm_rows re-read the last valid
+// row: their products land in accumulators that are never stored); B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
+// (K rows beyond naux and columns beyond nao² zero filled).  One source pointer per column, constant row stride; the V block is
+// shared by the ~100 CTAs working on the same k (L2 evict-last hint).
 __device__ __forceinline__ void ws_issue_main(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
-                                              int n0, int ncols, int ldb, int k0) {
+                                              int n0, int ncols, int ldb, int k0, uint64_t polB) {
   const int pt = threadIdx.x - 32 * NCONS;
+  const unsigned sA = gwp::smem_u32(stage);
   {
     const int u = pt & 7, rsub = pt >> 3;
     const bool kok = k0 + u < naux;
-    for (int r = rsub; r < TM; r += 16) {
-      const bool ok = kok && (r < tm_rows);
-      gwp::cp_async16_zfill(stage + r * KC + (u ^ ((r & 1) << 2)), ok ? W + (size_t)r * naux + k0 + u : W, ok);
+    const int nb = kok ? 16 : 0;
+    const c128 *src = W + (kok ? k0 + u : 0);
+#pragma unroll
+    for (int r = rsub; r < TM; r += gwp::NPROD_THR / 8) {
+      const int rr = min(r, tm_rows - 1);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"((sA + 16u * (unsigned)(r * KC + u)) ^ ((unsigned)(r & 1) << 6)),
+                   "l"(src + (size_t)rr * naux), "r"(nb));
     }
   }
-  c128 *sB = stage + TM * KC;
+  const unsigned sB = sA + 16u * TM * KC;
+  for (int cc = pt; cc < ncols; cc += gwp::NPROD_THR) {
+    const bool cok = n0 + cc < n2;
+    const c128 *src = V2 + (size_t)k0 * n2 + (cok ? n0 + cc : 0);
+    const unsigned dst = sB + 16u * (unsigned)cc;
 #pragma unroll
-  for (int r = 0; r < KC; r++) {
-    const bool rok = k0 + r < naux;
-    const c128 *src = V2 + (size_t)(k0 + r) * n2 + n0;
-    for (int cc = pt; cc < ncols; cc += gwp::NPROD_THR) {
-      const bool ok = rok && (n0 + cc < n2);
-      gwp::cp_async16_zfill(sB + r * ldb + cc, ok ? src + cc : V2, ok);
+    for (int r = 0; r < KC; r++) {
+      const bool ok = cok && (k0 + r < naux);
+      asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst + 16u * (unsigned)(r * ldb)),
+                   "l"(ok ? src + (size_t)r * n2 : V2), "r"(ok ? 16 : 0), "l"(polB));
     }
   }
 }
@@ -118,6 +128,8 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
   if (w >= NCONS) {
     // =============================== producer warpgroup ===============================
     gwp::reg_dec<40>();
+    uint64_t polB;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(polB));
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
       const int t = item % d.ntau, k = P.kof(item / d.ntau);
       for (int ql = 0; ql < d.nq; ql++) {
@@ -134,7 +146,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
             const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
             for (int j = 0; j < nmain; j++) {
               const int s = ring.acquire();
-              ws_issue_main(sStage + s * P.stage_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC);
+              ws_issue_main(sStage + s * P.stage_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC, polB);
               ring.commit();
             }
           }
