@@ -17,9 +17,12 @@
 //                        pass 1:  Xt[Q][b][d] = Σ_a V[k][k+q][Q][d][a] G[t][k+q][a][b]      rows (Q,d) flat
 //                        pass 2:  Z [Q][b][c] = Σ_d Xt[Q][b][d] G[tbar][k][c][d]            rows (Q,b) flat; in place
 //                      (in a cluster each CTA transforms half of the panel rows)
-//   producer warps   : 12-14 feed the main ring, 15 feeds the pass ring and the G matrices
+//   producer warps   : one thread of warp 12 feeds the main ring with TMA (cp.async.bulk.tensor.2d, 128-byte swizzle: one box
+//                      of Z rows and one box of V[k+q][k] rows per job, completion by mbarrier expect-tx); warp 15 feeds the
+//                      pass ring and the G matrices with cp.async (26-wide rows need padded destinations)
 // Xt/Z live in two per-cluster slabs of the workspace (TM·nao² complex each, double buffered over k, written and
 // re-read within ~100 µs, i.e. L2 resident); they never exist as a [t][q][k] tensor.
+#include <cuda.h>
 #include "gw_pipe.cuh"
 
 namespace s1 {
@@ -49,6 +52,7 @@ struct Params {
   int ldp, ksp, ndt;     // pass smem row stride (complex), k-steps = ceil(nao/4), n-tiles over nao
   int nt, ntc;           // n-tiles over naux; n-tiles per CTA
   int main_units, pass_units;   // complex elements per main / pass stage buffer
+  int main_off;                 // offset of the main ring in the (1024-byte aligned) dynamic shared memory, complex elements
   int prows;                    // rows per pass job: 8 * (m-tiles per pass warp) * 4 pass warps
   int nstage, pstage, ng;       // ring depths; number of G buffers (2: G[t] and G[tbar] side by side, 1: time shared)
   size_t slab_units;     // complex elements per slab (two slabs per cluster)
@@ -76,45 +80,13 @@ __device__ __forceinline__ void cpa_hint(unsigned dst, const void *src, int nbyt
   asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst), "l"(src), "r"(nbytes), "l"(pol));
 }
 
-// main job: A = Z[TM rows][k0..k0+8), B = Vb[brows rows][k0..k0+8); 16-byte units swizzled by row parity.
-// Rows beyond the valid range re-read the last valid row (their products land in accumulators that are never stored);
-// only the K tail of the last job is zero filled.  Each thread owns one 16-byte unit column and walks the rows with
-// constant strides, so the loop body is one address add per copy.
-__device__ __forceinline__ void issue_main(c128 *stage, const c128 *Z, int tm_rows, const c128 *Vb, int ncols, int brows, int n2, int k0,
-                                           uint64_t polA, uint64_t polB) {
-  constexpr int RS = N_MPROD / 8;                      // rows per sweep of the producer threads
-  const int pt = threadIdx.x - T_MPROD;
-  const int u = pt & 7, rsub = pt >> 3;
-  const bool kok = k0 + u < n2;
-  const int nbytes = kok ? 16 : 0;
-  const int koff = kok ? k0 + u : 0;
-  const unsigned sbase = gwp::smem_u32(stage) + 16u * (unsigned)u;
-  {
-    const c128 *src = Z + koff;
-#pragma unroll
-    for (int r = rsub; r < TM; r += RS) {
-      const int rr = min(r, tm_rows - 1);
-      const unsigned dst = (sbase + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
-      cpa_hint(dst, src + (size_t)rr * n2, nbytes, polA);
-    }
-  }
-  const unsigned sB = sbase + 16u * TM * KC;
-  const c128 *src = Vb + koff;
-  const size_t step = (size_t)RS * n2;
-  int r = rsub;
-  const c128 *sp = src + (size_t)r * n2;
-  for (; r + 3 * RS < ncols; r += 4 * RS, sp += 4 * step) {      // rows r, r+RS, r+2RS, r+3RS all valid (RS is even: same row parity)
-    const unsigned dst = (sB + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
-    cpa_hint(dst, sp, nbytes, polB);
-    cpa_hint(dst + RS * 16u * KC, sp + step, nbytes, polB);
-    cpa_hint(dst + 2 * RS * 16u * KC, sp + 2 * step, nbytes, polB);
-    cpa_hint(dst + 3 * RS * 16u * KC, sp + 3 * step, nbytes, polB);
-  }
-  for (; r < brows; r += RS) {
-    const int rr = min(r, ncols - 1);
-    const unsigned dst = (sB + (unsigned)r * (16u * KC)) ^ ((unsigned)(r & 1) << 6);
-    cpa_hint(dst, src + (size_t)rr * n2, nbytes, polB);
-  }
+// ---- TMA (main ring) ----
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
+               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(gwp::smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(gwp::smem_u32(bar)), "r"(bytes) : "memory");
 }
 
 // rows [row0, row0+prows) of a dense (rows x nao) matrix -> stage[r][ldp]   (pass-ring producer warp)
@@ -169,15 +141,16 @@ __device__ __forceinline__ Item decode_item(const Params &P, int item) {
 }
 
 template <int KSP_MAX>
-__global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
+__global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmZ) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  c128 *smem = reinterpret_cast<c128 *>(smem_raw);
+  // the TMA destinations (128-byte swizzle) need 1024-byte alignment: the launch asks for 1 KB of slack
+  c128 *smem = reinterpret_cast<c128 *>(smem_raw + ((1024u - (gwp::smem_u32(smem_raw) & 1023u)) & 1023u));
   const GwDims d = P.d;
   const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, naop = 8 * P.ndt;
   c128 *sG0 = smem;                                       // pass 1: sG0[b][a] = G[t][k+q][a][b]
   c128 *sG1 = sG0 + (P.ng == 2 ? naop * ldp : 0);         // pass 2: sG1[c][d] = G[tbar][k][c][d]  (== sG0 when time shared)
   c128 *sPass = smem + P.ng * naop * ldp;                 // pstage x pass_units
-  c128 *sMain = sPass + P.pstage * P.pass_units;          // nstage x main_units
+  c128 *sMain = smem + P.main_off;                        // nstage x main_units (1024-byte aligned stages)
   __shared__ uint64_t bars[2 * NST_MAX + 2 * PST_MAX + 6];
   uint64_t *full_m = bars, *empty_m = bars + NST_MAX, *full_p = bars + 2 * NST_MAX, *empty_p = full_p + PST_MAX;
   uint64_t *bar_g = empty_p + PST_MAX, *bar_phase = bar_g + 1, *zready = bar_g + 2, *zfree = bar_g + 4;
@@ -196,10 +169,10 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
 
   // zero all dynamic smem once (pad rows/columns must hold finite values: they meet zero operands); init barriers
   {
-    const int tot = P.ng * naop * ldp + P.pstage * P.pass_units + P.nstage * P.main_units;
+    const int tot = P.main_off + P.nstage * P.main_units;
     for (int i = threadIdx.x; i < tot; i += NTHR1) smem[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
-      for (int i = 0; i < P.nstage; i++) { gwp::mbar_init(full_m + i, N_MPROD); gwp::mbar_init(empty_m + i, NMAINW); }
+      for (int i = 0; i < P.nstage; i++) { gwp::mbar_init(full_m + i, 1); gwp::mbar_init(empty_m + i, NMAINW); }
       for (int i = 0; i < P.pstage; i++) { gwp::mbar_init(full_p + i, N_PPROD); gwp::mbar_init(empty_p + i, NPASSW); }
       gwp::mbar_init(bar_g, N_PPROD);
       gwp::mbar_init(bar_phase, NPASSW);
@@ -214,28 +187,34 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     // ====================================== producer warpgroup ======================================
     gwp::reg_dec<REG_PROD>();
     if (w < 15) {
-      // ---- main-ring producer (96 threads): Z of the current k and the raw V[k+q][k] rows of this CTA's columns ----
-      Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
-      unsigned kit = 0;
-      const int brows = 8 * ntc_mine;
-      const uint64_t polA = policy_evict_first(), polB = policy_evict_last();
-      for (int item = cid; item < P.nitems; item += ncl) {
-        const Item it = decode_item(P, item);
-        const int q = d.q0 + it.ql;
-        for (int k = 0; k < d.nk; k++, kit++) {
-          const int kq = gw_kadd(d, k, q);
-          const c128 *Vb = P.V + ((size_t)kq * d.nk + k) * vb + (size_t)col0 * n2;
-          const c128 *Z = slab0 + (size_t)(kit & 1u) * P.slab_units;
-          if (cs > 1) gwp::mbar_wait_cluster(zready + (kit & 1u), (kit >> 1) & 1u);
-          else gwp::mbar_wait(zready + (kit & 1u), (kit >> 1) & 1u);
-          for (int j = 0; j < nmain; j++) {
-            const int s = rm.acquire();
-            issue_main(sMain + s * P.main_units, Z, it.tm_rows, Vb, ncols, brows, n2, j * KC, polA, polB);
-            rm.commit();
+      // ---- main-ring producer: ONE thread issues two TMA box loads per job (Z rows of the current k; raw V[k+q][k] rows of
+      //      this CTA's columns) and arms the stage's mbarrier with the byte count ----
+      if (w == NMAINW + NPASSW && lane == 0) {
+        Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
+        unsigned kit = 0;
+        const uint64_t polA = policy_evict_first(), polB = policy_evict_last();
+        const unsigned bytesA = TM * KC * 16u, bytesB = 8u * (unsigned)P.ntc * KC * 16u;
+        for (int item = cid; item < P.nitems; item += ncl) {
+          const Item it = decode_item(P, item);
+          const int q = d.q0 + it.ql;
+          for (int k = 0; k < d.nk; k++, kit++) {
+            const int kq = gw_kadd(d, k, q);
+            const int yB = (kq * d.nk + k) * naux + col0;              // row of V viewed as [nk*nk*naux][nao²]
+            const int yA = (cid * 2 + (int)(kit & 1u)) * TM;           // row of the slab area viewed as [2*nclusters*TM][nao²]
+            if (cs > 1) gwp::mbar_wait_cluster(zready + (kit & 1u), (kit >> 1) & 1u);
+            else gwp::mbar_wait(zready + (kit & 1u), (kit >> 1) & 1u);
+            asm volatile("fence.proxy.async.global;\n" ::: "memory");   // Z was written through the generic proxy
+            for (int j = 0; j < nmain; j++) {
+              const int s = rm.acquire();
+              const unsigned dst = gwp::smem_u32(sMain + s * P.main_units);
+              mbar_expect_tx(full_m + s, bytesA + bytesB);
+              tma_load_2d(dst, &tmZ, 2 * KC * j, yA, full_m + s, polA);
+              tma_load_2d(dst + bytesA, &tmV, 2 * KC * j, yB, full_m + s, polB);
+              rm.advance();
+            }
           }
         }
       }
-      asm volatile("cp.async.wait_all;\n" ::: "memory");
     } else {
       // ---- pass-ring producer (32 threads): G matrices, V[k][k+q] rows (pass 1), Xt rows from the slab (pass 2) ----
       Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
@@ -322,7 +301,11 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
     // ========================================= main warps =========================================
     gwp::reg_inc<REG_MAIN>();
     const int g = lane >> 2, c = lane & 3;
-    const int sw = (g & 1) << 2;
+    // TMA 128-byte swizzle: 16-byte unit u of row r sits at u ^ (r & 7).  Fragment lane group g reads matrix row rho(g) of its
+    // 8-row tile, so that the two rows of a quarter-warp differ in bit 2 (conflict-free); the accumulator rows / columns are
+    // permuted accordingly in the epilogue.
+    const int rho = (g >> 1) + 4 * (g & 1);
+    const int sw = rho;
     Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned kit = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
@@ -348,8 +331,8 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
         for (int j = 0; j < nmain; j++) {
           const int s = rm.wait();
           if (active) {
-            const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + g) * KC;
-            const c128 *sBw = sMain + s * P.main_units + TM * KC + (8 * noff + g) * KC;
+            const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + rho) * KC;
+            const c128 *sBw = sMain + s * P.main_units + TM * KC + (8 * noff + rho) * KC;
             if (!narrow && njm == NJ) main_compute<NJ, 4, MT_W>(sAw, sBw, accr, acci, c, sw);
             else if (!narrow && njm == NJ - 1) main_compute<NJ - 1, 4, MT_W>(sAw, sBw, accr, acci, c, sw);
             else if (narrow && mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, accr, acci, c, sw);
@@ -396,19 +379,20 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P) {
         c128 *out = P.P0t + ((size_t)tt * d.nq + (tr ? qn : it.ql)) * naux * naux;
 #pragma unroll
         for (int i = 0; i < MT_W; i++) {
-          const int Q = it.Q0 + 8 * (mh * MT_W + i) + g;
+          const int Q = it.Q0 + 8 * (mh * MT_W + i) + rho;            // accumulator row g holds matrix row rho(g)
 #pragma unroll
           for (int jn = 0; jn < NJ; jn++) {
             if (jn < njm && Q < naux) {
-              const int col = 8 * (noff + nstride * jn) + 2 * c;
+              // accumulator columns 2c, 2c+1 hold matrix columns rho(2c) = c and rho(2c+1) = c + 4 of the n-tile
+              const int ca = 8 * (noff + nstride * jn) + c, cb = ca + 4;
               const c128 v0 = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
               const c128 v1 = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
               if (!tr) {
-                if (col < ncols) out[(size_t)Q * naux + col0 + col] = v0;
-                if (col + 1 < ncols) out[(size_t)Q * naux + col0 + col + 1] = v1;
+                if (ca < ncols) out[(size_t)Q * naux + col0 + ca] = v0;
+                if (cb < ncols) out[(size_t)Q * naux + col0 + cb] = v1;
               } else {
-                if (col < ncols) out[(size_t)(col0 + col) * naux + Q] = v0;
-                if (col + 1 < ncols) out[(size_t)(col0 + col + 1) * naux + Q] = v1;
+                if (ca < ncols) out[(size_t)(col0 + ca) * naux + Q] = v0;
+                if (cb < ncols) out[(size_t)(col0 + cb) * naux + Q] = v1;
               }
             }
           }
@@ -429,6 +413,7 @@ static int fill_qirr(const GwDims &d, short *qirr) {
 }
 
 struct Plan {
+  int main_off;
   int cs, ksp_max, nqt, nitems, nteff, nqeff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
   size_t smem, slab_units, work_bytes;
   bool ok;
@@ -455,14 +440,15 @@ static Plan make_plan(const gw_problem *p) {
   pl.pass_units = pl.prows * pl.ldp;
   // shared memory: prefer both G matrices resident and a 3-deep pass ring; shrink them while the main ring has < 4 stages
   const size_t gsz = (size_t)8 * pl.ndt * pl.ldp * sizeof(c128), psz = (size_t)pl.pass_units * sizeof(c128), msz = (size_t)pl.main_units * sizeof(c128);
-  const size_t cap = 226 * 1024;
+  const size_t cap = 225 * 1024;            // 1 KB of the 227 KB is alignment slack for the TMA destinations
   const int tryng[4] = {2, 2, 1, 1}, tryps[4] = {3, 2, 3, 2};
   for (int i = 0; i < 4; i++) {
     pl.ng = tryng[i]; pl.pstage = tryps[i];
-    const size_t fixed = pl.ng * gsz + pl.pstage * psz;
+    const size_t fixed = (pl.ng * gsz + pl.pstage * psz + 1023) / 1024 * 1024;      // main stages start 1024-byte aligned
+    pl.main_off = (int)(fixed / sizeof(c128));
     pl.nstage = fixed < cap ? (int)((cap - fixed) / msz) : 0;
     if (pl.nstage > 6) pl.nstage = 6;
-    pl.smem = fixed + (size_t)pl.nstage * msz;
+    pl.smem = fixed + (size_t)pl.nstage * msz + 1024;
     if (pl.nstage >= 4) break;
   }
   const int nsm = gwp::gw_num_sms();
@@ -507,10 +493,46 @@ double gw_stage1_flops(const gw_problem *p) {
   return tiles * (double)d.nk * pl.nteff * pl.nqeff * 2048.0;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
+      cudaGetLastError();
+      return nullptr;
+    }
+    fn = (EncodeTiledFn)ptr;
+  }
+  return fn;
+}
+// rows x (nao² complex = 2 nao² doubles) matrix, box = 8 complex x box_rows, 128-byte swizzle, zero fill outside
+static int make_rows_map(CUtensorMap *map, const void *base, size_t rows, int n2, int box_rows) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return (int)cudaErrorNotSupported;
+  const cuuint64_t gdim[2] = {(cuuint64_t)2 * n2, (cuuint64_t)rows};
+  const cuuint64_t gstr[1] = {(cuuint64_t)n2 * 16};
+  const cuuint32_t box[2] = {(cuuint32_t)(2 * s1::KC), (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
+}
+
 template <int KSP_MAX>
 static int launch_p0(const s1::Plan &pl, const s1::Params &P, cudaStream_t st) {
   cudaError_t e = cudaFuncSetAttribute(s1::p0_kernel<KSP_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
+  const int n2 = P.d.nao * P.d.nao;
+  CUtensorMap tmV, tmZ;
+  int rc = make_rows_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, n2, 8 * pl.ntc);
+  if (rc) return rc;
+  rc = make_rows_map(&tmZ, P.scratch, (size_t)gwp::gw_num_sms() * 2 * s1::TM, n2, s1::TM);
+  if (rc) return rc;
   cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof(cfg));
   cudaLaunchAttribute attr[1];
   cfg.blockDim = dim3(s1::NTHR1, 1, 1);
@@ -528,7 +550,7 @@ static int launch_p0(const s1::Plan &pl, const s1::Params &P, cudaStream_t st) {
     else cudaGetLastError();
   }
   cfg.gridDim = dim3(pl.cs * ncl, 1, 1);
-  e = cudaLaunchKernelEx(&cfg, s1::p0_kernel<KSP_MAX>, P);
+  e = cudaLaunchKernelEx(&cfg, s1::p0_kernel<KSP_MAX>, P, tmV, tmZ);
   return (int)e;
 }
 
@@ -540,7 +562,7 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
   P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
-  P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
+  P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.main_off = pl.main_off; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
   if (pl.ksp_max == 7) return launch_p0<7>(pl, P, st);
