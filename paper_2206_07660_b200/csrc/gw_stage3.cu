@@ -9,6 +9,7 @@
 // A persistent CTA owns one (t,k): it loops over q and over Q panels, and keeps the nao x nao Sigma accumulator in
 // registers for the whole item, so the q-sum needs no cross-CTA reduction and the result is deterministic.
 // U and T live in two per-CTA slabs of the workspace (L2 resident); the raw V2 block is the only big stream.
+#include <cuda.h>
 #include "gw_pipe.cuh"
 
 // GW_SYM_TR bookkeeping shared by both stage-3 kernels: the k <= -k half of the mesh (only for the full q range, nk <= 128)
@@ -412,6 +413,7 @@ struct Params {
   int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
   int ldb;                // row stride of the main-job B part
   int main_units, aux_units, nstage, astage;
+  int main_off;           // offset of the main ring in the 1024-byte aligned dynamic shared memory (complex elements)
   size_t slab_units;      // complex elements per slab (three slabs per CTA: U0, U1, T)
   int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
   short kirr[128];        // the evaluated k points when nkeff < nk
@@ -440,53 +442,37 @@ __device__ __forceinline__ void cpa_hint(unsigned dst, const void *src, int nbyt
 }
 __device__ __forceinline__ uint64_t policy_evict_last() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p)); return p; }
 
-// main job: A = W[TM rows][k0..k0+8) swizzled by row parity (rows beyond tm_rows re-read the last valid row);
-// B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb] (K rows beyond naux and columns beyond nao² zero filled)
-__device__ __forceinline__ void issue_main(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
-                                           int n0, int ncols, int ldb, int k0, uint64_t polB) {
-  const int pt = threadIdx.x - T_MPROD;
-  const unsigned sA = gwp::smem_u32(stage);
-  {
-    const int u = pt & 7, rsub = pt >> 3;
-    const bool kok = k0 + u < naux;
-    const int nb = kok ? 16 : 0;
-    const c128 *src = W + (kok ? k0 + u : 0);
-#pragma unroll
-    for (int r = rsub; r < TM; r += N_MPROD / 8) {
-      const int rr = min(r, tm_rows - 1);
-      cpa((sA + 16u * (unsigned)(r * KC + u)) ^ ((unsigned)(r & 1) << 6), src + (size_t)rr * naux, nb);
-    }
-  }
-  const unsigned sB = sA + 16u * TM * KC;
-  for (int cc = pt; cc < ncols; cc += N_MPROD) {
-    const bool cok = n0 + cc < n2;
-    const c128 *src = V2 + (size_t)k0 * n2 + (cok ? n0 + cc : 0);
-    const unsigned dst = sB + 16u * (unsigned)cc;
-#pragma unroll
-    for (int r = 0; r < KC; r++) {
-      const bool ok = cok && (k0 + r < naux);
-      cpa_hint(dst + 16u * (unsigned)(r * ldb), ok ? src + (size_t)r * n2 : V2, ok ? 16 : 0, polB);
-    }
-  }
-}
-
+// main job in shared memory (both parts written by TMA with the 128-byte swizzle: 16-byte unit u of row r sits at u ^ (r & 7)):
+//   A = W[TM rows][8 K]                    32 rows x 128 B
+//   B = one 1 KB box per n-tile: [8 K rows][8 columns]
+// Lane group g reads row / column rho(g) = (g >> 1) + 4 (g & 1) of its tile, so a quarter-warp touches eight different units.
 template <int NJM, int NSTRIDE = 4, int MTW = MT_W>
-__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, int ldb, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
+__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int rho) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
-    const int u = (4 * ks + c) ^ sw;
+    const int kr = 4 * ks + c;
+    const int u = kr ^ rho;
     c128 a[MTW], b[NJM];
 #pragma unroll
     for (int i = 0; i < MTW; i++) a[i] = sAw[i * 8 * KC + u];
-    const c128 *brow = sBw + (4 * ks + c) * ldb;
+    const c128 *bk = sBw + kr * 8 + u;                  // row kr of the box, column rho swizzled by the row
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++) b[jn] = brow[8 * NSTRIDE * jn];
+    for (int jn = 0; jn < NJM; jn++) b[jn] = bk[64 * NSTRIDE * jn];
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++)
 #pragma unroll
       for (int i = 0; i < MTW; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
   }
 }
+
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
+               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(gwp::smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(gwp::smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_normal() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;\n" : "=l"(p)); return p; }
 
 // aux ring jobs (producer warp 15)
 __device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd) {
@@ -535,14 +521,15 @@ __device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[N
   }
 }
 
-__global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
+__global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmV) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  c128 *smem = reinterpret_cast<c128 *>(smem_raw);
+  // the TMA destinations (128-byte swizzle) need 1024-byte alignment: the launch asks for 1 KB of slack
+  c128 *smem = reinterpret_cast<c128 *>(smem_raw + ((1024u - (gwp::smem_u32(smem_raw) & 1023u)) & 1023u));
   const GwDims d = P.d;
   const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, ldt = P.ldt;
   c128 *sG = smem;                                   // [32][ldp]: sG[a][b] = G[t][k-q][a][b]
   c128 *sAux = sG + 8 * NDT * ldp;                   // astage x aux_units
-  c128 *sMain = sAux + P.astage * P.aux_units;       // nstage x main_units
+  c128 *sMain = smem + P.main_off;                   // nstage x main_units, 1024-byte aligned stages
   __shared__ uint64_t bars[2 * NST_MAX + 2 * AST_MAX + 6];
   uint64_t *full_m = bars, *empty_m = bars + NST_MAX, *full_a = bars + 2 * NST_MAX, *empty_a = full_a + AST_MAX;
   uint64_t *bar_g = empty_a + AST_MAX, *bar_phase = bar_g + 1, *uready = bar_g + 2, *ufree = bar_g + 4;
@@ -552,10 +539,10 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
   const size_t vb = (size_t)naux * n2;
   const int nmain = (naux + KC - 1) / KC;
   {
-    const int tot = 8 * NDT * ldp + P.astage * P.aux_units + P.nstage * P.main_units;
+    const int tot = P.main_off + P.nstage * P.main_units;
     for (int i = threadIdx.x; i < tot; i += NTHR) smem[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
-      for (int i = 0; i < P.nstage; i++) { gwp::mbar_init(full_m + i, N_MPROD); gwp::mbar_init(empty_m + i, NMAINW); }
+      for (int i = 0; i < P.nstage; i++) { gwp::mbar_init(full_m + i, 1); gwp::mbar_init(empty_m + i, NMAINW); }
       for (int i = 0; i < P.astage; i++) { gwp::mbar_init(full_a + i, N_APROD); gwp::mbar_init(empty_a + i, NAUXW); }
       gwp::mbar_init(bar_g, N_APROD);
       gwp::mbar_init(bar_phase, NAUXW);
@@ -567,30 +554,34 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
   if (w >= NMAINW + NAUXW) {
     gwp::reg_dec<REG_PROD>();
     if (w < 15) {
-      // ---- main-ring producer: W panel rows and V2 chunk rows ----
-      Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
-      const uint64_t polB = policy_evict_last();
-      for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-        const int t = item % d.ntau, k = P.kof(item / d.ntau);
-        for (int ql = 0; ql < d.nq; ql++) {
-          const int kp = gw_ksub(d, k, d.q0 + ql);
-          const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
-          const c128 *Wq = P.Wt + ((size_t)t * d.nq + ql) * naux * naux;
-          for (int qt = 0; qt < P.nqt; qt++) {
-            const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0);
-            const c128 *W = Wq + (size_t)Q0 * naux;
-            for (int ch = 0; ch < P.nchunk; ch++) {
-              const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
-              for (int j = 0; j < nmain; j++) {
-                const int s = rm.acquire();
-                issue_main(sMain + s * P.main_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC, polB);
-                rm.commit();
+      // ---- main-ring producer: ONE thread issues the TMA box loads of a job (the W panel K slice; one 8 x 8 box of V2 per
+      //      n-tile of the chunk) and arms the stage's mbarrier with the byte count ----
+      if (w == NMAINW + NAUXW && lane == 0) {
+        Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
+        const uint64_t polA = policy_evict_normal(), polB = policy_evict_last();
+        for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
+          const int t = item % d.ntau, k = P.kof(item / d.ntau);
+          for (int ql = 0; ql < d.nq; ql++) {
+            const int kp = gw_ksub(d, k, d.q0 + ql);
+            const int yV = (kp * d.nk + k) * naux;                    // V[k-q][k] rows of V viewed as [nk*nk*naux][nao²]
+            const int yW = (t * d.nq + ql) * naux;                    // Wt[t][q] rows of Wt viewed as [ntau*nq*naux][naux]
+            for (int qt = 0; qt < P.nqt; qt++) {
+              for (int ch = 0; ch < P.nchunk; ch++) {
+                const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
+                for (int j = 0; j < nmain; j++) {
+                  const int s = rm.acquire();
+                  const unsigned dst = gwp::smem_u32(sMain + s * P.main_units);
+                  mbar_expect_tx(full_m + s, (unsigned)(TM * KC * 16 + ntc * 1024));
+                  tma_load_2d(dst, &tmW, 2 * KC * j, yW + qt * TM, full_m + s, polA);
+                  for (int i = 0; i < ntc; i++)
+                    tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)i, &tmV, 16 * (nt0 + i), yV + KC * j, full_m + s, polB);
+                  rm.advance();
+                }
               }
             }
           }
         }
       }
-      asm volatile("cp.async.wait_all;\n" ::: "memory");
     } else {
       // ---- aux-ring producer: G per q, U^T rows of the finished unit (pass A), then V1[Q] + T[Q] per Q (final) ----
       Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
@@ -675,7 +666,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
     // ============================================ main warps ============================================
     gwp::reg_inc<REG_MAIN>();
     const int g = lane >> 2, c = lane & 3;
-    const int sw = (g & 1) << 2;
+    const int rho = (g >> 1) + 4 * (g & 1);           // fragment row / column of this lane group (see main_compute)
     Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
     unsigned un = 0;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
@@ -702,24 +693,24 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
             for (int jb = 0; jb < nmain; jb++) {
               const int s = rm.wait();
               if (active) {
-                const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + g) * KC;
-                const c128 *sBw = sMain + s * P.main_units + TM * KC + 8 * noff + g;
+                const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + rho) * KC;
+                const c128 *sBw = sMain + s * P.main_units + TM * KC + 64 * noff;
                 if (narrow) {
-                  if (mtw == 1 && njm == 3) main_compute<3, 8, 1>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                  else if (mtw == 1 && njm == 2) main_compute<2, 8, 1>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                  else if (mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                  else if (njm == 4) main_compute<4, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                  else if (njm == 3) main_compute<3, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                  else if (njm == 2) main_compute<2, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                  else main_compute<1, 8, 2>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                  if (mtw == 1 && njm == 3) main_compute<3, 8, 1>(sAw, sBw, accr, acci, c, rho);
+                  else if (mtw == 1 && njm == 2) main_compute<2, 8, 1>(sAw, sBw, accr, acci, c, rho);
+                  else if (mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, accr, acci, c, rho);
+                  else if (njm == 4) main_compute<4, 8, 2>(sAw, sBw, accr, acci, c, rho);
+                  else if (njm == 3) main_compute<3, 8, 2>(sAw, sBw, accr, acci, c, rho);
+                  else if (njm == 2) main_compute<2, 8, 2>(sAw, sBw, accr, acci, c, rho);
+                  else main_compute<1, 8, 2>(sAw, sBw, accr, acci, c, rho);
                 }
-                else if (njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 4) main_compute<4>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 3) main_compute<3>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (njm == 2) main_compute<2>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else main_compute<1>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                else if (njm == 7) main_compute<7>(sAw, sBw, accr, acci, c, rho);
+                else if (njm == 6) main_compute<6>(sAw, sBw, accr, acci, c, rho);
+                else if (njm == 5) main_compute<5>(sAw, sBw, accr, acci, c, rho);
+                else if (njm == 4) main_compute<4>(sAw, sBw, accr, acci, c, rho);
+                else if (njm == 3) main_compute<3>(sAw, sBw, accr, acci, c, rho);
+                else if (njm == 2) main_compute<2>(sAw, sBw, accr, acci, c, rho);
+                else main_compute<1>(sAw, sBw, accr, acci, c, rho);
               }
               rm.release();
             }
@@ -728,13 +719,13 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
             // store U^T: element (Q, n=(b,j)) -> U[(Q*nao + j)*nao + b]
 #pragma unroll
             for (int i = 0; i < MT_W; i++) {
-              const int Ql = 8 * (mh * MT_W + i) + g;
+              const int Ql = 8 * (mh * MT_W + i) + rho;            // accumulator row g holds panel row rho(g)
 #pragma unroll
               for (int jn = 0; jn < NJ; jn++) {
                 if (jn < njm && Ql < tm_rows) {
 #pragma unroll
                   for (int e = 0; e < 2; e++) {
-                    const int n = n0 + 8 * (noff + nstride * jn) + 2 * c + e;
+                    const int n = n0 + 8 * (noff + nstride * jn) + c + 4 * e;   // accumulator columns 2c, 2c+1 hold columns c, c+4
                     if (n < n2) {
                       const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
                       U[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
@@ -752,7 +743,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P) {
   }
 }
 
-struct Plan { int nqt, nitems, ldp, ldt, nnt, nchunk, cht, ldb, main_units, aux_units, nstage, astage, grid; size_t smem, slab_units, work_bytes; bool ok; };
+struct Plan { int nqt, nitems, ldp, ldt, nnt, nchunk, cht, ldb, main_units, aux_units, nstage, astage, main_off, grid; size_t smem, slab_units, work_bytes; bool ok; };
 
 static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
@@ -766,20 +757,47 @@ static Plan make_plan(const gw_problem *p) {
   pl.ldb = pl.cht * 8 + 2;
   pl.nqt = (d.naux + TM - 1) / TM;
   { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
-  pl.main_units = TM * KC + KC * pl.ldb;
+  pl.main_units = TM * KC + 64 * pl.cht;      // A: 32 rows x 128 B; B: one 1 KB box per n-tile of the chunk
   const int s_pass = AROWS * pl.ldp, s_fin = 8 * NDT * pl.ldp + 4 * KSP * pl.ldt + 8;
   pl.aux_units = s_pass > s_fin ? s_pass : s_fin;
   pl.astage = 2;
-  const size_t cap = 226 * 1024, fixed = ((size_t)8 * NDT * pl.ldp + (size_t)pl.astage * pl.aux_units) * sizeof(c128);
+  // 1 KB of the 227 KB is alignment slack: the main stages (TMA destinations, 128-byte swizzle) start 1024-byte aligned
+  const size_t cap = 225 * 1024;
+  const size_t fixed = (((size_t)8 * NDT * pl.ldp + (size_t)pl.astage * pl.aux_units) * sizeof(c128) + 1023) / 1024 * 1024;
+  pl.main_off = (int)(fixed / sizeof(c128));
   pl.nstage = (int)((cap - fixed) / ((size_t)pl.main_units * sizeof(c128)));
   if (pl.nstage > 6) pl.nstage = 6;
-  pl.smem = fixed + (size_t)pl.nstage * pl.main_units * sizeof(c128);
+  pl.smem = fixed + (size_t)pl.nstage * pl.main_units * sizeof(c128) + 1024;
   const int nsm = gwp::gw_num_sms();
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
   pl.work_bytes = 256 + (size_t)nsm * 3 * pl.slab_units * sizeof(c128);
   pl.ok = pl.nstage >= 3;
   return pl;
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda):
+// [rows][ncplx complex] row-major matrix, box = box_rows x 8 complex, 128-byte swizzle
+static int make_map(CUtensorMap *map, const void *base, size_t rows, int ncplx, int box_rows) {
+  typedef CUresult (*Fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                         const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Fn fn = nullptr;
+  if (!fn) {
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
+      cudaGetLastError();
+      return (int)cudaErrorNotSupported;
+    }
+    fn = (Fn)ptr;
+  }
+  const cuuint64_t gdim[2] = {(cuuint64_t)2 * ncplx, (cuuint64_t)rows};
+  const cuuint64_t gstr[1] = {(cuuint64_t)ncplx * 16};
+  const cuuint32_t box[2] = {(cuuint32_t)(2 * KC), (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
 }
 
 static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
@@ -793,9 +811,17 @@ static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigm
   P.main_units = pl.main_units; P.aux_units = pl.aux_units; P.nstage = pl.nstage; P.astage = pl.astage; P.slab_units = pl.slab_units;
   P.fd_nao = FastDiv((unsigned)P.d.nao);
   P.nkeff = fill_kirr(P.d, P.kirr);
+  P.main_off = pl.main_off;
   cudaError_t e = cudaFuncSetAttribute(sigma_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
-  sigma_ws_kernel<<<pl.grid, NTHR, pl.smem, st>>>(P);
+  // tensor maps: Wt as [ntau*nq*naux rows][naux complex], box 32 rows x 8 complex; V as [nk*nk*naux rows][nao² complex],
+  // box 8 rows x 8 complex; 128-byte swizzle, zero fill outside the arrays
+  CUtensorMap tmW, tmV;
+  int rc = make_map(&tmW, Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, TM);
+  if (rc) return rc;
+  rc = make_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, KC);
+  if (rc) return rc;
+  sigma_ws_kernel<<<pl.grid, NTHR, pl.smem, st>>>(P, tmW, tmV);
   return (int)cudaGetLastError();
 }
 
