@@ -38,6 +38,7 @@ struct Params {
   int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
   int ldb;                // row stride of the main-job B part
   int stage_units, nstage;
+  int stage_off;          // offset of the ring in the 1024-byte aligned dynamic shared memory (complex elements)
   size_t slab_units;      // complex elements per slab (two slabs per CTA)
   int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
   short kirr[128];        // the evaluated k points when nkeff < nk
@@ -45,51 +46,29 @@ struct Params {
   FastDiv fd_nao;
 };
 
-// main job (producer warpgroup): A = W[tm rows][k0..k0+8) swizzled by row parity (rows beyond tm_rows re-read the last valid
-// row: their products land in accumulators that are never stored); B = V2[k0..k0+8 rows (Q')][n0..n0+ncols) as [8][ldb]
-// (K rows beyond naux and columns beyond nao² zero filled).  One source pointer per column, constant row stride; the V block is
-// shared by the ~100 CTAs working on the same k (L2 evict-last hint).
-__device__ __forceinline__ void ws_issue_main(c128 *stage, const c128 *W, int tm_rows, int naux, const c128 *V2, int n2,
-                                              int n0, int ncols, int ldb, int k0, uint64_t polB) {
-  const int pt = threadIdx.x - 32 * NCONS;
-  const unsigned sA = gwp::smem_u32(stage);
-  {
-    const int u = pt & 7, rsub = pt >> 3;
-    const bool kok = k0 + u < naux;
-    const int nb = kok ? 16 : 0;
-    const c128 *src = W + (kok ? k0 + u : 0);
-#pragma unroll
-    for (int r = rsub; r < TM; r += gwp::NPROD_THR / 8) {
-      const int rr = min(r, tm_rows - 1);
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"((sA + 16u * (unsigned)(r * KC + u)) ^ ((unsigned)(r & 1) << 6)),
-                   "l"(src + (size_t)rr * naux), "r"(nb));
-    }
-  }
-  const unsigned sB = sA + 16u * TM * KC;
-  for (int cc = pt; cc < ncols; cc += gwp::NPROD_THR) {
-    const bool cok = n0 + cc < n2;
-    const c128 *src = V2 + (size_t)k0 * n2 + (cok ? n0 + cc : 0);
-    const unsigned dst = sB + 16u * (unsigned)cc;
-#pragma unroll
-    for (int r = 0; r < KC; r++) {
-      const bool ok = cok && (k0 + r < naux);
-      asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst + 16u * (unsigned)(r * ldb)),
-                   "l"(ok ? src + (size_t)r * n2 : V2), "r"(ok ? 16 : 0), "l"(polB));
-    }
-  }
+// Main jobs are written by TMA with the 128-byte swizzle (16-byte unit u of row r sits at u ^ (r & 7)):
+//   A = W[TM rows][8 K]: 32 rows x 128 B;   B = one 1 KB box per n-tile of the chunk: [8 K rows][8 columns of V2].
+// Lane group g reads row / column rho(g) = (g >> 1) + 4 (g & 1) of its tile, so a quarter-warp touches eight different units.
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
+               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(gwp::smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(gwp::smem_u32(bar)), "r"(bytes) : "memory");
 }
 
 template <int NJM>
-__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, int ldb, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
+__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int rho) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
-    const int u = (4 * ks + c) ^ sw;
+    const int kr = 4 * ks + c;
+    const int u = kr ^ rho;
     c128 a[MT_W], b[NJM];
 #pragma unroll
     for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
-    const c128 *brow = sBw + (4 * ks + c) * ldb;
+    const c128 *bk = sBw + kr * 8 + u;
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++) b[jn] = brow[32 * jn];
+    for (int jn = 0; jn < NJM; jn++) b[jn] = bk[256 * jn];      // n-tiles 4 apart, 64 units per n-tile box
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++)
 #pragma unroll
@@ -98,13 +77,14 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, i
 }
 
 template <int KSP_MAX, int NCT>
-__global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
+__global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P, const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmV) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  c128 *smem = reinterpret_cast<c128 *>(smem_raw);
+  // the TMA destinations (128-byte swizzle) need 1024-byte alignment: the launch asks for 1 KB of slack
+  c128 *smem = reinterpret_cast<c128 *>(smem_raw + ((1024u - (gwp::smem_u32(smem_raw) & 1023u)) & 1023u));
   const GwDims d = P.d;
   const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, naop = 8 * P.ndt, ndt = P.ndt;
   c128 *sG = smem;                    // [naop][ldp]: sG[a][b] = G[t][k-q][a][b]  (operand [n=a][k=b] of pass A)
-  c128 *sStage = sG + naop * ldp;
+  c128 *sStage = smem + P.stage_off;   // ring of 1024-byte aligned stage buffers
   const int NSTAGE = P.nstage;
   __shared__ uint64_t bars[2 * NSTAGE_MAX + 2];
   uint64_t *bar_full = bars, *bar_empty = bars + NSTAGE_MAX, *bar_g = bars + 2 * NSTAGE_MAX, *bar_phase = bars + 2 * NSTAGE_MAX + 1;
@@ -113,7 +93,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
   c128 *slabT = slabU + P.slab_units;
   const size_t vb = (size_t)naux * n2;
   {
-    const int tot = naop * ldp + NSTAGE * P.stage_units;
+    const int tot = P.stage_off + NSTAGE * P.stage_units;
     for (int i = threadIdx.x; i < tot; i += NTHR_WS) smem[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
       for (int i = 0; i < NSTAGE; i++) { gwp::mbar_init(bar_full + i, gwp::NPROD_THR); gwp::mbar_init(bar_empty + i, NCONS); }
@@ -129,7 +109,8 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
   if (w >= NCONS) {
     // =============================== producer warpgroup ===============================
     gwp::reg_dec<40>();
-    uint64_t polB;
+    uint64_t polA, polB;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;\n" : "=l"(polA));
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(polB));
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
       const int t = item % d.ntau, k = P.kof(item / d.ntau);
@@ -137,18 +118,27 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
         const int q = d.q0 + ql, kp = gw_ksub(d, k, q);
         const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
         const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
-        const c128 *Wq = P.Wt + ((size_t)t * d.nq + ql) * naux * naux;
+        const int yV = (kp * d.nk + k) * naux, yW = (t * d.nq + ql) * naux;   // first rows of V[k-q][k] and Wt[t][q] in the TMA views
         gwp::ws_issue_matrix<false>(sG, P.G + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
         gwp::cp_async_arrive_noinc(bar_g);
         for (int qt = 0; qt < P.nqt; qt++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0);
-          const c128 *W = Wq + (size_t)Q0 * naux;
           for (int ch = 0; ch < P.nchunk; ch++) {
             const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0);
             for (int j = 0; j < nmain; j++) {
               const int s = ring.acquire();
-              ws_issue_main(sStage + s * P.stage_units, W, tm_rows, naux, V2, n2, nt0 * 8, ntc * 8, P.ldb, j * KC, polB);
-              ring.commit();
+              // main jobs come by TMA: one thread arms the barrier with the byte count and issues the boxes, the other
+              // producer threads only arrive (the ring's full barriers count all 128 producer threads for every job type)
+              if (threadIdx.x == 32 * NCONS) {
+                const unsigned dst = gwp::smem_u32(sStage + s * P.stage_units);
+                mbar_expect_tx(bar_full + s, (unsigned)(TM * KC * 16 + ntc * 1024));
+                tma_load_2d(dst, &tmW, 2 * KC * j, yW + Q0, bar_full + s, polA);
+                for (int i = 0; i < ntc; i++)
+                  tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)i, &tmV, 16 * (nt0 + i), yV + KC * j, bar_full + s, polB);
+              } else {
+                gwp::mbar_arrive(bar_full + s);
+              }
+              ring.advance();
             }
           }
           const int rows = tm_rows * nao, npass = (rows + PASS_ROWS - 1) / PASS_ROWS;
@@ -175,7 +165,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
     // =============================== consumer warps ===============================
     gwp::reg_inc<232>();
     const int g = lane >> 2, c = lane & 3;
-    const int sw = (g & 1) << 2;
+    const int rho = (g >> 1) + 4 * (g & 1);            // fragment row / column of this lane group in the TMA-swizzled main jobs
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
       const int t = item % d.ntau, k = P.kof(item / d.ntau);
       double sgr[NCT][2], sgi[NCT][2];
@@ -205,23 +195,23 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
             for (int jb = 0; jb < nmain; jb++) {
               const int s = ring.wait();
               if (active) {
-                const c128 *sAw = sStage + s * P.stage_units + (8 * mh * MT_W + g) * KC;
-                const c128 *sBw = sStage + s * P.stage_units + TM * KC + 8 * noff + g;
-                if (!narrow && njm == 7) main_compute<7>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (!narrow && njm == 6) main_compute<6>(sAw, sBw, P.ldb, accr, acci, c, sw);
-                else if (!narrow && njm == 5) main_compute<5>(sAw, sBw, P.ldb, accr, acci, c, sw);
+                const c128 *sAw = sStage + s * P.stage_units + (8 * mh * MT_W + rho) * KC;
+                const c128 *sBw = sStage + s * P.stage_units + TM * KC + 64 * noff;
+                if (!narrow && njm == 7) main_compute<7>(sAw, sBw, accr, acci, c, rho);
+                else if (!narrow && njm == 6) main_compute<6>(sAw, sBw, accr, acci, c, rho);
+                else if (!narrow && njm == 5) main_compute<5>(sAw, sBw, accr, acci, c, rho);
                 else {
 #pragma unroll
                   for (int ks = 0; ks < KC / 4; ks++) {
-                    const int u = (4 * ks + c) ^ sw;
+                    const int kr = 4 * ks + c, u = kr ^ rho;
                     c128 a[MT_W];
 #pragma unroll
                     for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
-                    const c128 *brow = sBw + (4 * ks + c) * P.ldb;
+                    const c128 *bk = sBw + kr * 8 + u;
 #pragma unroll
                     for (int jn = 0; jn < NJ; jn++) {
                       if (jn < njm) {
-                        const c128 b = brow[8 * nstride * jn];
+                        const c128 b = bk[64 * nstride * jn];
 #pragma unroll
                         for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
                       }
@@ -234,13 +224,13 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
             // store U^T: element (Q, n=(b,j)) -> slabU[(Q*nao + j)*nao + b]
 #pragma unroll
             for (int i = 0; i < MT_W; i++) {
-              const int Ql = 8 * (mh * MT_W + i) + g;
+              const int Ql = 8 * (mh * MT_W + i) + rho;            // accumulator row g holds panel row rho(g)
 #pragma unroll
               for (int jn = 0; jn < NJ; jn++) {
                 if (jn < njm && Ql < tm_rows) {
 #pragma unroll
                   for (int e = 0; e < 2; e++) {
-                    const int n = n0 + 8 * (noff + nstride * jn) + 2 * c + e;
+                    const int n = n0 + 8 * (noff + nstride * jn) + c + 4 * e;   // accumulator columns 2c, 2c+1 hold columns c, c+4
                     if (n < n2) {
                       const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
                       slabU[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
@@ -282,6 +272,7 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P) {
 }
 
 struct Plan {
+  int stage_off;
   int ksp_max, nct, nqt, nitems, ldp, ksp, ndt, ldt, kh, kspf, ldpf, nnt, nchunk, cht, ldb, stage_units, grid, nstage;
   size_t smem, slab_units, work_bytes;
   bool ok;
@@ -305,8 +296,10 @@ static Plan make_plan(const gw_problem *p) {
   pl.ldb = pl.cht * 8 + 2;
   pl.nqt = (d.naux + TM - 1) / TM;
   { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
-  const int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + KC * pl.ldb;
-  const size_t fixed = (size_t)naop * pl.ldp * sizeof(c128);
+  const int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + 64 * pl.cht;   // main: A 32 rows x 128 B + one 1 KB box per n-tile
+  // the ring starts 1024-byte aligned and every stage is a multiple of 1024 bytes (TMA destinations, 128-byte swizzle)
+  const size_t fixed = ((size_t)naop * pl.ldp * sizeof(c128) + 1023) / 1024 * 1024;
+  pl.stage_off = (int)(fixed / sizeof(c128));
   // final jobs cover one Q, or half of its K range when a whole Q would leave fewer than 3 ring stages
   for (pl.kh = 1; pl.kh <= 2; pl.kh++) {
     pl.kspf = (pl.ksp + pl.kh - 1) / pl.kh;
@@ -316,10 +309,11 @@ static Plan make_plan(const gw_problem *p) {
     pl.stage_units = s_pass;
     if (s_main > pl.stage_units) pl.stage_units = s_main;
     if (s_fin > pl.stage_units) pl.stage_units = s_fin;
+    pl.stage_units = (pl.stage_units + 63) / 64 * 64;
     const size_t per = (size_t)pl.stage_units * sizeof(c128);
     pl.nstage = (int)((225 * 1024 - fixed) / per);
     if (pl.nstage > 6) pl.nstage = 6;
-    pl.smem = fixed + (size_t)pl.nstage * per;
+    pl.smem = fixed + (size_t)pl.nstage * per + 1024;
     if (pl.nstage >= 3) break;
   }
   if (pl.kh > 2) pl.kh = 2;
@@ -353,11 +347,19 @@ double gw_stage3_flops(const gw_problem *p) {
   return tiles * (double)d.nq * fill_kirr(d, tmp) * d.ntau * 2048.0;
 }
 
+namespace s3w { static int make_map(CUtensorMap *map, const void *base, size_t rows, int ncplx, int box_rows); }
+
 template <int KSP_MAX, int NCT>
 static int launch_sigma(const s3::Plan &pl, const s3::Params &P, cudaStream_t st) {
   cudaError_t e = cudaFuncSetAttribute(s3::sigma_kernel<KSP_MAX, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
-  s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR_WS, pl.smem, st>>>(P);
+  // tensor maps of the main jobs: Wt as [ntau*nq*naux rows][naux complex] (box 32 x 8), V as [nk*nk*naux rows][nao² complex] (box 8 x 8)
+  CUtensorMap tmW, tmV;
+  int rc = s3w::make_map(&tmW, P.Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, s3::TM);
+  if (rc) return rc;
+  rc = s3w::make_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, s3::KC);
+  if (rc) return rc;
+  s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR_WS, pl.smem, st>>>(P, tmW, tmV);
   return (int)cudaGetLastError();
 }
 
@@ -370,7 +372,7 @@ static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigm
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
   P.scratch = (c128 *)((char *)p->work + 256);
   P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt; P.kh = pl.kh; P.kspf = pl.kspf; P.ldpf = pl.ldpf; P.fd_kw = gwp::FastDiv((unsigned)(4 * pl.kspf));
-  P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.slab_units = pl.slab_units;
+  P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb; P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.stage_off = pl.stage_off; P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
   P.nkeff = fill_kirr(P.d, P.kirr);
   if (pl.nct == 2) {
