@@ -170,8 +170,8 @@ class ClockSampler:
 
 # dram traffic per launch of the dominant kernel from the committed ncu capture (profiles/), keyed by config; None = not captured
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu captures summarised in profiles/ (key: config, stage)
-NCU_TRAFFIC_BYTES = {("cfg2", 0): 4802780972032 + 1769176705024,      # profiles/r01_dram_cfg2.csv, s1::p0_kernel<7>
-                     ("cfg2", 2): 5304567847168 + 1975679740672}      # s3w::sigma_ws_kernel
+NCU_TRAFFIC_BYTES = {("cfg2", 0): 2674593790976 + 1641546826752,      # profiles/r01_dram_cfg2.csv, s1::p0_kernel<7>
+                     ("cfg2", 2): 3435090394112 + 1932940943360}      # s3w::sigma_ws_kernel
 
 
 def run_ours(args):

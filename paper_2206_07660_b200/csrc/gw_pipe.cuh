@@ -1,5 +1,7 @@
-// gw_pipe.cuh — building blocks shared by the stage kernels: cp.async stage jobs and complex-tile DMMA passes.
-// All kernels run 256 threads (8 warps) per CTA, one CTA per SM, with an NSTAGE-deep cp.async ring of stage buffers.
+// gw_pipe.cuh — building blocks shared by the stage kernels: cp.async stage jobs, mbarrier rings, cluster helpers and the
+// complex-tile DMMA passes (small-K GEMMs against an nao x nao matrix held in shared memory).
+// Stage 4 runs 256 threads per CTA with a 3-deep cp.async ring (NTHR, NSTAGE below); stages 1 and 3 are warp specialised
+// (gw_stage1.cu, gw_stage3.cu) and use the mbarrier ring / setmaxnreg helpers further down.  One CTA per SM everywhere.
 #pragma once
 #include "gw_common.cuh"
 
