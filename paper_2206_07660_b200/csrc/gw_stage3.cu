@@ -129,12 +129,13 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P, const
               const int s = ring.acquire();
               // main jobs come by TMA: one thread arms the barrier with the byte count and issues the boxes, the other
               // producer threads only arrive (the ring's full barriers count all 128 producer threads for every job type)
-              if (threadIdx.x == 32 * NCONS) {
+              if (w == NCONS) {                                  // first producer warp: its 32 lanes issue the boxes in one go
                 const unsigned dst = gwp::smem_u32(sStage + s * P.stage_units);
-                mbar_expect_tx(bar_full + s, (unsigned)(TM * KC * 16 + ntc * 1024));
-                tma_load_2d(dst, &tmW, 2 * KC * j, yW + Q0, bar_full + s, polA);
-                for (int i = 0; i < ntc; i++)
-                  tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)i, &tmV, 16 * (nt0 + i), yV + KC * j, bar_full + s, polB);
+                if (lane == 0) mbar_expect_tx(bar_full + s, (unsigned)(TM * KC * 16 + ntc * 1024));
+                __syncwarp();
+                if (lane == 31) tma_load_2d(dst, &tmW, 2 * KC * j, yW + Q0, bar_full + s, polA);
+                if (lane < ntc) tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)lane, &tmV, 16 * (nt0 + lane), yV + KC * j, bar_full + s, polB);
+                if (lane != 0) gwp::mbar_arrive(bar_full + s);
               } else {
                 gwp::mbar_arrive(bar_full + s);
               }
@@ -558,7 +559,9 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
     if (w < 15) {
       // ---- main-ring producer: ONE thread issues the TMA box loads of a job (the W panel K slice; one 8 x 8 box of V2 per
       //      n-tile of the chunk) and arms the stage's mbarrier with the byte count ----
-      if (w == NMAINW + NAUXW && lane == 0) {
+      if (w == NMAINW + NAUXW) {
+        // the 32 lanes of this warp issue the boxes of a job in one go: lane 0 arms the barrier, lanes < ntc load one V box
+        // each, lane 31 loads the W box
         Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
         const uint64_t polA = policy_evict_normal(), polB = policy_evict_last();
         for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
@@ -573,10 +576,10 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
                 for (int j = 0; j < nmain; j++) {
                   const int s = rm.acquire();
                   const unsigned dst = gwp::smem_u32(sMain + s * P.main_units);
-                  mbar_expect_tx(full_m + s, (unsigned)(TM * KC * 16 + ntc * 1024));
-                  tma_load_2d(dst, &tmW, 2 * KC * j, yW + qt * TM, full_m + s, polA);
-                  for (int i = 0; i < ntc; i++)
-                    tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)i, &tmV, 16 * (nt0 + i), yV + KC * j, full_m + s, polB);
+                  if (lane == 0) mbar_expect_tx(full_m + s, (unsigned)(TM * KC * 16 + ntc * 1024));
+                  __syncwarp();
+                  if (lane == 31) tma_load_2d(dst, &tmW, 2 * KC * j, yW + qt * TM, full_m + s, polA);
+                  if (lane < ntc) tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)lane, &tmV, 16 * (nt0 + lane), yV + KC * j, full_m + s, polB);
                   rm.advance();
                 }
               }
