@@ -258,7 +258,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
     // ========================================= pass warps =========================================
     if constexpr (REG_PASS > 65536 / NTHR1) gwp::reg_inc<REG_PASS>(); else gwp::reg_dec<REG_PASS>();
     const int wp = w - NMAINW;
-    constexpr int PMT = 1;                             // m-tiles per pass warp (prows = 32*PMT); 2 measured slower (fewer main registers)
+    constexpr int PMT = KSP_MAX <= 8 ? 2 : 1;          // m-tiles per pass warp on the exact path (prows = 32*PMT there)
     Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
     unsigned kit = 0, ph = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
@@ -436,7 +436,7 @@ static Plan make_plan(const gw_problem *p) {
   { short tmp[128]; pl.nqeff = fill_qirr(d, tmp); }
   pl.nitems = pl.nqt * pl.nteff * pl.nqeff;
   pl.main_units = (TM + 8 * pl.ntc) * KC;
-  pl.prows = 32;
+  pl.prows = (pl.ksp == pl.ksp_max && pl.ksp_max <= 8) ? 64 : 32;
   pl.pass_units = pl.prows * pl.ldp;
   // shared memory: prefer both G matrices resident and a 3-deep pass ring; shrink them while the main ring has < 4 stages
   const size_t gsz = (size_t)8 * pl.ndt * pl.ldp * sizeof(c128), psz = (size_t)pl.pass_units * sizeof(c128), msz = (size_t)pl.main_units * sizeof(c128);

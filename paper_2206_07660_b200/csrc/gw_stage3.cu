@@ -403,7 +403,8 @@ namespace s3w {
 using gwp::FastDiv;
 constexpr int NMAINW = 8, NAUXW = 4, NTHR = 512;
 constexpr int T_MPROD = 384, N_MPROD = 96, T_APROD = 480, N_APROD = 32;
-constexpr int KC = 8, MT_W = 2, NJ = 7, TM = 32, KSP = 7, NDT = 4, AROWS = 32;
+constexpr int KC = 8, MT_W = 2, NJ = 7, TM = 32, KSP = 7, NDT = 4;
+constexpr int AMT = 1, AROWS = 32 * AMT;      // pass A: m-tiles per aux warp and rows per job (2 measured slower)
 constexpr int NST_MAX = 8, AST_MAX = 4;
 constexpr int REG_MAIN = 176, REG_AUX = 120, REG_PROD = 40;
 
@@ -637,7 +638,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
           gwp::mbar_wait(bar_g, un & 1u);
           for (int j = 0; j < npass; j++) {
             const int s = ra.wait();
-            gwp::pass_compute_exact_mt<KSP, true, 1>(sAux + s * P.aux_units, sG, slabT, j * AROWS, rows, nao, ldp, wa, P.fd_nao);
+            gwp::pass_compute_exact_mt<KSP, true, AMT>(sAux + s * P.aux_units, sG, slabT, j * AROWS, rows, nao, ldp, wa, P.fd_nao);
             ra.release();
           }
           __threadfence(); __syncwarp();
