@@ -66,10 +66,13 @@ typedef struct {
 } gw_problem;
 
 /* gw_problem.symmetry flag.  Time reversal: G[t][−k] = conj(G[t][k]) and V[−k1][−k2] = conj(V[k1][k2]) element-wise (the same
- * property that makes I − P̃0(iΩ) Hermitian for the Cholesky solve; the paper exploits k ↔ −k too).  Then
+ * property that makes I − P̃0(iΩ) Hermitian for the Cholesky solve; the paper exploits k ↔ −k too), together with
+ * V[k1][k2][Q][i][j] = conj(V[k2][k1][Q][j][i]) and Hermitian G[t][k] (true of the BASELINE.json inputs and of any physical G).  Then
+ * P̃0^q(τ) is Hermitian,
  * P̃0^q(β−τ) = P̃0^q(τ) and Σ^{−k}(τ) = conj Σ^{k}(τ), and the library evaluates only the irreducible half and copies the rest:
  *   gw_polarization : tau nodes t <= ntau-1-t are computed, P0t[ntau-1-t] is a copy of P0t[t]; for the full q range and
  *                     nk <= 128 also only q <= −q, and P0t[t][−q] = transpose(P0t[t][q])  (216 -> 112 q points);
+ *                     of each Q panel only the column tiles up to its diagonal block are computed, the rest is the conjugate mirror;
  *   gw_selfenergy   : k <= −k are computed, Sigma[t][−k] = conj(Sigma[t][k])  (only for the full q range and nk <= 128);
  * the other calls ignore the flag.  Computed elements are bit-identical to the literal evaluation.  If the inputs do not
  * have the symmetry the copied elements are wrong — nothing checks it. */

@@ -46,6 +46,7 @@ struct Params {
   int cs;                // CTAs per cluster = column splits of the panel
   int nqt, nitems;       // Q tiles per (t,q); total work items
   int nteff;             // tau nodes evaluated: ntau, or ceil(ntau/2) under GW_SYM_TR (the rest is mirrored)
+  int herm;              // GW_SYM_TR: P0t[t][q] is Hermitian, only the column tiles up to the panel's diagonal block are computed
   int nqeff;             // q points evaluated: nq, or the q <= -q half under GW_SYM_TR (P0[-q] = P0[q]^T is copied)
   short qirr[128];       // the evaluated q points when nqeff < nq
   __device__ __forceinline__ int qof(int i) const { return nqeff < d.nq ? (int)qirr[i] : i; }
@@ -319,7 +320,9 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
       const int noff = narrow ? w : (((w & 3) - mh + 4) & 3);
       const int nstride = narrow ? 8 : 4;
       const int mtw = (narrow && mtc == 1) ? 1 : MT_W;
-      const int njm = (ntc_mine > noff) ? (ntc_mine - noff + nstride - 1) / nstride : 0;
+      // Hermitian mode: columns right of the panel's diagonal block come from the mirror writes of the later panels
+      const int ntc_item = P.herm ? min(ntc_mine, max(0, it.Q0 + TM - col0 + 7) / 8) : ntc_mine;
+      const int njm = (ntc_item > noff) ? (ntc_item - noff + nstride - 1) / nstride : 0;
       const bool active = (mh * MT_W < mtc) && njm > 0;
       double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
 #pragma unroll
@@ -387,12 +390,18 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
               const int ca = 8 * (noff + nstride * jn) + c, cb = ca + 4;
               const c128 v0 = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
               const c128 v1 = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
-              if (!tr) {
-                if (ca < ncols) out[(size_t)Q * naux + col0 + ca] = v0;
-                if (cb < ncols) out[(size_t)Q * naux + col0 + cb] = v1;
-              } else {
-                if (ca < ncols) out[(size_t)(col0 + ca) * naux + Q] = v0;
-                if (cb < ncols) out[(size_t)(col0 + cb) * naux + Q] = v1;
+              // element (Q, col) goes to [Q][col], or to [col][Q] in the transposed copy for -q; in Hermitian mode the elements
+              // left of the diagonal block also fill their mirror image with the conjugate
+#pragma unroll
+              for (int e = 0; e < 2; e++) {
+                const int cl = e ? cb : ca;
+                if (cl < ncols) {
+                  const c128 v = e ? v1 : v0;
+                  const size_t col = (size_t)(col0 + cl);
+                  const size_t direct = tr ? col * naux + Q : (size_t)Q * naux + col;
+                  out[direct] = v;
+                  if (P.herm && (int)col < it.Q0) out[tr ? (size_t)Q * naux + col : col * naux + Q] = make_double2(v.x, -v.y);
+                }
               }
             }
           }
@@ -487,7 +496,9 @@ double gw_stage1_flops(const gw_problem *p) {
     // main: warps whose first m-tile is valid execute MT_W m-tiles x their n-tiles x 2 k-steps per job
     const double mtiles = mtc <= 2 ? (double)mtc : (double)((mtc + s1::MT_W - 1) / s1::MT_W) * s1::MT_W;   // ragged panel: narrow ownership
     const double nmain = (d.nao * d.nao + s1::KC - 1) / s1::KC;
-    const double mainv = mtiles * pl.nt * (s1::KC / 4) * nmain;
+    int nt_eff = pl.nt;                         // Hermitian mode: n-tiles up to the panel's diagonal block
+    if ((d.sym & GW_SYM_TR) && nt_eff > (qt * s1::TM + s1::TM + 7) / 8) nt_eff = (qt * s1::TM + s1::TM + 7) / 8;
+    const double mainv = mtiles * nt_eff * (s1::KC / 4) * nmain;
     tiles += pass + mainv;
   }
   return tiles * (double)d.nk * pl.nteff * pl.nqeff * 2048.0;
@@ -561,7 +572,7 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   s1::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
+  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.herm = (P.d.sym & GW_SYM_TR) ? 1 : 0; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
   P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.main_off = pl.main_off; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
