@@ -60,6 +60,11 @@ CONFIGS = {
     "Q": GWConfig("cfgQ", (4, 4, 4), 52, 400, 8, 8, 1000.0, -3.0, 5.0, 0.04, BASE_SEED + 95),
     # config-4-shaped basis (nao=52, naux > 224: the wide-panel / split-K kernel variants) at a size the oracle does in full
     "L": GWConfig("cfgL", (2, 1, 1), 52, 230, 8, 8, 50.0, -3.0, 5.0, 0.04, BASE_SEED + 96),
+    # config 4's exact kernel launch shape (nao=52, naux=400: 25 n-tiles per CTA of the stage-1 cluster, 13 Q panels, split-K
+    # final jobs) on a 2-point mesh with 6 tau nodes, small enough for the oracle to do in full
+    "M": GWConfig("cfgM", (2, 1, 1), 52, 400, 6, 6, 50.0, -3.0, 5.0, 0.04, BASE_SEED + 91),
+    # naux beyond one cluster's 448 panel columns (stage 1 runs two column passes), small basis
+    "X": GWConfig("cfgX", (2, 1, 1), 6, 460, 6, 6, 20.0, -1.5, 2.0, 0.04, BASE_SEED + 90),
 }
 
 

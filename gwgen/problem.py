@@ -25,13 +25,29 @@ class Problem:
     extras: dict = field(default_factory=dict)
 
 
-def make_problem(cfg, v_device="cpu", with_V=True) -> Problem:
+def make_problem(cfg, v_device="cpu", with_V=True, raw=False) -> Problem:
+    """raw=False: the BASELINE.json inputs (time-reversal symmetric Fock-built G, group-averaged V).
+    raw=True : inputs with NO symmetry at all — V blocks are independent draws (V[k1][k2] unrelated to V[k2][k1] or
+               V[-k1][-k2]), G[t][k] and gamma[k] are seeded non-Hermitian complex matrices, extras["W"] is a seeded
+               non-Hermitian [ntau][nk][naux][naux] array to stand in for Wt.  They tell the printed index patterns of
+               Eq. 22 / 28b / 31 apart from their symmetric twins (transposed or conjugated operands); stage 2 (Cholesky)
+               is not defined on them."""
     if not isinstance(cfg, GWConfig):
         cfg = get_config(cfg)
     mesh = KMesh(cfg.mesh)
     gr = make_grids(cfg.ntau, cfg.nw, cfg.beta)
     eps, U = make_fock(cfg, mesh)
-    G = greens_function(eps, U, gr["tau"], cfg.beta)
-    gamma = density_matrix(eps, U, cfg.beta)
-    V = make_V(cfg, mesh, device=v_device) if with_V else None
-    return Problem(cfg, mesh, gr["tau"], gr["nbos"], gr["T_wt"], gr["T_tw"], eps, U, G, gamma, V)
+    extras = {}
+    if raw:
+        rng = np.random.default_rng([cfg.seed, 7])
+        cplx = lambda shape, sc: np.ascontiguousarray((rng.normal(size=shape) + 1j * rng.normal(size=shape)) * sc)
+        # a tau-dependent scale keeps the decades-wide dynamic range of a physical G(tau)
+        scale = np.exp(-6.0 * np.minimum(gr["tau"], cfg.beta - gr["tau"]) / cfg.beta).reshape(-1, 1, 1, 1)
+        G = cplx((cfg.ntau, mesh.nk, cfg.nao, cfg.nao), 1.0 / np.sqrt(cfg.nao)) * scale
+        gamma = cplx((mesh.nk, cfg.nao, cfg.nao), 1.0 / np.sqrt(cfg.nao))
+        extras["W"] = cplx((cfg.ntau, mesh.nk, cfg.naux, cfg.naux), 1.0 / np.sqrt(cfg.naux))
+    else:
+        G = greens_function(eps, U, gr["tau"], cfg.beta)
+        gamma = density_matrix(eps, U, cfg.beta)
+    V = make_V(cfg, mesh, device=v_device, raw=raw) if with_V else None
+    return Problem(cfg, mesh, gr["tau"], gr["nbos"], gr["T_wt"], gr["T_tw"], eps, U, G, gamma, V, extras)

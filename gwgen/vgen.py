@@ -55,8 +55,9 @@ def _raw_block(seed, blk_index, n_per_block, device):
     return torch.complex(r * torch.cos(ang), r * torch.sin(ang))
 
 
-def make_V_block(cfg, mesh, k1, k2, device="cpu", neg=None):
-    """V[k1][k2] as a torch complex128 tensor [naux][nao][nao] on `device`."""
+def make_V_block(cfg, mesh, k1, k2, device="cpu", neg=None, raw=False):
+    """V[k1][k2] as a torch complex128 tensor [naux][nao][nao] on `device`.
+    raw=True: the i.i.d. block R[k1][k2] itself, with none of the symmetries (tests of the literal, symmetry-free path)."""
     nk, nao, naux = mesh.nk, cfg.nao, cfg.naux
     if neg is None:
         neg = mesh.neg()
@@ -66,18 +67,26 @@ def make_V_block(cfg, mesh, k1, k2, device="cpu", neg=None):
     def R(a, b):
         return _raw_block(seed, int(a) * nk + int(b), n, device).view(naux, nao, nao)
 
+    if raw:
+        return R(k1, k2).contiguous()
+
     m1, m2 = int(neg[k1]), int(neg[k2])
     v = R(k1, k2) + R(k2, k1).conj().transpose(1, 2) + R(m1, m2).conj() + R(m2, m1).transpose(1, 2)
     return (0.5 * v).resolve_conj().contiguous()
 
 
-def make_V(cfg, mesh, device="cpu", out=None):
+def make_V(cfg, mesh, device="cpu", out=None, raw=False):
     """Full V[k1][k2][Q][i][j] on `device` (torch complex128).  Fills one orbit of the symmetry group per
-    generated block, so every block is generated once."""
+    generated block, so every block is generated once.  raw=True: every block is its own i.i.d. draw (no symmetry)."""
     nk, nao, naux = mesh.nk, cfg.nao, cfg.naux
     neg = mesh.neg()
     if out is None:
         out = torch.empty((nk, nk, naux, nao, nao), dtype=torch.complex128, device=device)
+    if raw:
+        for k1 in range(nk):
+            for k2 in range(nk):
+                out[k1, k2] = make_V_block(cfg, mesh, k1, k2, device, neg, raw=True)
+        return out
     done = np.zeros((nk, nk), dtype=bool)
     for k1 in range(nk):
         for k2 in range(nk):

@@ -9,7 +9,8 @@
  *   - gw_c128 is layout-compatible with C99 `double complex`, std::complex<double>, cuDoubleComplex,
  *     torch.complex128.  All arrays are dense, row-major, 16-byte aligned.
  *   - "device" pointers are CUDA global memory of the current device; the caller owns every buffer,
- *     the library allocates nothing on the four hot calls, keeps no state between calls and never
+ *     the library allocates nothing on the four hot calls, keeps no state between calls (apart from the cached
+ *     address of the driver's tensor-map encoder, a process-wide constant) and never
  *     frees caller memory.  Inputs are const and unmodified; outputs are fully overwritten.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  The calls only
  *     enqueue work; they never synchronise the host.
@@ -44,7 +45,14 @@ enum {
   GW_EINVAL = -1,   /* null / misaligned pointer, non-positive size, bad q range */
   GW_ENOMEM = -2,   /* workspace too small */
   GW_EARCH = -3,    /* current device is not sm_100 */
-  GW_ESHAPE = -4    /* size outside what the kernels support (nao > 64, ntau or nw > 128) */
+  GW_ESHAPE = -4,   /* size outside what the kernels support; checked before anything is launched and before the workspace
+                       check (gw_workspace_bytes returns 0 for such a problem):
+                         nao > 64;  ntau > 200 or nw > 200 (the paper's range is N_tau = 10-200);
+                         nw > ntau (stage 2 keeps the frequency-domain intermediate in the first nw slices of the Wt buffer);
+                         naux > 896 (stage 1: panel columns = 2 CTAs x 2 column passes x 224; the paper's N_aux/N_orb = 3-10,
+                         PAPER.md:96, gives naux <= 640 at nao = 64) */
+  GW_ENOTPD = -5    /* gw_sigma_iteration_host only: a Cholesky factorisation of I - P0(q, iOmega_n) met a non-positive pivot
+                       (the device calls report that through `info` instead); Sigma / Wt are then not meaningful */
 };
 
 typedef struct {
@@ -89,7 +97,9 @@ int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P0t, void *s
  *   P0w[n] = Σ_t T_wt[n][t] P0t[t];   Ww[n] = (I − P0w[n])^-1 P0w[n]  (Cholesky);   Wt[t] = Σ_n T_tw[t][n] Ww[n]
  *   P0t : device [ntau][nq][naux][naux]    in
  *   Wt  : device [ntau][nq][naux][naux]    out; may alias P0t (then P0t is overwritten)
- *   info: device int32[2] or NULL.  Set to {-1,-1} on success, else {q, n} of one failing factorisation. */
+ *   info: device int32[2], 8-byte aligned, or NULL.  Set to {-1,-1} on success, else {q, n} of ONE failing factorisation:
+ *         the one with the smallest n, then the smallest q (a single 64-bit atomic minimum, so the pair is never mixed
+ *         between two failing matrices and the report is deterministic). */
 int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, void *stream);
 
 /* Stage 2 plus the integrand of the dynamical part of the GW Luttinger-Ward functional, Eq. 37:
@@ -102,7 +112,7 @@ int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P0t, gw_c128
 
 /* Generic imaginary-axis grid transform — the kernel of Eq. 28a / Eq. 30 exposed for the next workflow step, the fermionic
  * τ→iω_n transform of Σ̃ (Eq. 13; Fig. 4 step after the hot path):
- *   Y[o][m] = Σ_i T[o][i] X[i][m],   o < n_out, i < n_in, m < len      (complex T; n_out, n_in <= 128)
+ *   Y[o][m] = Σ_i T[o][i] X[i][m],   o < n_out, i < n_in, m < len      (complex T; n_out, n_in <= 200)
  *   T : device [n_out][n_in];  X : device [n_in][len];  Y : device [n_out][len], may alias X (each column block is read
  *   completely before it is written).  Returns GW_EINVAL / GW_ESHAPE / GW_EARCH or a launch error. */
 int gw_transform(int32_t n_out, int32_t n_in, const gw_c128 *T, const gw_c128 *X, gw_c128 *Y, size_t len, void *stream);
@@ -128,7 +138,8 @@ size_t gw_workspace_bytes(const gw_problem *p);
  * T_wt, T_tw, runs the four stages above on `stream`, downloads Sigma and K, and synchronises the stream.
  * All pointers here (including p->V, p->T_wt, p->T_tw) are HOST memory (pinned memory makes the copies
  * asynchronous).  Device memory is allocated and freed inside the call.  Optional outputs may be NULL:
- *   P0t_out, Wt_out : host [ntau][nq][naux][naux];  stage_ms: host float[6] = H2D, stage 1..4, D2H times (ms). */
+ *   P0t_out, Wt_out : host [ntau][nq][naux][naux];  stage_ms: host float[6] = H2D, stage 1..4, D2H times (ms).
+ * Returns GW_ENOTPD if stage 2 reported a non-positive pivot (the outputs are still copied back), else as the device calls. */
 int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, const gw_c128 *gamma, gw_c128 *Sigma, gw_c128 *K,
                             gw_c128 *P0t_out, gw_c128 *Wt_out, float *stage_ms, void *stream);
 
@@ -142,6 +153,10 @@ int gw_launch_count(const gw_problem *p);
 /* Register-resident DMMA.8x8x4 loop on all SMs for about `ms` milliseconds; returns sustained FP64 TFLOP/s
  * in *tflops (the "measured FP64 peak" the roofline divides by; MEASURED_PEAKS.json has no FP64 entry). */
 int gw_fp64_peak(double ms, double *tflops, void *stream);
+
+/* The same measurement with a register-resident plain DFMA loop (no tensor-core instruction).  The roofline denominator of
+ * bench.py is the larger of the two. */
+int gw_fp64_peak_dfma(double ms, double *tflops, void *stream);
 
 const char *gw_strerror(int code);
 int gw_version(void);

@@ -52,10 +52,11 @@ def lib():
         L.gw_executed_flops.argtypes = [P, ctypes.POINTER(ctypes.c_double)]
         L.gw_launch_count.argtypes = [P]
         L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
+        L.gw_fp64_peak_dfma.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
-                  "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_version"):
+                  "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -258,4 +259,10 @@ def gw_launch_count(prob):
 def gw_fp64_peak(ms=200.0, stream=None):
     out = ctypes.c_double(0.0)
     _check(lib().gw_fp64_peak(ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_fp64_peak")
+    return out.value
+
+
+def gw_fp64_peak_dfma(ms=200.0, stream=None):
+    out = ctypes.c_double(0.0)
+    _check(lib().gw_fp64_peak_dfma(ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_fp64_peak_dfma")
     return out.value

@@ -5,14 +5,19 @@
 #include <string.h>
 #include "gw_common.cuh"
 
+// the current device must be sm_100; queried on every call (microseconds against kernels that run for seconds), so the
+// verdict follows cudaSetDevice
 static int check_arch() {
-  static int cached = 0;
-  if (cached) return cached == 1 ? GW_OK : GW_EARCH;
   int dev = 0, major = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return GW_EARCH; }
   if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return GW_EARCH; }
-  cached = (major == 10) ? 1 : 2;
-  return cached == 1 ? GW_OK : GW_EARCH;
+  return major == 10 ? GW_OK : GW_EARCH;
+}
+
+static int gw_sm_count() {
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) { cudaGetLastError(); nsm = 148; }
+  return nsm;
 }
 
 static bool aligned16(const void *p) { return p && (((uintptr_t)p) & 15) == 0; }
@@ -27,7 +32,7 @@ static int check_problem(const gw_problem *p, bool need_T) {
   if (p->q_begin < 0 || p->q_end > nk || p->q_begin >= p->q_end) return GW_EINVAL;
   if (!aligned16(p->V)) return GW_EINVAL;
   if (need_T && (!aligned16(p->T_wt) || !aligned16(p->T_tw))) return GW_EINVAL;
-  if (p->nao > 64 || p->ntau > 128 || p->nw > 128) return GW_ESHAPE;
+  if (p->nao > GW_MAX_NAO || p->ntau > GW_MAX_NTAU || p->nw > GW_MAX_NTAU || p->nw > p->ntau || p->naux > GW_MAX_NAUX) return GW_ESHAPE;
   return GW_OK;
 }
 
@@ -41,19 +46,16 @@ extern "C" int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P
 
 extern "C" size_t gw_workspace_bytes(const gw_problem *p) {
   if (check_problem(p, false) != GW_OK) return 0;
-  GwDims d = gw_dims(p);
+  // a stage whose planner cannot place the problem answers 0: then the whole problem is refused (never a partial yes)
+  const size_t s[4] = {gw_stage1_workspace(p), gw_stage2_workspace(p), gw_stage3_workspace(p), gw_stage4_workspace(p)};
   size_t m = 0;
-  size_t s;
-  if ((s = gw_stage1_workspace(p)) > m) m = s;
-  if ((s = gw_stage2_workspace(p)) > m) m = s;
-  if ((s = gw_stage3_workspace(p)) > m) m = s;
-  if ((s = gw_stage4_workspace(p)) > m) m = s;
+  for (int i = 0; i < 4; i++) { if (s[i] == 0) return 0; if (s[i] > m) m = s[i]; }
   return (m + 255) / 256 * 256;
 }
 
 extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, void *stream) {
   int rc = check_problem(p, true); if (rc) return rc;
-  if (!aligned16(P0t) || !aligned16(Wt)) return GW_EINVAL;
+  if (!aligned16(P0t) || !aligned16(Wt) || (((uintptr_t)info) & 7)) return GW_EINVAL;
   if (!p->work || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   if ((rc = check_arch())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
@@ -62,7 +64,7 @@ extern "C" int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, 
 
 extern "C" int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, double *phi, void *stream) {
   int rc = check_problem(p, true); if (rc) return rc;
-  if (!aligned16(P0t) || !aligned16(Wt) || !phi || (((uintptr_t)phi) & 7)) return GW_EINVAL;
+  if (!aligned16(P0t) || !aligned16(Wt) || !phi || (((uintptr_t)phi) & 7) || (((uintptr_t)info) & 7)) return GW_EINVAL;
   if (!p->work || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   if ((rc = check_arch())) return rc;
   return gw_launch_stage2(p, (const c128 *)P0t, (c128 *)Wt, info, phi, (cudaStream_t)stream);
@@ -116,6 +118,7 @@ extern "C" int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, co
   const size_t bP = (size_t)d.ntau * d.nq * a2 * 16, bT = (size_t)d.nw * d.ntau * 16;
   c128 *dV = 0, *dG = 0, *dg = 0, *dP = 0, *dS = 0, *dK = 0, *dTwt = 0, *dTtw = 0; void *dW = 0; int32_t *dinfo = 0;
   cudaEvent_t ev[7]; for (int i = 0; i < 7; i++) ev[i] = 0;
+  int32_t hinfo[2] = {-1, -1};
   gw_problem dp = *p;
   size_t wb = 0;
   for (int i = 0; i < 7; i++) CU(cudaEventCreate(&ev[i]));
@@ -145,9 +148,11 @@ extern "C" int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, co
   if (Wt_out) CU(cudaMemcpyAsync(Wt_out, dP, bP, cudaMemcpyDeviceToHost, st));
   CU(cudaMemcpyAsync(Sigma, dS, bG, cudaMemcpyDeviceToHost, st));
   CU(cudaMemcpyAsync(K, dK, bg, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(hinfo, dinfo, 8, cudaMemcpyDeviceToHost, st));
   CU(cudaEventRecord(ev[6], st));
   CU(cudaStreamSynchronize(st));
   if (stage_ms) for (int i = 0; i < 6; i++) CU(cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]));
+  if (hinfo[0] != -1 || hinfo[1] != -1) rc = GW_ENOTPD;
 done:
   cudaFree(dV); cudaFree(dG); cudaFree(dg); cudaFree(dP); cudaFree(dS); cudaFree(dK); cudaFree(dTwt); cudaFree(dTtw); cudaFree(dW); cudaFree(dinfo);
   for (int i = 0; i < 7; i++) if (ev[i]) cudaEventDestroy(ev[i]);
@@ -174,7 +179,7 @@ extern "C" int gw_fp64_peak(double ms, double *tflops, void *stream) {
   if (!tflops || !(ms > 0)) return GW_EINVAL;
   int rc = check_arch(); if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  int dev = 0, nsm = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nsm = gw_sm_count();
   double *out = 0; cudaEvent_t e0 = 0, e1 = 0; float t = 0;
   const int iters = 20000, grid = nsm * 2;
   const double fl = 2.0 * 256 * 8 * (double)iters * 8 * grid;   // per launch
@@ -194,13 +199,54 @@ done:
   return rc;
 }
 
+// ---- the same probe with plain DFMA (no tensor-core instruction): 16 independent chains per thread ----
+__global__ void __launch_bounds__(256) fp64_dfma_kernel(double *out, int iters) {
+  double acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i] = threadIdx.x * 1e-3 + i;
+  const double a = 1.0 - 1e-9 * threadIdx.x, b = 1e-6;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) acc[i] = fma(acc[i], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += acc[i];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int gw_fp64_peak_dfma(double ms, double *tflops, void *stream) {
+  if (!tflops || !(ms > 0)) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nsm = gw_sm_count();
+  double *out = 0; cudaEvent_t e0 = 0, e1 = 0; float t = 0;
+  const int iters = 20000, grid = nsm * 4;
+  const double fl = 2.0 * 256 * 16 * (double)iters * grid;      // per launch
+  int reps = 1;
+  CU(cudaMalloc(&out, sizeof(double) * grid * 256));
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  fp64_dfma_kernel<<<grid, 256, 0, st>>>(out, iters);            // warm-up, ~2.6 ms
+  reps = (int)(ms / 2.6) + 1;
+  CU(cudaEventRecord(e0, st));
+  for (int r = 0; r < reps; r++) fp64_dfma_kernel<<<grid, 256, 0, st>>>(out, iters);
+  CU(cudaEventRecord(e1, st));
+  CU(cudaEventSynchronize(e1));
+  CU(cudaEventElapsedTime(&t, e0, e1));
+  *tflops = fl * reps / (t * 1e-3) * 1e-12;
+done:
+  cudaFree(out); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1);
+  return rc;
+}
+
 extern "C" const char *gw_strerror(int code) {
   switch (code) {
     case GW_OK: return "ok";
     case GW_EINVAL: return "invalid argument (null/misaligned pointer, non-positive size or bad q range)";
     case GW_ENOMEM: return "workspace too small";
     case GW_EARCH: return "current device is not sm_100 (B200)";
-    case GW_ESHAPE: return "size not supported by the kernels (nao > 64, ntau or nw > 128)";
+    case GW_ESHAPE: return "size not supported by the kernels (nao > 64, ntau or nw > 200, nw > ntau, naux > 896)";
+    case GW_ENOTPD: return "I - P0(q, iOmega) is not positive definite (non-positive Cholesky pivot in stage 2)";
     default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown error";
   }
 }

@@ -8,6 +8,11 @@
 
 typedef double2 c128;   // (re, im); layout-compatible with gw_c128
 
+// shape limits of the kernels (GW_ESHAPE, documented in gw.h)
+#define GW_MAX_NAO 64
+#define GW_MAX_NTAU 200
+#define GW_MAX_NAUX 896
+
 struct GwDims {
   int nk1, nk2, nk3, nk;
   int nao, naux, ntau, nw;

@@ -44,6 +44,8 @@ struct Params {
   const c128 *V, *G;
   c128 *P0t, *scratch;
   int cs;                // CTAs per cluster = column splits of the panel
+  int ncp;               // column passes: an item covers cs*8*ntc columns of its Q panel (ncp > 1 only for naux > 448; Z is
+                         // then produced once per pass)
   int nqt, nitems;       // Q tiles per (t,q); total work items
   int nteff;             // tau nodes evaluated: ntau, or ceil(ntau/2) under GW_SYM_TR (the rest is mirrored)
   int herm;              // GW_SYM_TR: P0t[t][q] is Hermitian, only the column tiles up to the panel's diagonal block are computed
@@ -132,11 +134,12 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
 // decode a work item: Q-tile index fastest (a cluster's item sequence cycles through full and ragged panels, so the short,
 // bandwidth-hungry ragged panels are spread over the whole run), then t, then q slowest (concurrent clusters share the V
 // blocks of one q in L2)
-struct Item { int t, ql, Q0, tm_rows; };
+struct Item { int t, ql, Q0, tm_rows, cbase; };   // cbase: first n-tile of the item's column pass (per cluster)
 __device__ __forceinline__ Item decode_item(const Params &P, int item) {
   const GwDims &d = P.d;
   Item it;
-  const int qt = item % P.nqt, r = item / P.nqt;
+  const int qt = item % P.nqt; int r = item / P.nqt;
+  it.cbase = (r % P.ncp) * P.cs * P.ntc; r /= P.ncp;
   it.t = r % P.nteff; it.ql = P.qof(r / P.nteff); it.Q0 = qt * TM; it.tm_rows = min(TM, d.naux - it.Q0);
   return it;
 }
@@ -164,9 +167,6 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
   const int nmain = (n2 + KC - 1) / KC;
   const int rows_cta = TM / cs;                           // panel rows transformed by this CTA's pass warps
   const int r0 = (int)rank * rows_cta;
-  const int col0 = 8 * (int)rank * P.ntc;                 // first Q' column of this CTA
-  const int ncols = max(0, min(naux - col0, 8 * P.ntc));
-  const int ntc_mine = (ncols + 7) / 8;
 
   // zero all dynamic smem once (pad rows/columns must hold finite values: they meet zero operands); init barriers
   {
@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
           const int q = d.q0 + it.ql;
           for (int k = 0; k < d.nk; k++, kit++) {
             const int kq = gw_kadd(d, k, q);
-            const int yB = (kq * d.nk + k) * naux + col0;              // row of V viewed as [nk*nk*naux][nao²]
+            const int yB = (kq * d.nk + k) * naux + 8 * (it.cbase + (int)rank * P.ntc);   // row of V viewed as [nk*nk*naux][nao²]
             const int yA = (cid * 2 + (int)(kit & 1u)) * TM;           // row of the slab area viewed as [2*nclusters*TM][nao²]
             if (cs > 1) gwp::mbar_wait_cluster(zready + (kit & 1u), (kit >> 1) & 1u);
             else gwp::mbar_wait(zready + (kit & 1u), (kit >> 1) & 1u);
@@ -311,6 +311,9 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
     unsigned kit = 0;
     for (int item = cid; item < P.nitems; item += ncl) {
       const Item it = decode_item(P, item);
+      const int col0 = 8 * (it.cbase + (int)rank * P.ntc);    // first Q' column of this CTA in this item
+      const int ncols = max(0, min(naux - col0, 8 * P.ntc));
+      const int ntc_mine = (ncols + 7) / 8;
       const int mtc = (it.tm_rows + 7) / 8;
       // tile ownership.  Full panels: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile.  Ragged last panel
       // (<= 16 rows): all eight warps share m-tiles 0 (and 1), every 8th n-tile each, so the panel costs time in proportion
@@ -423,7 +426,7 @@ static int fill_qirr(const GwDims &d, short *qirr) {
 
 struct Plan {
   int main_off;
-  int cs, ksp_max, nqt, nitems, nteff, nqeff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
+  int cs, ncp, ksp_max, nqt, nitems, nteff, nqeff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
   size_t smem, slab_units, work_bytes;
   bool ok;
 };
@@ -432,8 +435,9 @@ static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
   GwDims d = gw_dims(p);
   pl.nt = (d.naux + 7) / 8;
-  if (pl.nt <= 4 * NJ) pl.cs = 1; else if (pl.nt <= 8 * NJ) pl.cs = 2; else { pl.ok = false; return pl; }
-  pl.ntc = (pl.nt + pl.cs - 1) / pl.cs;
+  pl.cs = pl.nt <= 4 * NJ ? 1 : 2;
+  pl.ncp = (pl.nt + pl.cs * 4 * NJ - 1) / (pl.cs * 4 * NJ);
+  pl.ntc = (pl.nt + pl.cs * pl.ncp - 1) / (pl.cs * pl.ncp);
   pl.ksp = (d.nao + 3) / 4;
   pl.ksp_max = pl.ksp <= 7 ? 7 : (pl.ksp <= 13 ? 13 : 16);
   if (pl.ksp > 16) { pl.ok = false; return pl; }
@@ -443,7 +447,7 @@ static Plan make_plan(const gw_problem *p) {
   pl.nqt = (d.naux + TM - 1) / TM;
   pl.nteff = (d.sym & GW_SYM_TR) ? (d.ntau + 1) / 2 : d.ntau;
   { short tmp[128]; pl.nqeff = fill_qirr(d, tmp); }
-  pl.nitems = pl.nqt * pl.nteff * pl.nqeff;
+  pl.nitems = pl.nqt * pl.ncp * pl.nteff * pl.nqeff;
   pl.main_units = (TM + 8 * pl.ntc) * KC;
   pl.prows = (pl.ksp == pl.ksp_max && pl.ksp_max <= 8) ? 64 : 32;
   pl.pass_units = pl.prows * pl.ldp;
@@ -491,7 +495,7 @@ double gw_stage1_flops(const gw_problem *p) {
       if (rows < 0) rows = 0;
       mt_pass += (rows * d.nao + 7) / 8;
     }
-    const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp;
+    const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp * pl.ncp;
     const int mtc = (tm_rows + 7) / 8;
     // main: warps whose first m-tile is valid execute MT_W m-tiles x their n-tiles x 2 k-steps per job
     const double mtiles = mtc <= 2 ? (double)mtc : (double)((mtc + s1::MT_W - 1) / s1::MT_W) * s1::MT_W;   // ragged panel: narrow ownership
@@ -572,7 +576,7 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   s1::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.cs = pl.cs; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.herm = (P.d.sym & GW_SYM_TR) ? 1 : 0; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
+  P.cs = pl.cs; P.ncp = pl.ncp; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.herm = (P.d.sym & GW_SYM_TR) ? 1 : 0; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
   P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.main_off = pl.main_off; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);

@@ -37,40 +37,43 @@ __global__ void __launch_bounds__(NTHR, 1) transform_kernel(int n_out, int n_in,
     cp_async_commit();
     cp_async_wait<0>();
     __syncthreads();
-    double accr[2][8][2], acci[2][8][2];
+    // output rows in chunks of 128 (two 8-row m-tiles per warp); the column block stays in shared memory
+    for (int oc = 0; oc < n_out; oc += 128) {
+      double accr[2][8][2], acci[2][8][2];
 #pragma unroll
-    for (int i = 0; i < 2; i++)
+      for (int i = 0; i < 2; i++)
 #pragma unroll
-      for (int j = 0; j < 8; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
-    const int o0 = 8 * w + g, o1 = 8 * (w + 8) + g;
-    const bool act0 = 8 * w < n_out, act1 = 8 * (w + 8) < n_out;
-    if (act0) {
-      for (int ks = 0; ks < ksteps; ks++) {
-        const int i = 4 * ks + c;
-        c128 a0 = make_double2(0.0, 0.0), a1 = a0;
-        if (i < n_in) {
-          if (o0 < n_out) a0 = __ldg(T + (size_t)o0 * n_in + i);
-          if (act1 && o1 < n_out) a1 = __ldg(T + (size_t)o1 * n_in + i);
-        }
-        const c128 *brow = sX + i * LDX + g;
+        for (int j = 0; j < 8; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
+      const int o0 = oc + 8 * w + g, o1 = oc + 8 * (w + 8) + g;
+      const bool act0 = oc + 8 * w < n_out, act1 = oc + 8 * (w + 8) < n_out;
+      if (act0) {
+        for (int ks = 0; ks < ksteps; ks++) {
+          const int i = 4 * ks + c;
+          c128 a0 = make_double2(0.0, 0.0), a1 = a0;
+          if (i < n_in) {
+            if (o0 < n_out) a0 = __ldg(T + (size_t)o0 * n_in + i);
+            if (act1 && o1 < n_out) a1 = __ldg(T + (size_t)o1 * n_in + i);
+          }
+          const c128 *brow = sX + i * LDX + g;
 #pragma unroll
-        for (int nt = 0; nt < 8; nt++) {
-          const c128 b = brow[8 * nt];
-          cmma(accr[0][nt], acci[0][nt], a0, b);
-          if (act1) cmma(accr[1][nt], acci[1][nt], a1, b);
+          for (int nt = 0; nt < 8; nt++) {
+            const c128 b = brow[8 * nt];
+            cmma(accr[0][nt], acci[0][nt], a0, b);
+            if (act1) cmma(accr[1][nt], acci[1][nt], a1, b);
+          }
         }
       }
-    }
-    __syncthreads();   // every warp is done reading sX before anyone writes Y (X may alias Y) — and before the next block load
+      // X may alias Y: the whole column block was read into shared memory before the first store of this block
 #pragma unroll
-    for (int h = 0; h < 2; h++) {
-      const int o = h == 0 ? o0 : o1;
-      if ((h == 0 ? act0 : act1) && o < n_out) {
+      for (int h = 0; h < 2; h++) {
+        const int o = h == 0 ? o0 : o1;
+        if ((h == 0 ? act0 : act1) && o < n_out) {
 #pragma unroll
-        for (int nt = 0; nt < 8; nt++) {
-          const int col = 8 * nt + 2 * c;
-          if (col < ncol) Y[(size_t)o * len + m0 + col] = make_double2(accr[h][nt][0], acci[h][nt][0]);
-          if (col + 1 < ncol) Y[(size_t)o * len + m0 + col + 1] = make_double2(accr[h][nt][1], acci[h][nt][1]);
+          for (int nt = 0; nt < 8; nt++) {
+            const int col = 8 * nt + 2 * c;
+            if (col < ncol) Y[(size_t)o * len + m0 + col] = make_double2(accr[h][nt][0], acci[h][nt][0]);
+            if (col + 1 < ncol) Y[(size_t)o * len + m0 + col + 1] = make_double2(accr[h][nt][1], acci[h][nt][1]);
+          }
         }
       }
     }
@@ -281,7 +284,9 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
         update_tiles<true, false, false>(Pm, n, j0, n, sRow, ldn, sBlk, ldn, kst);
       __syncthreads();
     }
-    if (threadIdx.x == 0 && s_bad && P.info) { P.info[0] = P.q0 + mi % P.nq; P.info[1] = mi / P.nq; }
+    // one 64-bit atomic minimum over (n, q): info[0] = q is the low word, info[1] = n the high word; {-1,-1} = all ones
+    if (threadIdx.x == 0 && s_bad && P.info)
+      atomicMin(reinterpret_cast<unsigned long long *>(P.info), ((unsigned long long)(unsigned)(mi / P.nq) << 32) | (unsigned)(P.q0 + mi % P.nq));
     __syncthreads();
   }
 }
@@ -329,7 +334,7 @@ int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *in
   if (!pl.ok) return GW_ESHAPE;
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   GwDims d = gw_dims(p);
-  if (d.nw != d.ntau) return GW_ESHAPE;   // the frequency-domain intermediate lives in the Wt buffer
+  if (d.nw > d.ntau) return GW_ESHAPE;    // the frequency-domain intermediate lives in the first nw slices of the Wt buffer
   const size_t len = (size_t)d.nq * d.naux * d.naux;
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(s2::transform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_t)) != cudaSuccess) return (int)e;
@@ -345,7 +350,7 @@ int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *in
 }
 
 int gw_launch_transform(int n_out, int n_in, const c128 *T, const c128 *X, c128 *Y, size_t len, cudaStream_t st) {
-  if (n_out <= 0 || n_in <= 0 || n_out > 128 || n_in > 128) return GW_ESHAPE;
+  if (n_out <= 0 || n_in <= 0 || n_out > GW_MAX_NTAU || n_in > GW_MAX_NTAU) return GW_ESHAPE;
   const int nsm = gwp::gw_num_sms();
   const size_t nb = (len + s2::NC - 1) / s2::NC;
   if (nb == 0) return GW_OK;

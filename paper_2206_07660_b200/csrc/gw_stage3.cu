@@ -318,8 +318,7 @@ static Plan make_plan(const gw_problem *p) {
     if (pl.nstage >= 3) break;
   }
   if (pl.kh > 2) pl.kh = 2;
-  int dev = 0, nsm = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-  if (nsm <= 0) nsm = 148;
+  const int nsm = gwp::gw_num_sms();
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
   pl.work_bytes = 256 + (size_t)nsm * 2 * pl.slab_units * sizeof(c128);

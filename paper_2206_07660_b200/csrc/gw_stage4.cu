@@ -11,7 +11,7 @@
 
 namespace s4 {
 
-using gwp::NTHR; using gwp::NSTAGE; using gwp::PASS_ROWS;
+using gwp::NTHR; using gwp::PASS_ROWS;
 constexpr int TM = 32;
 
 struct Params {
@@ -20,6 +20,7 @@ struct Params {
   c128 *part, *scratch;
   unsigned *counter;
   int nitems, ldp, ksp, ndt, ldt, stage_units;
+  int nstage;             // cp.async ring depth: 3, or 2 when three stages of the widest job do not fit (nao > 52)
   int kh, kspf, ldpf;     // final jobs: K splits per Q, k-steps per split, row stride of the X part
   size_t slab_units;
 };
@@ -29,6 +30,7 @@ __global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   c128 *smem = reinterpret_cast<c128 *>(smem_raw);
   const GwDims d = P.d;
+  const int NSTAGE = P.nstage;
   const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, ndt = P.ndt, naop = 8 * ndt;
   c128 *sGt = smem;                   // [naop][ldp]: sGt[b][a] = gamma[k'][a][b]
   c128 *sStage = sGt + naop * ldp;
@@ -63,7 +65,7 @@ __global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
         cp_async_commit();
       }
       for (int jb = 0; jb < npass; jb++) {
-        cp_async_wait<NSTAGE - 2>();
+        if (NSTAGE == 3) cp_async_wait<1>(); else cp_async_wait<0>();
         __syncthreads();
         const int nx = jb + NSTAGE - 1;
         if (nx < npass) gwp::issue_pass_job(sStage + (nx % NSTAGE) * P.stage_units, V1t, nx * PASS_ROWS, rows, nao, ldp);
@@ -82,7 +84,7 @@ __global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
         cp_async_commit();
       }
       for (int jb = 0; jb < nfin; jb++) {
-        cp_async_wait<NSTAGE - 2>();
+        if (NSTAGE == 3) cp_async_wait<1>(); else cp_async_wait<0>();
         __syncthreads();
         const int nx = jb + NSTAGE - 1;
         if (nx < nfin) issue_fin(nx);
@@ -107,7 +109,7 @@ __global__ void exchange_reduce_kernel(GwDims d, const c128 *__restrict__ part, 
   K[i] = make_double2(pref * re, pref * im);
 }
 
-struct Plan { gwp::PassGeom g; int nitems, stage_units, grid, kh, kspf, ldpf; size_t smem, slab_units, part_units, work_bytes; bool ok; };
+struct Plan { gwp::PassGeom g; int nitems, stage_units, nstage, grid, kh, kspf, ldpf; size_t smem, slab_units, part_units, work_bytes; bool ok; };
 
 static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
@@ -116,22 +118,25 @@ static Plan make_plan(const gw_problem *p) {
   if (!pl.g.ok) { pl.ok = false; return pl; }
   pl.nitems = d.nk * d.nq;
   const int s_pass = PASS_ROWS * pl.g.ldp;
-  for (pl.kh = 1; pl.kh <= 2; pl.kh++) {     // a final job covers one Q, or half of its K range if a whole Q does not fit
-    pl.kspf = (pl.g.ksp + pl.kh - 1) / pl.kh;
-    int f4 = pl.kspf * 4; if (f4 % 8 == 0) f4 += 4;
-    pl.ldpf = f4;
-    const int s_fin = pl.g.naop * pl.ldpf + 4 * pl.kspf * pl.g.ldt + 8;
-    pl.stage_units = s_pass > s_fin ? s_pass : s_fin;
-    pl.smem = ((size_t)pl.g.naop * pl.g.ldp + (size_t)NSTAGE * pl.stage_units) * sizeof(c128);
-    if (pl.smem <= 227 * 1024) break;
+  // a final job covers one Q, or 1/kh of its K range if a whole Q does not fit; the ring is 3 deep, or 2 for the widest bases
+  pl.ok = false;
+  for (pl.nstage = 3; pl.nstage >= 2 && !pl.ok; pl.nstage--) {
+    for (pl.kh = 1; pl.kh <= 2; pl.kh++) {
+      pl.kspf = (pl.g.ksp + pl.kh - 1) / pl.kh;
+      int f4 = pl.kspf * 4; if (f4 % 8 == 0) f4 += 4;
+      pl.ldpf = f4;
+      const int s_fin = pl.g.naop * pl.ldpf + 4 * pl.kspf * pl.g.ldt + 8;
+      pl.stage_units = s_pass > s_fin ? s_pass : s_fin;
+      pl.smem = ((size_t)pl.g.naop * pl.g.ldp + (size_t)pl.nstage * pl.stage_units) * sizeof(c128);
+      if (pl.smem <= 227 * 1024) { pl.ok = true; break; }
+    }
+    if (pl.ok) break;
   }
-  if (pl.kh > 2) pl.kh = 2;
   const int nsm = gwp::gw_num_sms();
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
   pl.part_units = (size_t)d.nq * d.nk * d.nao * d.nao;
   pl.work_bytes = 256 + ((size_t)nsm * pl.slab_units + pl.part_units) * sizeof(c128);
-  pl.ok = pl.smem <= 227 * 1024;
   return pl;
 }
 
@@ -172,7 +177,7 @@ int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream
   P.scratch = (c128 *)((char *)p->work + 256);
   P.part = P.scratch + (size_t)gwp::gw_num_sms() * pl.slab_units;
   P.nitems = pl.nitems; P.ldp = pl.g.ldp; P.ksp = pl.g.ksp; P.ndt = pl.g.ndt; P.ldt = pl.g.ldt; P.kh = pl.kh; P.kspf = pl.kspf; P.ldpf = pl.ldpf;
-  P.stage_units = pl.stage_units; P.slab_units = pl.slab_units;
+  P.stage_units = pl.stage_units; P.nstage = pl.nstage; P.slab_units = pl.slab_units;
   cudaError_t e = cudaMemsetAsync(p->work, 0, 256, st);
   if (e != cudaSuccess) return (int)e;
   int rc;

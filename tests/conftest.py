@@ -35,6 +35,22 @@ def problems():
     return get
 
 
+_raw_cache = {}
+
+
+@pytest.fixture(scope="session")
+def raw_problems():
+    """Seeded problems with NO input symmetry (gwgen.make_problem(raw=True)): independent V blocks, non-Hermitian G, gamma, W."""
+    import gwgen
+
+    def get(name):
+        if name not in _raw_cache:
+            _raw_cache[name] = gwgen.make_problem(name, raw=True)
+        return _raw_cache[name]
+
+    return get
+
+
 _oracle_cache = {}
 
 

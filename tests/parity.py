@@ -16,6 +16,20 @@ def worst_slice(a, b, lead=2):
     return float(np.max(num / np.maximum(den, 1e-300)))
 
 
+def max_elem(a, b):
+    """largest element-wise |a - b| relative to the largest |b| of the array (reported next to the Frobenius numbers so that a
+    regression confined to one tile is visible; not gated)."""
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.max(np.abs(a - b)) / max(float(np.max(np.abs(b))), 1e-300))
+
+
+def report(tag, key, got, ref):
+    """relative Frobenius error (the gated number), printed with the worst element."""
+    e = relerr(got, ref)
+    print(f"parity {tag} {key}: rel Frobenius {e:.2e}, max element |d|/max|ref| {max_elem(got, ref):.2e}")
+    return e
+
+
 def device_problem(p, q_begin=0, q_end=None, device="cuda", symmetry=0):
     import paper_2206_07660_b200 as gw
     cfg = p.cfg

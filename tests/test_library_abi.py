@@ -41,6 +41,7 @@ def test_strerror_and_version(gwlib):
     assert gwlib.gw_version() >= 100
     assert gwlib.gw_strerror(0) == "ok"
     assert "sm_100" in gwlib.gw_strerror(-3)
+    assert "nw > ntau" in gwlib.gw_strerror(-4) and "positive definite" in gwlib.gw_strerror(-5)
 
 
 def test_validation_without_device(gwlib):
@@ -57,6 +58,15 @@ def test_validation_without_device(gwlib):
     c.q_begin = 0; c.q_end = 8; c.nao = 80
     assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4096), ctypes.c_void_p(4096), None) == -4   # GW_ESHAPE
     c.nao = 26
+    # every documented GW_ESHAPE condition (gw.h), refused before any launch; the workspace query answers 0 for them
+    for field, bad, good in (("ntau", 201, 104), ("nw", 105, 104), ("naux", 897, 100), ("nao", 65, 26)):
+        setattr(c, field, bad)
+        assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4096), ctypes.c_void_p(4096), None) == -4, field
+        assert L.gw_workspace_bytes(ctypes.byref(c)) == 0, field
+        setattr(c, field, good)
+    c.ntau = 200; c.nw = 150; c.naux = 896; c.nao = 64          # the documented maxima are accepted by the planner
+    assert L.gw_workspace_bytes(ctypes.byref(c)) > 0
+    c.ntau = 104; c.nw = 104; c.naux = 100; c.nao = 26
     assert L.gw_polarization(ctypes.byref(c), ctypes.c_void_p(4097), ctypes.c_void_p(4096), None) == -1  # misaligned
     assert L.gw_workspace_bytes(ctypes.byref(c)) > 0
     assert L.gw_launch_count(ctypes.byref(c)) == 8
@@ -80,3 +90,18 @@ def test_product_path_does_not_import_oracle():
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_2206_07660_b200" not in txt.replace("paper_2206_07660_b200/csrc", ""), f
+
+
+def test_every_documented_shape_is_plannable(gwlib):
+    """gw.h documents nao <= 64, naux <= 896, nw <= ntau <= 200: the planners of all four stages must place every such problem
+    (gw_workspace_bytes answers 0 as soon as one stage cannot)."""
+    from paper_2206_07660_b200.binding import _CProblem
+    L = gwlib.lib()
+    bad = []
+    for nao in range(1, 65):
+        for naux in (1, 37, 200, 448, 449, 640, 896):
+            for ntau, nw in ((8, 8), (200, 200), (200, 13)):
+                c = _CProblem(2, 1, 3, nao, naux, ntau, nw, 2, 0, 6, 10.0, 4096, 4096, 4096, None, 0)
+                if L.gw_workspace_bytes(ctypes.byref(c)) == 0:
+                    bad.append((nao, naux, ntau, nw))
+    assert not bad, bad[:10]

@@ -344,3 +344,75 @@ def test_P12_fermionic_transform_closed_form(oracle_lib):
     ref = 1.0 / (1j * f["omega"][:, None] - eps[None, :])
     assert np.max(np.abs(got - ref) / np.abs(ref)) < 1e-9
     assert np.allclose(got, np.tensordot(f["T_wt_f"], G, axes=(1, 0)), rtol=1e-13, atol=0)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# Raw-input pins (no symmetry in V, G, gamma, W): the printed index patterns of Eq. 22 / 28b / 31 are told apart from
+# their symmetric twins.  On the BASELINE inputs V[k+q][k]_bc = conj V[k][k+q]_cb and G = G^+, so an oracle that read the
+# conjugate-transposed block, or G^+ in place of G, would pass P2-P10 above; on raw inputs it fails by O(1).
+# ----------------------------------------------------------------------------------------------------------------
+def _raw_oracle(oracle_lib, p):
+    cfg = p.cfg
+    vb = oracle_lib.VBlocks(cfg, p.V.numpy())
+    P0t = oracle_lib.polarization(cfg, vb, p.G)
+    Sg = oracle_lib.selfenergy(cfg, vb, p.G, p.extras["W"])
+    K = oracle_lib.exchange(cfg, vb, p.gamma)
+    return vb, P0t, Sg, K
+
+
+def test_raw_inputs_have_no_symmetry(raw_problems):
+    p = raw_problems("T")
+    V = p.V.numpy()
+    neg = p.mesh.neg()
+    assert relerr(V[1, 2], np.conj(np.swapaxes(V[2, 1], -1, -2))) > 0.5          # no pair symmetry
+    assert relerr(V[neg[1], neg[2]], np.conj(V[1, 2])) > 0.5                      # no time reversal
+    assert relerr(p.G, np.conj(np.swapaxes(p.G, -1, -2))) > 0.5                   # G not Hermitian
+    assert relerr(p.extras["W"], np.conj(np.swapaxes(p.extras["W"], -1, -2))) > 0.5
+
+
+def test_P10_literal_einsum_raw(raw_problems, oracle_lib):
+    """Eq. 28b / 31 / 22 exactly as printed, 4-index einsum with the generator's tables,
+    on symmetry-free inputs; and the symmetric twins are shown to differ, so the pin bites."""
+    p = raw_problems("T")
+    cfg = p.cfg
+    vb, P0t, Sg, K = _raw_oracle(oracle_lib, p)
+    V, G, W = p.V.numpy(), p.G, p.extras["W"]
+    add, sub = p.mesh.add_table(), p.mesh.sub_table()
+    N, nk = cfg.ntau, cfg.nk
+    lit = np.zeros_like(P0t); twin_V = np.zeros_like(P0t); twin_G = np.zeros_like(P0t)
+    for t in range(N):
+        for q in range(nk):
+            for k in range(nk):
+                kq = add[k][q]
+                lit[t, q] += np.einsum("Qda,cd,ab,Pbc->QP", V[k, kq], G[N - 1 - t, k], G[t, kq], V[kq, k])
+                twin_V[t, q] += np.einsum("Qda,cd,ab,Pcb->QP", V[k, kq], G[N - 1 - t, k], G[t, kq], V[k, kq].conj())
+                twin_G[t, q] += np.einsum("Qda,dc,ab,Pbc->QP", V[k, kq], G[N - 1 - t, k].conj(), G[t, kq], V[kq, k])
+    pref = -cfg.spin_deg / nk
+    assert relerr(P0t, pref * lit) < 1e-13
+    assert relerr(P0t, pref * twin_V) > 0.5 and relerr(P0t, pref * twin_G) > 0.5
+    S = np.zeros_like(Sg); S_twin = np.zeros_like(Sg); Kl = np.zeros_like(K); K_twin = np.zeros_like(K)
+    for k in range(nk):
+        for q in range(nk):
+            km = sub[k][q]
+            for t in range(N):
+                S[t, k] += np.einsum("ab,Qia,QP,Pbj->ij", G[t, km], V[k, km], W[t, q], V[km, k])
+                S_twin[t, k] += np.einsum("ab,Qia,PQ,Pbj->ij", G[t, km], V[k, km], W[t, q], V[km, k])     # W transposed
+            Kl[k] += np.einsum("Qia,ab,Qbj->ij", V[k, km], p.gamma[km], V[km, k])
+            K_twin[k] += np.einsum("Qia,ab,Qjb->ij", V[k, km], p.gamma[km], V[k, km].conj())            # V[k'][k] -> V[k][k']^+
+    assert relerr(Sg, -S / nk) < 1e-13 and relerr(Sg, -S_twin / nk) > 0.5
+    assert relerr(K, -Kl / nk) < 1e-13 and relerr(K, -K_twin / nk) > 0.5
+
+
+@pytest.mark.parametrize("name", ["T", "R"])
+def test_P7_P9_raw(raw_problems, oracle_lib, name):
+    """Trace identity (P7) and exchange limit (P9) hold for ARBITRARY inputs: checked on the symmetry-free ones."""
+    p = raw_problems(name)
+    cfg = p.cfg
+    vb, P0t, Sg, K = _raw_oracle(oracle_lib, p)
+    lhs = np.einsum("tkij,tkji->t", Sg, p.G[::-1])
+    rhs = np.einsum("tqab,tqba->t", p.extras["W"], P0t[::-1]) / cfg.spin_deg
+    assert np.max(np.abs(lhs - rhs) / np.abs(rhs)) < 1e-11
+    I = np.ascontiguousarray(np.broadcast_to(np.eye(cfg.naux, dtype=complex), (cfg.nk, cfg.naux, cfg.naux)))
+    for k in (0, cfg.nk - 1):
+        S = oracle_lib.sigma_slice(cfg, vb, np.ascontiguousarray(-p.gamma), I, k)
+        assert relerr(S, -K[k]) < 1e-13
