@@ -15,11 +15,11 @@ not available offline; see DESIGN.md "Input recipe".
 """
 from .configs import CONFIGS, GWConfig, get_config
 from .mesh import KMesh
-from .grids import make_grids, make_fermionic_transform
-from .fock import make_fock, greens_function, density_matrix
+from .grids import make_grids, make_fermionic_transform, make_fermionic_grids
+from .fock import make_fock, greens_function, density_matrix, make_h0_s
 from .vgen import make_V, make_V_block
 from .problem import make_problem, Problem
 
-__all__ = ["CONFIGS", "GWConfig", "get_config", "KMesh", "make_grids", "make_fermionic_transform", "make_fock",
+__all__ = ["CONFIGS", "GWConfig", "get_config", "KMesh", "make_grids", "make_fermionic_transform", "make_fermionic_grids", "make_h0_s", "make_fock",
            "greens_function", "density_matrix", "make_V", "make_V_block",
            "make_problem", "Problem"]

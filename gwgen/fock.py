@@ -62,3 +62,26 @@ def density_matrix(eps, U, beta):
     """γ[k][i][j] complex128."""
     f = fermi(eps, beta)
     return np.ascontiguousarray(np.einsum("kin,kn,kjn->kij", U, f, U.conj()))
+
+
+def make_h0_s(cfg, mesh, eps, U):
+    """One-electron Hamiltonian H0[k] and overlap S[k] for the loop closure (Eq. 15-16): the paper takes them from
+    PySCF; here H0[k] = U diag(eps) U^+ (the Fock spectrum that also built G) and S[k] = Q diag(s) Q^+ with seeded
+    s in [0.6, 1.4] (a non-orthogonal basis, Hermitian positive definite), both time-reversal symmetric: X[-k] = conj X[k]."""
+    rng = np.random.default_rng([cfg.seed, 3])
+    nk, nao = mesh.nk, cfg.nao
+    neg = mesh.neg()
+    H0 = np.einsum("kin,kn,kjn->kij", U, eps, U.conj())
+    S = np.zeros((nk, nao, nao), dtype=np.complex128)
+    for k in range(nk):
+        if k > neg[k]:
+            continue
+        A = rng.normal(size=(nao, nao))
+        if neg[k] != k:
+            A = A + 1j * rng.normal(size=(nao, nao))
+        Q, _ = np.linalg.qr(A)
+        sv = rng.uniform(0.6, 1.4, nao)
+        Sk = (Q * sv[None, :]) @ Q.conj().T
+        S[k] = 0.5 * (Sk + Sk.conj().T)
+        S[neg[k]] = S[k].conj()
+    return np.ascontiguousarray(H0), np.ascontiguousarray(S)

@@ -88,3 +88,43 @@ def make_fermionic_transform(ntau, beta, nw=None):
     om = (2 * S + 1) * np.pi / beta
     If = np.array([(beta / 2) * (Tg * (wg * np.exp(1j * w * beta * (1.0 + xg) / 2))).sum(1) for w in om])
     return {"nfer": S, "omega": om, "T_wt_f": np.ascontiguousarray((If @ C).astype(np.complex128))}
+
+
+def make_fermionic_grids(ntau, beta):
+    """Fermionic companions of make_grids on the SAME Chebyshev-Gauss tau nodes, for the loop closure (Eq. 13-16, PAPER.md:110-129;
+    Fig. 4 steps 3-4).  All four are *inputs* of the C ABI (gw_fermi_grid); kernels and oracle only apply them.
+
+      nfer[nwf]      nwf = 2*(ntau//2) Matsubara indices, symmetric under n <-> -n-1 (omega_n <-> -omega_n): the non-negative half
+                     is bosonic_set(ntau//2) read as fermionic indices
+      omega[nwf]     omega_n = (2n+1) pi / beta
+      T_wt_f[nwf][ntau]  tau -> i omega_n (Eq. 13): Chebyshev analysis with all ntau polynomials, then the exact integrals
+                         I_f[n][j] = (beta/2) int_-1^1 T_j(x) e^{i omega_n beta (1+x)/2} dx  (Gauss-Legendre)
+      T_tw_f[ntau][nwf]  i omega_n -> tau (Eq. 14) by least squares on the first L = 2*ntau//3 polynomials: T_L(x_t)^T pinv(I_f[:, :L]).
+                         The integrals carry the 1/(i omega_n) tail of a fermionic function exactly (boundary terms of a polynomial),
+                         so no separate tail treatment is needed.
+      t_beta[nwf]        G(tau = beta^-) = sum_n t_beta[n] G(i omega_n)   (the same fit evaluated at x = +1; gamma = -G(beta^-))
+      e_beta[ntau]       G(tau = beta^-) = sum_t e_beta[t] G(tau_t)       (Chebyshev interpolation from the nodes to x = +1)
+    """
+    N = ntau
+    half = max(N // 2, 1)
+    pos = bosonic_set(half)[:half] if half >= 3 else np.arange(half, dtype=np.int64)
+    S = np.concatenate([-(pos[::-1]) - 1, pos]).astype(np.int64)
+    L = max((2 * N) // 3, 1)
+    t = np.arange(N)
+    x = -np.cos(np.pi * (2 * t + 1) / (2 * N))
+    j = np.arange(N)
+    Tt = np.cos(np.outer(j, np.arccos(x)))
+    C = Tt * (2.0 / N)
+    C[0] *= 0.5
+    M = 2 * N + 2 * int(np.abs(S).max()) + 300
+    xg, wg = np.polynomial.legendre.leggauss(M)
+    Tg = np.cos(np.outer(j, np.arccos(xg)))
+    om = (2 * S + 1) * np.pi / beta
+    If = np.array([(beta / 2) * (Tg * (wg * np.exp(1j * w * beta * (1.0 + xg) / 2))).sum(1) for w in om])
+    pin = np.linalg.pinv(If[:, :L])
+    cond = np.linalg.cond(If[:, :L])
+    if not cond < 1e6:
+        raise RuntimeError(f"ill-conditioned fermionic sampling set: cond={cond:.3e}")
+    cc = lambda a: np.ascontiguousarray(np.asarray(a).astype(np.complex128))
+    return {"nfer": S, "omega": np.ascontiguousarray(om.astype(np.float64)), "T_wt_f": cc(If @ C), "T_tw_f": cc(Tt[:L].T @ pin),
+            "t_beta": cc(np.ones(L) @ pin), "e_beta": cc(C.sum(axis=0)), "cond": cond}

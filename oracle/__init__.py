@@ -37,9 +37,11 @@ def lib():
         for name in ("gwref_kadd", "gwref_ksub", "gwref_p0t_slice", "gwref_polarization", "gwref_dyson",
                      "gwref_screened_interaction_q", "gwref_screened_interaction", "gwref_sigma_slice",
                      "gwref_selfenergy", "gwref_exchange_slice", "gwref_exchange", "gwref_sigma_slice_qrange",
-                     "gwref_exchange_slice_qrange"):
+                     "gwref_exchange_slice_qrange", "gwref_hartree", "gwref_dyson_update_one", "gwref_dyson_update", "gwref_find_mu"):
             getattr(_lib, name).restype = ctypes.c_int
         _lib.gwref_transform.restype = None
+        _lib.gwref_electron_count.restype = ctypes.c_double
+        _lib.gwref_axpby.restype = None
     return _lib
 
 
@@ -194,3 +196,81 @@ def exchange(cfg, vb, gamma):
     if lib().gwref_exchange(ctypes.byref(d), vb.table, _p(gamma), _p(out)):
         raise RuntimeError("oracle: a needed V block is not resident")
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# loop closure (Fig. 4, Eq. 15, 16, 20)
+# ---------------------------------------------------------------------------------------------------------------------
+def _pd(a):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def hartree(cfg, vb, gamma):
+    """Eq. 20: J[k][i][j]."""
+    out = np.empty((cfg.nk, cfg.nao, cfg.nao), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_hartree(ctypes.byref(d), vb.table, _p(gamma), _p(out)):
+        raise RuntimeError("oracle: a needed V block is not resident")
+    return out
+
+
+def dyson_update(cfg, omega, mu, S, F, Sigma_w=None):
+    """Eq. 16 for all (n, k): G_w[n][k] = [(i omega_n + mu) S[k] - F[k] - Sigma_w[n][k]]^-1."""
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    out = np.empty((len(omega), cfg.nk, cfg.nao, cfg.nao), np.complex128)
+    d = _dims(cfg)
+    if lib().gwref_dyson_update(ctypes.byref(d), len(omega), _pd(omega), ctypes.c_double(mu), _p(S), _p(F),
+                                _p(Sigma_w) if Sigma_w is not None else None, _p(out)):
+        raise RuntimeError("oracle: zero pivot")
+    return out
+
+
+def electron_count(cfg, t_beta, S, G_w):
+    """Eq. 15 with gamma = -G(beta^-) = -sum_n t_beta[n] G_w[n]."""
+    d = _dims(cfg)
+    return float(lib().gwref_electron_count(ctypes.byref(d), G_w.shape[0], _p(t_beta), _p(S), _p(G_w)))
+
+
+def find_mu(cfg, omega, t_beta, S, F, Sigma_w, n_target, mu_lo, mu_hi, mu_tol=1e-12):
+    """Bisection for the chemical potential (Fig. 4 step 3).  Returns (mu, N_e(mu))."""
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    scratch = np.empty((len(omega), cfg.nk, cfg.nao, cfg.nao), np.complex128)
+    mu, ne = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    d = _dims(cfg)
+    rc = lib().gwref_find_mu(ctypes.byref(d), len(omega), _pd(omega), _p(t_beta), _p(S), _p(F),
+                             _p(Sigma_w) if Sigma_w is not None else None, ctypes.c_double(n_target), ctypes.c_double(mu_lo),
+                             ctypes.c_double(mu_hi), ctypes.c_double(mu_tol), _p(scratch), ctypes.byref(mu), ctypes.byref(ne))
+    if rc:
+        raise RuntimeError(f"oracle: chemical-potential search failed (code {rc})")
+    return mu.value, ne.value
+
+
+def axpby(a, X, b, Y):
+    """Y <- a X + b Y."""
+    class C(ctypes.Structure):
+        _fields_ = [("re", ctypes.c_double), ("im", ctypes.c_double)]
+    assert X.shape == Y.shape
+    lib().gwref_axpby.argtypes = [ctypes.c_size_t, C, ctypes.c_void_p, C, ctypes.c_void_p]
+    lib().gwref_axpby(X.size, C(complex(a).real, complex(a).imag), _p(X), C(complex(b).real, complex(b).imag), _p(Y))
+    return Y
+
+
+def scgw_iteration(cfg, vb, T_wt, T_tw, fg, H0, S, G, n_target, mu_lo, mu_hi, alpha=1.0, mu_tol=1e-12):
+    """One scGW iteration in the order of Fig. 4: G(tau) -> Sigma_inf (Eq. 20, 22), Sigma~(tau) (Alg. 1) ->
+    Sigma~(i omega_n) (Eq. 13) -> mu (Eq. 15) -> G(i omega_n) (Eq. 16) -> G(tau) (Eq. 14) -> damping.  fg = gwgen.make_fermionic_grids(...).
+    Every step is one of the oracle's C routines; this function only sequences them."""
+    Gb = transform(fg["e_beta"].reshape(1, -1), G)[0]                         # G(beta^-)
+    gamma = axpby(-1.0, Gb, 0.0, np.zeros_like(Gb))                            # gamma = -G(beta^-)  (PAPER.md:118)
+    J = hartree(cfg, vb, gamma)
+    K = exchange(cfg, vb, gamma)
+    P0t = polarization(cfg, vb, G)
+    Wt = screened_interaction(cfg, T_wt, T_tw, P0t)
+    Sigma_t = selfenergy(cfg, vb, G, Wt)
+    Sigma_w = transform(fg["T_wt_f"], Sigma_t)
+    F = axpby(1.0, J, 1.0, axpby(1.0, K, 1.0, H0.copy()))                      # F = H0 + K + J  (Eq. 17-18)
+    mu, ne = find_mu(cfg, fg["omega"], fg["t_beta"], S, F, Sigma_w, n_target, mu_lo, mu_hi, mu_tol)
+    G_w = dyson_update(cfg, fg["omega"], mu, S, F, Sigma_w)
+    G_new = transform(fg["T_tw_f"], G_w)
+    G_mix = axpby(alpha, G_new, 1.0 - alpha, G.copy())
+    return dict(gamma=gamma, J=J, K=K, P0t=P0t, Wt=Wt, Sigma_t=Sigma_t, Sigma_w=Sigma_w, F=F, mu=mu, ne=ne, G_w=G_w, G_new=G_new, G=G_mix)

@@ -16,6 +16,8 @@
  *           for k { read V(k,k-q); for tau: Eq. 31 } }   -> gwref_sigma_slice
  *   Eq. 22 (static exchange)                             -> gwref_exchange_slice
  *   Eq. 37 summand tr{ln[I - P0(iOmega)] + P0(iOmega)}   -> gwref_phi
+ *   loop closure (Fig. 4): Eq. 20 -> gwref_hartree; Eq. 16 -> gwref_dyson_update; Eq. 15 -> gwref_electron_count;
+ *   chemical potential -> gwref_find_mu
  *
  * No blocking, fusion or reordering beyond the temporaries A, B, X, Y named in
  * SURVEY.md §8(c); the linear solve is Gaussian elimination with partial pivoting
@@ -39,7 +41,9 @@
  * Parity pins: tests/test_oracle_pins.py (closed form P1, Lindhard P2, invariants P3-P5,
  * brute-force Matsubara sum P6, trace identity P7, solve residual P8, exchange limit P9,
  * literal 4-index evaluation P10, scalar form / series / eigenvalue route of the Eq. 37 summand P11, fermionic
- * transform of a single pole P12).
+ * transform of a single pole P12; loop closure: non-interacting closed form of Eq. 16 in the generalised eigenbasis P13,
+ * Fermi-function electron count and root of the chemical-potential search P14, literal einsum of Eq. 20 P15,
+ * back transform of a single pole P16).
  * Nothing here is "parity unpinned".
  */
 #include <complex.h>
@@ -371,6 +375,141 @@ int gwref_exchange(const gwref_dims *d, const c128 *const *Vblk, const c128 *gam
 #pragma omp parallel for schedule(dynamic) reduction(| : bad)
   for (int k = 0; k < nk; k++) bad |= gwref_exchange_slice(d, Vblk, gamma, k, K + (size_t)k * n2);
   return bad;
+}
+
+/* =====================================================================================================================
+ * Loop closure: the rest of one scGW iteration, Fig. 4 steps 1, 3, 4.
+ * Same rules as above: plain loops, the paper's order, no symmetry used.
+ * ===================================================================================================================== */
+
+/* ---- Hartree term, Eq. 20 (the printed label "(19)" is lost in the text, the second line is Eq. 20):
+ *   J[k][i][j] = (1/N_k) sum_k' sum_sigma1 sum_ab sum_Q V^{kk}_{ij}(Q) gamma^{k'}_{a sigma1, b sigma1} V^{k'k'}_{ba}(Q)
+ * gamma: [nk][nao][nao] per spin channel; the sum over sigma1 of a closed shell is the factor spin_deg (reading R3).
+ * Only the diagonal blocks V[k][k] are read.  Returns 1 if one of them is missing. */
+int gwref_hartree(const gwref_dims *d, const c128 *const *Vblk, const c128 *gamma, c128 *J) {
+  const int nk = d->nk1 * d->nk2 * d->nk3, nao = d->nao, naux = d->naux;
+  const size_t n2 = (size_t)nao * nao;
+  for (int k = 0; k < nk; k++) if (!Vblk[(size_t)k * nk + k]) return 1;
+  for (int k = 0; k < nk; k++)
+    for (int i = 0; i < nao; i++)
+      for (int j = 0; j < nao; j++) {
+        c128 s = 0;
+        for (int kp = 0; kp < nk; kp++) {
+          const c128 *Vkk = Vblk[(size_t)k * nk + k], *Vpp = Vblk[(size_t)kp * nk + kp], *g = gamma + (size_t)kp * n2;
+          for (int a = 0; a < nao; a++)
+            for (int b = 0; b < nao; b++)
+              for (int Q = 0; Q < naux; Q++) s += Vkk[Q * n2 + i * nao + j] * g[a * nao + b] * Vpp[Q * n2 + b * nao + a];
+        }
+        J[(size_t)k * n2 + i * nao + j] = (double)d->spin_deg / (double)nk * s;
+      }
+  return 0;
+}
+
+/* ---- Dyson equation, Eq. 16, one (k, i omega_n):
+ *   G = [ (i omega_n + mu) S - F - Sigma_w ]^-1,   F = H0 + Sigma_inf (static part, Eq. 17-18), Sigma_w = Sigma~(i omega_n) or NULL
+ * "The inverse is defined as a matrix inversion in spin-orbital space": Gaussian elimination with partial
+ * pivoting on [A | I], then back substitution.  Returns 1 on a zero pivot. */
+int gwref_dyson_update_one(int n, double omega, double mu, const c128 *S, const c128 *F, const c128 *Sigma_w, c128 *G) {
+  c128 *A = (c128 *)malloc(sizeof(c128) * n * n);
+  const c128 z = mu + I * omega;
+  for (int i = 0; i < n; i++)
+    for (int j = 0; j < n; j++) {
+      A[(size_t)i * n + j] = z * S[(size_t)i * n + j] - F[(size_t)i * n + j] - (Sigma_w ? Sigma_w[(size_t)i * n + j] : 0);
+      G[(size_t)i * n + j] = (i == j) ? 1.0 : 0.0;
+    }
+  int fail = 0;
+  for (int c = 0; c < n && !fail; c++) {
+    int p = c;
+    double best = cabs(A[(size_t)c * n + c]);
+    for (int r = c + 1; r < n; r++) { double v = cabs(A[(size_t)r * n + c]); if (v > best) { best = v; p = r; } }
+    if (best == 0.0) { fail = 1; break; }
+    if (p != c)
+      for (int j = 0; j < n; j++) {
+        c128 t = A[(size_t)c * n + j]; A[(size_t)c * n + j] = A[(size_t)p * n + j]; A[(size_t)p * n + j] = t;
+        t = G[(size_t)c * n + j]; G[(size_t)c * n + j] = G[(size_t)p * n + j]; G[(size_t)p * n + j] = t;
+      }
+    for (int r = c + 1; r < n; r++) {
+      const c128 f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+      if (f == 0) continue;
+      for (int j = c; j < n; j++) A[(size_t)r * n + j] -= f * A[(size_t)c * n + j];
+      for (int j = 0; j < n; j++) G[(size_t)r * n + j] -= f * G[(size_t)c * n + j];
+    }
+  }
+  if (!fail)
+    for (int c = n - 1; c >= 0; c--)
+      for (int j = 0; j < n; j++) {
+        c128 s = G[(size_t)c * n + j];
+        for (int r = c + 1; r < n; r++) s -= A[(size_t)c * n + r] * G[(size_t)r * n + j];
+        G[(size_t)c * n + j] = s / A[(size_t)c * n + c];
+      }
+  free(A);
+  return fail;
+}
+
+/* Eq. 16 for all (n, k).  S, F: [nk][nao][nao]; Sigma_w, G_w: [nwf][nk][nao][nao] (Sigma_w may be NULL); omega: [nwf]. */
+int gwref_dyson_update(const gwref_dims *d, int nwf, const double *omega, double mu, const c128 *S, const c128 *F,
+                       const c128 *Sigma_w, c128 *G_w) {
+  const int nk = d->nk1 * d->nk2 * d->nk3, nao = d->nao;
+  const size_t n2 = (size_t)nao * nao;
+  int fail = 0;
+#pragma omp parallel for collapse(2) schedule(dynamic) reduction(| : fail)
+  for (int n = 0; n < nwf; n++)
+    for (int k = 0; k < nk; k++)
+      fail |= gwref_dyson_update_one(nao, omega[n], mu, S + k * n2, F + k * n2,
+                                     Sigma_w ? Sigma_w + ((size_t)n * nk + k) * n2 : NULL, G_w + ((size_t)n * nk + k) * n2);
+  return fail;
+}
+
+/* ---- Electron count, Eq. 15:  N_e = (1/N_k) sum_k tr[gamma^k S^k] over spin orbitals, gamma^k = -G^k(tau = beta^-).
+ * G(beta^-) is obtained from the sampled G(i omega_n) with the given evaluation vector: G(beta^-) = sum_n t_beta[n] G_w[n]
+ * (reading R6: the grids and their maps are inputs).  The spin trace of a closed shell is the factor spin_deg. */
+double gwref_electron_count(const gwref_dims *d, int nwf, const c128 *t_beta, const c128 *S, const c128 *G_w) {
+  const int nk = d->nk1 * d->nk2 * d->nk3, nao = d->nao;
+  const size_t n2 = (size_t)nao * nao;
+  c128 tot = 0;
+  for (int k = 0; k < nk; k++)
+    for (int i = 0; i < nao; i++)
+      for (int j = 0; j < nao; j++) {
+        c128 gb = 0;                                              /* G^k_ij(beta^-) */
+        for (int n = 0; n < nwf; n++) gb += t_beta[n] * G_w[((size_t)n * nk + k) * n2 + i * nao + j];
+        tot += -gb * S[(size_t)k * n2 + j * nao + i];             /* tr[gamma S] = sum_ij gamma_ij S_ji */
+      }
+  return (double)d->spin_deg / (double)nk * creal(tot);
+}
+
+/* ---- Chemical potential (Fig. 4 step 3): adjust mu until N_e(mu) equals n_target ("threshold value of 1e-9").
+ * Bisection on the monotone function N_e(mu) of Eq. 15-16 (reading R16):
+ *   1. widen [lo, hi] by its own width (at most 60 times) until N_e(lo) <= n_target <= N_e(hi);
+ *   2. halve it until hi - lo <= mu_tol (at most 200 times): mid goes to lo if N_e(mid) < n_target, else to hi;
+ *   3. mu = (lo + hi)/2; *ne_out = N_e(mu).
+ * Returns 0; 1 if a pivot vanished; 2 if no bracket was found.  Gw_scratch: [nwf][nk][nao][nao]. */
+int gwref_find_mu(const gwref_dims *d, int nwf, const double *omega, const c128 *t_beta, const c128 *S, const c128 *F,
+                  const c128 *Sigma_w, double n_target, double mu_lo, double mu_hi, double mu_tol, c128 *Gw_scratch,
+                  double *mu_out, double *ne_out) {
+  double lo = mu_lo, hi = mu_hi;
+  int fail = 0;
+#define NE(mu_) (fail |= gwref_dyson_update(d, nwf, omega, (mu_), S, F, Sigma_w, Gw_scratch), gwref_electron_count(d, nwf, t_beta, S, Gw_scratch))
+  double nlo = NE(lo), nhi = NE(hi);
+  int it = 0;
+  while ((nlo > n_target || nhi < n_target) && it < 60) {
+    const double w = hi - lo;
+    if (nlo > n_target) { lo -= w; nlo = NE(lo); } else { hi += w; nhi = NE(hi); }
+    it++;
+  }
+  if (nlo > n_target || nhi < n_target) return 2;
+  for (it = 0; it < 200 && hi - lo > mu_tol; it++) {
+    const double mid = 0.5 * (lo + hi);
+    if (NE(mid) < n_target) lo = mid; else hi = mid;
+  }
+  *mu_out = 0.5 * (lo + hi);
+  *ne_out = NE(*mu_out);
+#undef NE
+  return fail;
+}
+
+/* Y = a X + b Y (simple mixing of two iterates, PAPER.md:326-330 mentions DIIS; plain damping is the baseline it improves on) */
+void gwref_axpby(size_t n, c128 a, const c128 *X, c128 b, c128 *Y) {
+  for (size_t i = 0; i < n; i++) Y[i] = a * X[i] + b * Y[i];
 }
 
 /* number of OpenMP threads the loops above will use (reported as cpu_baseline.cores) */

@@ -416,3 +416,112 @@ def test_P7_P9_raw(raw_problems, oracle_lib, name):
     for k in (0, cfg.nk - 1):
         S = oracle_lib.sigma_slice(cfg, vb, np.ascontiguousarray(-p.gamma), I, k)
         assert relerr(S, -K[k]) < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# Loop closure: Eq. 15, 16, 20 and the chemical-potential search.
+# ----------------------------------------------------------------------------------------------------------------
+def _closure_inputs(p):
+    cfg = p.cfg
+    H0, S = gwgen.make_h0_s(cfg, p.mesh, p.eps, p.U)
+    fg = gwgen.make_fermionic_grids(cfg.ntau, cfg.beta)
+    return H0, S, fg
+
+
+def test_P13_dyson_noninteracting_closed_form(problems, oracle_lib):
+    """Sigma = 0: G(i omega_n) = [(i omega_n + mu) S - H0]^-1 = C diag(1/(i omega_n + mu - e)) C^+ with the generalised eigenpairs
+    H0 C = S C e, C^+ S C = 1 (scipy.linalg.eigh, another basis and a library routine), and with a self-energy: A G = 1."""
+    import scipy.linalg as sla
+    p = problems("R")
+    cfg = p.cfg
+    H0, S, fg = _closure_inputs(p)
+    mu = 0.137
+    G_w = oracle_lib.dyson_update(cfg, fg["omega"], mu, S, H0)
+    for k in (0, 5, cfg.nk - 1):
+        e, C = sla.eigh(H0[k], S[k])
+        for n in (0, len(fg["omega"]) // 2, len(fg["omega"]) - 1):
+            ref = (C / (1j * fg["omega"][n] + mu - e)[None, :]) @ C.conj().T
+            assert relerr(G_w[n, k], ref) < 1e-12
+    rng = np.random.default_rng(2)
+    Sw = rng.normal(size=G_w.shape) + 1j * rng.normal(size=G_w.shape)          # arbitrary (non-Hermitian) Sigma~(i omega_n)
+    G2 = oracle_lib.dyson_update(cfg, fg["omega"], mu, S, H0, Sw)
+    for n in (0, 7):
+        for k in (1, 4):
+            A = (1j * fg["omega"][n] + mu) * S[k] - H0[k] - Sw[n, k]
+            assert np.linalg.norm(A @ G2[n, k] - np.eye(cfg.nao)) < 1e-12 * np.linalg.norm(A) * np.linalg.norm(G2[n, k])
+
+
+def test_P14_electron_count_and_mu(problems, oracle_lib):
+    """Sigma = 0 (config T: beta = 10, 32 nodes, where the grid is accurate to ~1e-9): Eq. 15 gives N_e(mu) = (s/N_k) sum_k sum_i
+    f(e_i^k - mu) with the generalised eigenvalues, and the chemical-potential search lands on the root of that closed form
+    (scipy.optimize.brentq)."""
+    import scipy.linalg as sla
+    import scipy.optimize as sop
+    p = problems("T")
+    cfg = p.cfg
+    H0, S, fg = _closure_inputs(p)
+    ev = np.array([sla.eigh(H0[k], S[k], eigvals_only=True) for k in range(cfg.nk)])
+    ne_ref = lambda mu: cfg.spin_deg / cfg.nk * float(np.sum(1.0 / (1.0 + np.exp(cfg.beta * (ev - mu)))))
+    for mu in (-0.4, 0.0, 0.3):
+        G_w = oracle_lib.dyson_update(cfg, fg["omega"], mu, S, H0)
+        assert abs(oracle_lib.electron_count(cfg, fg["t_beta"], S, G_w) - ne_ref(mu)) < 1e-8
+    target = cfg.spin_deg * 1.25                               # 2.5 electrons per cell: mu inside the band
+    mu, ne = oracle_lib.find_mu(cfg, fg["omega"], fg["t_beta"], S, H0, None, target, -0.1, 0.1)      # bracket must be widened
+    mu_ref = sop.brentq(lambda m: ne_ref(m) - target, -5.0, 5.0, xtol=1e-14)
+    assert abs(ne - target) < 1e-9                             # the paper's threshold (PAPER.md:320)
+    assert abs(mu - mu_ref) < 1e-7
+    # gamma from G(tau) (e_beta) and from G(i omega_n) (t_beta) agree: the two evaluation vectors are consistent with the transform pair
+    G_w = oracle_lib.dyson_update(cfg, fg["omega"], mu, S, H0)
+    Gb_w = np.tensordot(fg["t_beta"], G_w, axes=(0, 0))
+    Gb_t = np.tensordot(fg["e_beta"], oracle_lib.transform(fg["T_tw_f"], G_w), axes=(0, 0))
+    assert relerr(Gb_t, Gb_w) < 1e-8
+
+
+def test_P15_hartree_literal_einsum(problems, raw_problems, oracle_lib):
+    """Eq. 20 as printed, numpy einsum over the diagonal blocks, on symmetric and on symmetry-free inputs."""
+    for p in (problems("R"), raw_problems("T")):
+        cfg = p.cfg
+        V = p.V.numpy()
+        Vd = np.stack([V[k, k] for k in range(cfg.nk)])                      # [k][Q][i][j]
+        rho = np.einsum("kab,kQba->Q", p.gamma, Vd)
+        ref = cfg.spin_deg / cfg.nk * np.einsum("kQij,Q->kij", Vd, rho)
+        assert relerr(oracle_lib.hartree(cfg, oracle_lib.VBlocks(cfg, V), p.gamma), ref) < 1e-13
+
+
+def test_P16_fermionic_back_transform_closed_form(oracle_lib):
+    """1/(i omega_n - eps) -> -e^{-eps tau}/(1+e^{-beta eps}) (Eq. 14) and its value at beta^-; forward transform (Eq. 13) back again."""
+    beta, N = 10.0, 32
+    g = gwgen.make_grids(N, N, beta)
+    fg = gwgen.make_fermionic_grids(N, beta)
+    assert np.array_equal(fg["nfer"], -fg["nfer"][::-1] - 1)                 # symmetric under omega_n -> -omega_n
+    assert np.allclose(fg["omega"], (2 * fg["nfer"] + 1) * np.pi / beta, rtol=1e-15)
+    eps = np.array([0.7, -0.3, 0.05])
+    Gw = np.ascontiguousarray(1.0 / (1j * fg["omega"][:, None] - eps[None, :]))
+    ref = -np.exp(-np.outer(g["tau"], eps)) / (1.0 + np.exp(-beta * eps))
+    assert np.max(np.abs(oracle_lib.transform(fg["T_tw_f"], Gw) - ref)) < 1e-9
+    assert np.max(np.abs(oracle_lib.transform(fg["t_beta"].reshape(1, -1), Gw)[0] + 1.0 / (1.0 + np.exp(beta * eps)))) < 1e-9
+    assert np.max(np.abs(oracle_lib.transform(fg["e_beta"].reshape(1, -1), ref.astype(complex))[0] + 1.0 / (1.0 + np.exp(beta * eps)))) < 1e-9
+    assert np.max(np.abs(oracle_lib.transform(fg["T_wt_f"], ref.astype(complex)) - Gw)) < 1e-9
+
+
+def test_P17_scgw_iteration_noninteracting_limit(problems, oracle_lib):
+    """V = 0: one iteration of Fig. 4 returns the non-interacting Green's function of (H0, S) at the chemical potential of the
+    Fermi-function count, whatever G went in: G(tau) = -C diag(e^{-(e-mu) tau}/(1+e^{-beta(e-mu)})) C^+."""
+    import scipy.linalg as sla
+    import scipy.optimize as sop
+    p = problems("T")
+    cfg = p.cfg
+    H0, S, fg = _closure_inputs(p)
+    V0 = np.zeros(tuple(p.V.shape), np.complex128)
+    target = cfg.spin_deg * 1.5
+    r = oracle_lib.scgw_iteration(cfg, oracle_lib.VBlocks(cfg, V0), p.T_wt, p.T_tw, fg, H0, S, p.G, target, -1.0, 1.0)
+    ev = [sla.eigh(H0[k], S[k]) for k in range(cfg.nk)]
+    mu_ref = sop.brentq(lambda m: cfg.spin_deg / cfg.nk * sum(np.sum(1.0 / (1.0 + np.exp(cfg.beta * (e - m)))) for e, _ in ev) - target, -5, 5, xtol=1e-14)
+    assert abs(r["mu"] - mu_ref) < 1e-7
+    assert np.abs(r["Sigma_t"]).max() == 0.0 and np.abs(r["J"]).max() == 0.0
+    for k in range(cfg.nk):
+        e, C = ev[k]
+        x = e - mu_ref
+        g = -np.exp(-np.outer(p.tau, x)) / (1.0 + np.exp(-cfg.beta * x))
+        ref = np.einsum("in,tn,jn->tij", C, g, C.conj())
+        assert np.max(np.abs(r["G_new"][:, k] - ref)) < 1e-7
