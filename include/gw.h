@@ -143,6 +143,48 @@ size_t gw_workspace_bytes(const gw_problem *p);
 int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, const gw_c128 *gamma, gw_c128 *Sigma, gw_c128 *K,
                             gw_c128 *P0t_out, gw_c128 *Wt_out, float *stage_ms, void *stream);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Loop closure: the remaining steps of one scGW iteration (Fig. 4).  The fermionic tau <-> i omega_n
+ * transforms of Eq. 13 / 14 are gw_transform with the caller's fermionic matrices; G(tau = beta^-)
+ * (gamma = -G(beta^-)) is gw_transform with a 1 x ntau evaluation vector.  Grids are inputs (reading R6).
+ * ------------------------------------------------------------------------------------------------------------------ */
+
+/* Hartree term, Eq. 20 (the label "(19)" is lost in the text):
+ *   J[k][i][j] = (s/N_k) Σ_k' Σ_ab Σ_Q V[k][k][Q][i][j] gamma[k'][a][b] V[k'][k'][Q][b][a]        (s = spin_deg: the sum over sigma_1)
+ *   gamma : device [nk][nao][nao] in;  J : device [nk][nao][nao] out.  Reads only the diagonal blocks V[k][k]; uses p->work
+ *   (any q shard: J does not depend on q_begin / q_end). */
+int gw_hartree(const gw_problem *p, const gw_c128 *gamma, gw_c128 *J, void *stream);
+
+/* Dyson equation, Eq. 16, for every (n, k):
+ *   G_w[n][k] = [ (i omega[n] + mu) S[k] − F[k] − Sigma_w[n][k] ]^-1        ("matrix inversion in spin-orbital space")
+ *   omega : device double [nwf] (fermionic Matsubara frequencies);  S, F : device [nk][nao][nao] (overlap; F = H0 + Sigma_inf,
+ *   Eq. 17-18);  Sigma_w : device [nwf][nk][nao][nao] or NULL;  G_w : device [nwf][nk][nao][nao] out (must not alias Sigma_w's
+ *   other matrices; the same matrix is read completely before it is written, so G_w == Sigma_w is allowed).
+ *   In-kernel Gauss-Jordan elimination with partial pivoting, one CTA per matrix; nao <= 64 (GW_ESHAPE).
+ *   info : device int32[2], 8-byte aligned, or NULL: {-1,-1}, else {n, k} of one singular matrix (smallest k, then n). */
+int gw_dyson_update(int32_t nk, int32_t nao, int32_t nwf, const double *omega, double mu, const gw_c128 *S, const gw_c128 *F,
+                    const gw_c128 *Sigma_w, gw_c128 *G_w, int32_t *info, void *stream);
+
+/* Electron count, Eq. 15:  *ne = (s/N_k) Σ_k tr[gamma^k S^k],  gamma^k = −Σ_n t_beta[n] G_w[n][k]
+ *   t_beta : device [nwf] (evaluation vector G(beta^-) = Σ_n t_beta[n] G(i omega_n));  partial : device scratch [nk];
+ *   ne : device double out.  Fixed summation order (deterministic). */
+int gw_electron_count(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, const gw_c128 *t_beta, const gw_c128 *S,
+                      const gw_c128 *G_w, gw_c128 *partial, double *ne, void *stream);
+
+/* Chemical potential (Fig. 4 step 3: mu is adjusted until N_e is right to 1e-9): bisection on N_e(mu) of
+ * Eq. 15-16 (reading R16): widen [mu_lo, mu_hi] by its own width (<= 60 times) until it brackets n_target, halve it
+ * until its width <= mu_tol (<= 200 times), return the midpoint and N_e there; G_w then holds G(i omega_n) at that mu.
+ * Every N_e evaluation is one gw_dyson_update + gw_electron_count on `stream`; this call SYNCHRONISES the stream after each
+ * (it reads N_e back), unlike the calls above.  mu_out, ne_out, n_eval (optional) are HOST pointers.
+ * Returns GW_OK, GW_ENOTPD if a matrix was singular, GW_EINVAL also when no bracket was found. */
+int gw_find_mu(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, const double *omega, const gw_c128 *t_beta, const gw_c128 *S,
+               const gw_c128 *F, const gw_c128 *Sigma_w, double n_target, double mu_lo, double mu_hi, double mu_tol, gw_c128 *G_w,
+               gw_c128 *partial, double *ne_dev, double *mu_out, double *ne_out, int32_t *n_eval, void *stream);
+
+/* Y[i] = (a_re + i a_im) X[i] + (b_re + i b_im) Y[i], i < n (damping of two iterates, F = H0 + J + K, gamma = −G(beta^-)).
+ * Y is not read when b == 0.  X, Y : device, may be equal. */
+int gw_axpby(size_t n, double a_re, double a_im, const gw_c128 *X, double b_re, double b_im, gw_c128 *Y, void *stream);
+
 /* Executed FP64 flops of the last configuration of each stage kernel for `p` (what the kernels actually
  * issue, padding and recomputation included; 2 flops per real FMA).  out: host double[4] = stage 1..4. */
 int gw_executed_flops(const gw_problem *p, double *out);

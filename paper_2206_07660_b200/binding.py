@@ -53,10 +53,18 @@ def lib():
         L.gw_launch_count.argtypes = [P]
         L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
         L.gw_fp64_peak_dfma.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
+        i32, dbl = ctypes.c_int32, ctypes.c_double
+        L.gw_hartree.argtypes = [P, vp, vp, vp]
+        L.gw_dyson_update.argtypes = [i32, i32, i32, vp, dbl, vp, vp, vp, vp, vp, vp]
+        L.gw_electron_count.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+        L.gw_find_mu.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, vp,
+                                 ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(i32), vp]
+        L.gw_axpby.argtypes = [sz, dbl, dbl, vp, dbl, dbl, vp, vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
-                  "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version"):
+                  "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version",
+                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -266,3 +274,99 @@ def gw_fp64_peak_dfma(ms=200.0, stream=None):
     out = ctypes.c_double(0.0)
     _check(lib().gw_fp64_peak_dfma(ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_fp64_peak_dfma")
     return out.value
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# loop closure (gw.h "Loop closure"; Fig. 4 of the paper)
+# ---------------------------------------------------------------------------------------------------------------------
+def _c128(t, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()):
+        raise GWError(f"{name}: need a contiguous CUDA complex128 tensor")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _f64(t, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise GWError(f"{name}: need a contiguous CUDA float64 tensor")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def gw_hartree(prob, gamma, J=None, stream=None):
+    """Eq. 20: J[k] from gamma[k'] and the diagonal blocks V[k][k]."""
+    shape = (prob.nk, prob.nao, prob.nao)
+    if J is None:
+        J = torch.empty(shape, dtype=torch.complex128, device=gamma.device)
+    _check(lib().gw_hartree(prob.ref(), _dev(gamma, shape, "gamma"), _dev(J, shape, "J"), _stream(stream)), "gw_hartree")
+    return J
+
+
+def gw_dyson_update(omega, mu, S, F, Sigma_w=None, G_w=None, info=None, stream=None):
+    """Eq. 16 for all (n, k): G_w[n][k] = [(i omega_n + mu) S[k] - F[k] - Sigma_w[n][k]]^-1."""
+    nk, nao = int(S.shape[0]), int(S.shape[1])
+    nwf = int(omega.numel())
+    shape = (nwf, nk, nao, nao)
+    if G_w is None:
+        G_w = torch.empty(shape, dtype=torch.complex128, device=S.device)
+    if info is None:
+        info = torch.empty(2, dtype=torch.int32, device=S.device)
+    _check(lib().gw_dyson_update(nk, nao, nwf, _f64(omega, "omega"), float(mu), _dev(S, (nk, nao, nao), "S"), _dev(F, (nk, nao, nao), "F"),
+                                 _dev(Sigma_w, shape, "Sigma_w") if Sigma_w is not None else None, _dev(G_w, shape, "G_w"),
+                                 ctypes.c_void_p(info.data_ptr()), _stream(stream)), "gw_dyson_update")
+    return G_w, info
+
+
+def gw_electron_count(t_beta, S, G_w, spin_deg=2, stream=None):
+    """Eq. 15: N_e from G(i omega_n) (returns a 1-element CUDA float64 tensor; no host sync)."""
+    nwf, nk, nao = int(G_w.shape[0]), int(G_w.shape[1]), int(G_w.shape[2])
+    partial = torch.empty(nk, dtype=torch.complex128, device=S.device)
+    ne = torch.empty(1, dtype=torch.float64, device=S.device)
+    _check(lib().gw_electron_count(nk, nao, nwf, int(spin_deg), _dev(t_beta, (nwf,), "t_beta"), _dev(S, (nk, nao, nao), "S"),
+                                   _c128(G_w, "G_w"), _c128(partial, "partial"), _f64(ne, "ne"), _stream(stream)), "gw_electron_count")
+    return ne
+
+
+def gw_find_mu(omega, t_beta, S, F, Sigma_w, n_target, mu_lo, mu_hi, mu_tol=1e-12, spin_deg=2, G_w=None, stream=None):
+    """Chemical-potential search of Fig. 4 step 3 (synchronises the stream).  Returns (mu, N_e(mu), G_w at mu, evaluations)."""
+    nk, nao = int(S.shape[0]), int(S.shape[1])
+    nwf = int(omega.numel())
+    shape = (nwf, nk, nao, nao)
+    if G_w is None:
+        G_w = torch.empty(shape, dtype=torch.complex128, device=S.device)
+    partial = torch.empty(nk, dtype=torch.complex128, device=S.device)
+    ne = torch.empty(1, dtype=torch.float64, device=S.device)
+    mu_o, ne_o, ev = ctypes.c_double(0.0), ctypes.c_double(0.0), ctypes.c_int32(0)
+    _check(lib().gw_find_mu(nk, nao, nwf, int(spin_deg), _f64(omega, "omega"), _dev(t_beta, (nwf,), "t_beta"), _dev(S, (nk, nao, nao), "S"),
+                            _dev(F, (nk, nao, nao), "F"), _dev(Sigma_w, shape, "Sigma_w") if Sigma_w is not None else None,
+                            float(n_target), float(mu_lo), float(mu_hi), float(mu_tol), _dev(G_w, shape, "G_w"), _c128(partial, "partial"),
+                            _f64(ne, "ne"), ctypes.byref(mu_o), ctypes.byref(ne_o), ctypes.byref(ev), _stream(stream)), "gw_find_mu")
+    return mu_o.value, ne_o.value, G_w, ev.value
+
+
+def gw_axpby(a, X, b, Y, stream=None):
+    """Y <- a X + b Y (complex scalars a, b)."""
+    if X.shape != Y.shape:
+        raise GWError("gw_axpby: shapes differ")
+    a, b = complex(a), complex(b)
+    _check(lib().gw_axpby(X.numel(), a.real, a.imag, _c128(X, "X"), b.real, b.imag, _c128(Y, "Y"), _stream(stream)), "gw_axpby")
+    return Y
+
+
+def gw_scgw_iteration(prob, fg, H0, S, G, n_target, mu_lo, mu_hi, alpha=1.0, mu_tol=1e-12, stream=None):
+    """One scGW iteration in the order of Fig. 4, every step a C-ABI call (this function only sequences them):
+    G(tau) -> gamma = -G(beta^-) -> J (Eq. 20), K (Eq. 22), Sigma~(tau) (Algorithm 1) -> Sigma~(i omega_n) (Eq. 13) -> mu (Eq. 15) ->
+    G(i omega_n) (Eq. 16) -> G(tau) (Eq. 14) -> damping.  fg: dict of CUDA tensors omega, T_wt_f, T_tw_f, t_beta, e_beta
+    (gwgen.make_fermionic_grids).  Returns a dict of CUDA tensors and the scalars mu, ne."""
+    Gb = gw_transform(fg["e_beta"].reshape(1, -1), G, stream=stream)[0].contiguous()
+    gamma = gw_axpby(-1.0, Gb, 0.0, torch.empty_like(Gb), stream)
+    J = gw_hartree(prob, gamma, stream=stream)
+    K = gw_exchange(prob, gamma, stream=stream)
+    P0t = gw_polarization(prob, G, stream=stream)
+    Wt, info = gw_screened_interaction(prob, P0t, P0t, stream=stream)
+    Sigma_t = gw_selfenergy(prob, G, Wt, stream=stream)
+    Sigma_w = gw_transform(fg["T_wt_f"], Sigma_t, stream=stream)
+    F = gw_axpby(1.0, J, 1.0, gw_axpby(1.0, K, 1.0, H0.clone(), stream), stream)
+    mu, ne, G_w, n_eval = gw_find_mu(fg["omega"], fg["t_beta"], S, F, Sigma_w, n_target, mu_lo, mu_hi, mu_tol, prob.spin_deg, stream=stream)
+    G_new = gw_transform(fg["T_tw_f"], G_w, stream=stream)
+    G_mix = gw_axpby(alpha, G_new, 1.0 - alpha, G.clone(), stream)
+    return dict(gamma=gamma, J=J, K=K, Wt=Wt, info=info, Sigma_t=Sigma_t, Sigma_w=Sigma_w, F=F, mu=mu, ne=ne, G_w=G_w, G_new=G_new,
+                G=G_mix, n_eval=n_eval)

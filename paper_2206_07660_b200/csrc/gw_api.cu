@@ -159,6 +159,95 @@ done:
   return rc;
 }
 
+
+// ---- loop closure (gw_loop.cu) ----
+extern "C" int gw_hartree(const gw_problem *p, const gw_c128 *gamma, gw_c128 *J, void *stream) {
+  int rc = check_problem(p, false); if (rc) return rc;
+  if (!aligned16(gamma) || !aligned16(J)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  return gw_launch_hartree(p, (const c128 *)gamma, (c128 *)J, (cudaStream_t)stream);
+}
+
+static int check_loop_args(int nk, int nao, int nwf, const void *omega, const void *S, const void *F, const void *G_w) {
+  if (nk <= 0 || nao <= 0 || nwf <= 0 || nk > (1 << 20) || nwf > (1 << 20)) return GW_EINVAL;
+  if (!omega || (((uintptr_t)omega) & 7) || !aligned16(S) || !aligned16(F) || !aligned16(G_w)) return GW_EINVAL;
+  if (nao > GW_MAX_NAO) return GW_ESHAPE;
+  return GW_OK;
+}
+
+extern "C" int gw_dyson_update(int32_t nk, int32_t nao, int32_t nwf, const double *omega, double mu, const gw_c128 *S, const gw_c128 *F,
+                               const gw_c128 *Sigma_w, gw_c128 *G_w, int32_t *info, void *stream) {
+  int rc = check_loop_args(nk, nao, nwf, omega, S, F, G_w); if (rc) return rc;
+  if ((Sigma_w && !aligned16(Sigma_w)) || (((uintptr_t)info) & 7)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  return gw_launch_dyson_update(nk, nao, nwf, omega, mu, (const c128 *)S, (const c128 *)F, (const c128 *)Sigma_w, (c128 *)G_w, info, (cudaStream_t)stream);
+}
+
+extern "C" int gw_electron_count(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, const gw_c128 *t_beta, const gw_c128 *S,
+                                 const gw_c128 *G_w, gw_c128 *partial, double *ne, void *stream) {
+  if (nk <= 0 || nao <= 0 || nwf <= 0 || (spin_deg != 1 && spin_deg != 2)) return GW_EINVAL;
+  if (!aligned16(t_beta) || !aligned16(S) || !aligned16(G_w) || !aligned16(partial) || !ne || (((uintptr_t)ne) & 7)) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  return gw_launch_electron_count(nk, nao, nwf, spin_deg, (const c128 *)t_beta, (const c128 *)S, (const c128 *)G_w, (c128 *)partial, ne, (cudaStream_t)stream);
+}
+
+extern "C" int gw_find_mu(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, const double *omega, const gw_c128 *t_beta, const gw_c128 *S,
+                          const gw_c128 *F, const gw_c128 *Sigma_w, double n_target, double mu_lo, double mu_hi, double mu_tol, gw_c128 *G_w,
+                          gw_c128 *partial, double *ne_dev, double *mu_out, double *ne_out, int32_t *n_eval, void *stream) {
+  int rc = check_loop_args(nk, nao, nwf, omega, S, F, G_w); if (rc) return rc;
+  if ((spin_deg != 1 && spin_deg != 2) || !aligned16(t_beta) || !aligned16(partial) || !ne_dev || (((uintptr_t)ne_dev) & 7) || !mu_out || !ne_out) return GW_EINVAL;
+  if ((Sigma_w && !aligned16(Sigma_w)) || !(mu_hi > mu_lo) || !(mu_tol > 0)) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  int32_t *dinfo = 0; int32_t hinfo[2] = {-1, -1};
+  int evals = 0; bool singular = false;
+  CU(cudaMalloc(&dinfo, 8));
+  {
+    // N_e(mu): Eq. 16 for all (n, k), then Eq. 15; the value is read back (8 bytes) with the factorisation status
+    auto NE = [&](double mu, double *val) -> int {
+      int r = gw_launch_dyson_update(nk, nao, nwf, omega, mu, (const c128 *)S, (const c128 *)F, (const c128 *)Sigma_w, (c128 *)G_w, dinfo, st);
+      if (r) return r;
+      r = gw_launch_electron_count(nk, nao, nwf, spin_deg, (const c128 *)t_beta, (const c128 *)S, (const c128 *)G_w, (c128 *)partial, ne_dev, st);
+      if (r) return r;
+      cudaError_t e = cudaMemcpyAsync(val, ne_dev, 8, cudaMemcpyDeviceToHost, st);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(hinfo, dinfo, 8, cudaMemcpyDeviceToHost, st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+      if (e != cudaSuccess) return (int)e;
+      if (hinfo[0] != -1 || hinfo[1] != -1) singular = true;
+      evals++;
+      return 0;
+    };
+    double lo = mu_lo, hi = mu_hi, nlo = 0, nhi = 0, nmid = 0;
+    if ((rc = NE(lo, &nlo)) || (rc = NE(hi, &nhi))) goto done;
+    int it = 0;
+    while ((nlo > n_target || nhi < n_target) && it < 60) {
+      const double w = hi - lo;
+      if (nlo > n_target) { lo -= w; if ((rc = NE(lo, &nlo))) goto done; }
+      else { hi += w; if ((rc = NE(hi, &nhi))) goto done; }
+      it++;
+    }
+    if (nlo > n_target || nhi < n_target) { rc = GW_EINVAL; goto done; }
+    for (it = 0; it < 200 && hi - lo > mu_tol; it++) {
+      const double mid = 0.5 * (lo + hi);
+      if ((rc = NE(mid, &nmid))) goto done;
+      if (nmid < n_target) lo = mid; else hi = mid;
+    }
+    *mu_out = 0.5 * (lo + hi);
+    if ((rc = NE(*mu_out, ne_out))) goto done;
+    if (singular) rc = GW_ENOTPD;
+  }
+done:
+  if (n_eval) *n_eval = evals;
+  cudaFree(dinfo);
+  return rc;
+}
+
+extern "C" int gw_axpby(size_t n, double a_re, double a_im, const gw_c128 *X, double b_re, double b_im, gw_c128 *Y, void *stream) {
+  if (!aligned16(X) || !aligned16(Y)) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  return gw_launch_axpby(n, make_double2(a_re, a_im), (const c128 *)X, make_double2(b_re, b_im), (c128 *)Y, (cudaStream_t)stream);
+}
+
 // ---- FP64 peak probe: register-resident DMMA.8x8x4 loop, 8 independent accumulators per warp ----
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, int iters) {
   double acc[8][2];

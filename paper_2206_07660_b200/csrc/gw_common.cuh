@@ -78,6 +78,12 @@ int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *in
 int gw_launch_transform(int n_out, int n_in, const c128 *T, const c128 *X, c128 *Y, size_t len, cudaStream_t st);
 int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st);
 int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st);
+int gw_launch_hartree(const gw_problem *p, const c128 *gamma, c128 *J, cudaStream_t st);
+int gw_launch_dyson_update(int nk, int nao, int nwf, const double *omega, double mu, const c128 *S, const c128 *F, const c128 *Sigma_w, c128 *G_w,
+                           int32_t *info, cudaStream_t st);
+int gw_launch_electron_count(int nk, int nao, int nwf, int spin_deg, const c128 *t_beta, const c128 *S, const c128 *G_w, c128 *partial, double *ne,
+                             cudaStream_t st);
+int gw_launch_axpby(size_t n, c128 a, const c128 *X, c128 b, c128 *Y, cudaStream_t st);
 size_t gw_stage1_workspace(const gw_problem *p);
 size_t gw_stage2_workspace(const gw_problem *p);
 size_t gw_stage3_workspace(const gw_problem *p);

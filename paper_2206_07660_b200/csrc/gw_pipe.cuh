@@ -3,6 +3,7 @@
 // Stage 4 runs 256 threads per CTA with a 3-deep cp.async ring (NTHR, NSTAGE below); stages 1 and 3 are warp specialised
 // (gw_stage1.cu, gw_stage3.cu) and use the mbarrier ring / setmaxnreg helpers further down.  One CTA per SM everywhere.
 #pragma once
+#include <cuda.h>
 #include "gw_common.cuh"
 
 namespace gwp {
@@ -302,7 +303,7 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, unsigned parity
 struct Ring {
   uint64_t *full, *empty;   // [nstage] each
   int nstage;
-  unsigned it;              // stage index of the next job (same sequence on both sides)
+  unsigned it = 0;          // stage index of the next job (same sequence on both sides)
   unsigned ph = 0;          // parity of the current round (no integer division per job)
   __device__ __forceinline__ int stage() const { return (int)it; }
   __device__ __forceinline__ void advance() { if (++it == (unsigned)nstage) { it = 0; ph ^= 1u; } }
@@ -313,6 +314,45 @@ struct Ring {
   __device__ __forceinline__ int wait() { const int s = stage(); mbar_wait(full + s, ph); return s; }
   __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) mbar_arrive(empty + stage()); advance(); }
 };
+
+// ---- TMA (cp.async.bulk.tensor) and L2 eviction policies, shared by stages 1 and 3 ----
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
+               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// the slabs are read exactly once after they are written (evict first); the V blocks are shared by every CTA working on the same
+// q / k (evict last)
+__device__ __forceinline__ uint64_t policy_evict_first() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p)); return p; }
+__device__ __forceinline__ uint64_t policy_evict_last() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p)); return p; }
+__device__ __forceinline__ uint64_t policy_evict_normal() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;\n" : "=l"(p)); return p; }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda; the entry point's address is a
+// process-wide constant, cached).  View: [rows][ncplx complex] row-major matrix of doubles, box = box_rows x 8 complex (128 bytes),
+// 128-byte swizzle, zero fill outside the array.
+static inline int make_tensor_map(CUtensorMap *map, const void *base, size_t rows, int ncplx, int box_rows) {
+  typedef CUresult (*Fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                         const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Fn fn = nullptr;
+  if (!fn) {
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
+      cudaGetLastError();
+      return (int)cudaErrorNotSupported;
+    }
+    fn = (Fn)ptr;
+  }
+  const cuuint64_t gdim[2] = {(cuuint64_t)2 * ncplx, (cuuint64_t)rows};
+  const cuuint64_t gstr[1] = {(cuuint64_t)ncplx * 16};
+  const cuuint32_t box[2] = {16u, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
+}
 
 // producer-warpgroup versions of the job issue functions (128 threads: threadIdx.x - 32*NCONS)
 __device__ __forceinline__ void ws_issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd) {

@@ -8,11 +8,13 @@
 // so the second operand is the raw V block (rows Q', K contiguous), never transformed.
 //
 // Work decomposition: a work item is a row panel [TM = 32 Q-rows] x [all naux Q'] of one (t,q); it is owned by one CTA
-// (naux <= 224) or by a cluster of two CTAs that split the Q' columns (naux <= 448), and its accumulators stay in
+// (naux <= 128) or by a cluster of two or four CTAs that split the Q' columns (naux <= 256 / 512), and its accumulators stay in
 // registers over the whole k loop (the k-sum is inside the K loop; no cross-CTA reduction, deterministic).
 // A CTA is warp specialised (16 warps, register budgets rebalanced with setmaxnreg):
-//   main warps 0-7   : acc[Q][Q'] += Σ_K Z[Q][K] V[k+q][k][Q'][K] on FP64 tensor cores (DMMA.8x8x4, 4-real-GEMM complex
-//                      scheme), operands streamed through an mbarrier-tracked cp.async ring
+//   main warps 0-7   : acc[Q][Q'] += Σ_K Z[Q][K] V[k+q][k][Q'][K] on FP64 tensor cores (DMMA.8x8x4), operands streamed through an
+//                      mbarrier-tracked TMA ring.  Complex tile products use the 3M scheme: three real DMMAs per complex
+//                      8x8x4 product, K1 += Ar·Br, K2 += Ai·Bi, K3 += (Ar+Ai)·(Br+Bi); Re = K1 − K2, Im = K3 − K1 − K2, with
+//                      three real accumulator sets per tile (warp tile 2 x 4 tiles) and the operand sums formed in registers
 //   pass warps 8-11  : produce Z for the NEXT k while the main warps consume the current one
 //                        pass 1:  Xt[Q][b][d] = Σ_a V[k][k+q][Q][d][a] G[t][k+q][a][b]      rows (Q,d) flat
 //                        pass 2:  Z [Q][b][c] = Σ_d Xt[Q][b][d] G[tbar][k][c][d]            rows (Q,b) flat; in place
@@ -22,7 +24,6 @@
 //                      pass ring and the G matrices with cp.async (26-wide rows need padded destinations)
 // Xt/Z live in two per-cluster slabs of the workspace (TM·nao² complex each, double buffered over k, written and
 // re-read within ~100 µs, i.e. L2 resident); they never exist as a [t][q][k] tensor.
-#include <cuda.h>
 #include "gw_pipe.cuh"
 
 namespace s1 {
@@ -35,7 +36,9 @@ constexpr int T_PPROD = 32 * 15, N_PPROD = 32;        // pass-ring producer thre
 constexpr int NST_MAX = 8, PST_MAX = 4;
 constexpr int KC = 8;           // complex K per main job (one 128-byte row per operand row)
 constexpr int MT_W = 2;         // m-tiles per main warp
-constexpr int NJ = 7;           // n-tiles per main warp (4 column groups x 7 = 28 n-tiles = 224 columns per CTA)
+// n-tiles per main warp: 3M scheme 4 (three accumulator sets; 4 column groups x 4 = 16 n-tiles = 128 columns per CTA), 4-real-GEMM
+// scheme 7 (two accumulator sets; 28 n-tiles = 224 columns per CTA)
+constexpr int NJ_3M = 4, NJ_4M = 7;
 constexpr int TM = 32;          // panel rows
 constexpr int REG_MAIN = 176, REG_PASS = 120, REG_PROD = 40;   // 256*176 + 128*120 + 128*40 = 65536
 
@@ -62,35 +65,7 @@ struct Params {
   FastDiv fd_nao;
 };
 
-// ring bookkeeping (same job sequence on the producer and the consumer side)
-struct Ring {
-  uint64_t *full, *empty;
-  int nstage; unsigned it;     // `it` = stage index, `ph` = parity of the current round (no integer division per job)
-  unsigned ph;
-  __device__ __forceinline__ int stage() const { return (int)it; }
-  __device__ __forceinline__ void advance() { if (++it == (unsigned)nstage) { it = 0; ph ^= 1u; } }
-  __device__ __forceinline__ int acquire() { const int s = stage(); gwp::mbar_wait(empty + s, ph ^ 1u); return s; }
-  __device__ __forceinline__ void commit() { gwp::cp_async_arrive_noinc(full + stage()); advance(); }
-  __device__ __forceinline__ int wait() { const int s = stage(); gwp::mbar_wait(full + s, ph); return s; }
-  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); advance(); }
-};
-
-// L2 eviction policies: the slabs are read exactly once after they are written (evict first), the V blocks are shared by
-// every CTA working on the same q (evict last)
-__device__ __forceinline__ uint64_t policy_evict_first() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p)); return p; }
-__device__ __forceinline__ uint64_t policy_evict_last() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p)); return p; }
-__device__ __forceinline__ void cpa_hint(unsigned dst, const void *src, int nbytes, uint64_t pol) {
-  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst), "l"(src), "r"(nbytes), "l"(pol));
-}
-
-// ---- TMA (main ring) ----
-__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
-               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(gwp::smem_u32(bar)), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(gwp::smem_u32(bar)), "r"(bytes) : "memory");
-}
+using gwp::Ring; using gwp::tma_load_2d; using gwp::mbar_expect_tx; using gwp::policy_evict_first; using gwp::policy_evict_last;
 
 // rows [row0, row0+prows) of a dense (rows x nao) matrix -> stage[r][ldp]   (pass-ring producer warp)
 __device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd, int prows) {
@@ -113,9 +88,10 @@ __device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao,
 }
 
 // main warps: one main job (KC/4 k-steps) for this warp's MTW x NJM tiles (n-tiles NSTRIDE apart); all fragment loads
-// hoisted per k-step
-template <int NJM, int NSTRIDE, int MTW>
-__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int sw) {
+// hoisted per k-step.  S3M: acc[0] += Ar Br, acc[1] += Ai Bi, acc[2] += (Ar+Ai)(Br+Bi); else acc[0] / acc[1] = real / imaginary
+// part by four real DMMAs.
+template <bool S3M, int NJM, int NSTRIDE, int MTW, int NJ>
+__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&acc)[S3M ? 3 : 2][MT_W][NJ][2], int c, int sw) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
     const int u = (4 * ks + c) ^ sw;
@@ -124,11 +100,34 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
     for (int i = 0; i < MTW; i++) a[i] = sAw[i * 8 * KC + u];
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++) b[jn] = sBw[jn * NSTRIDE * 8 * KC + u];
+    if constexpr (S3M) {
+      double as[MTW];
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++)
+      for (int i = 0; i < MTW; i++) as[i] = a[i].x + a[i].y;
 #pragma unroll
-      for (int i = 0; i < MTW; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
+      for (int jn = 0; jn < NJM; jn++) {
+        const double bs = b[jn].x + b[jn].y;
+#pragma unroll
+        for (int i = 0; i < MTW; i++) {
+          dmma884(acc[0][i][jn][0], acc[0][i][jn][1], a[i].x, b[jn].x);
+          dmma884(acc[1][i][jn][0], acc[1][i][jn][1], a[i].y, b[jn].y);
+          dmma884(acc[2][i][jn][0], acc[2][i][jn][1], as[i], bs);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int jn = 0; jn < NJM; jn++)
+#pragma unroll
+        for (int i = 0; i < MTW; i++) cmma(acc[0][i][jn], acc[1][i][jn], a[i], b[jn]);
+    }
   }
+}
+
+// njm (1..NJ) is warp-uniform: pick the straight-line instance
+template <bool S3M, int NSTRIDE, int MTW, int NJ, int NJM = NJ>
+__device__ __forceinline__ void main_dispatch(int njm, const c128 *sAw, const c128 *sBw, double (&acc)[S3M ? 3 : 2][MT_W][NJ][2], int c, int sw) {
+  if (njm == NJM) main_compute<S3M, NJM, NSTRIDE, MTW, NJ>(sAw, sBw, acc, c, sw);
+  else if constexpr (NJM > 1) main_dispatch<S3M, NSTRIDE, MTW, NJ, NJM - 1>(njm, sAw, sBw, acc, c, sw);
 }
 
 // decode a work item: Q-tile index fastest (a cluster's item sequence cycles through full and ragged panels, so the short,
@@ -144,7 +143,7 @@ __device__ __forceinline__ Item decode_item(const Params &P, int item) {
   return it;
 }
 
-template <int KSP_MAX>
+template <int KSP_MAX, bool S3M>
 __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmZ) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   // the TMA destinations (128-byte swizzle) need 1024-byte alignment: the launch asks for 1 KB of slack
@@ -301,6 +300,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
   } else {
     // ========================================= main warps =========================================
     gwp::reg_inc<REG_MAIN>();
+    constexpr int NJ = S3M ? NJ_3M : NJ_4M, NACC = S3M ? 3 : 2;
     const int g = lane >> 2, c = lane & 3;
     // TMA 128-byte swizzle: 16-byte unit u of row r sits at u ^ (r & 7).  Fragment lane group g reads matrix row rho(g) of its
     // 8-row tile, so that the two rows of a quarter-warp differ in bit 2 (conflict-free); the accumulator rows / columns are
@@ -327,11 +327,13 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
       const int ntc_item = P.herm ? min(ntc_mine, max(0, it.Q0 + TM - col0 + 7) / 8) : ntc_mine;
       const int njm = (ntc_item > noff) ? (ntc_item - noff + nstride - 1) / nstride : 0;
       const bool active = (mh * MT_W < mtc) && njm > 0;
-      double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
+      double acc[NACC][MT_W][NJ][2];
 #pragma unroll
-      for (int i = 0; i < MT_W; i++)
+      for (int x = 0; x < NACC; x++)
 #pragma unroll
-        for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
+        for (int i = 0; i < MT_W; i++)
+#pragma unroll
+          for (int j = 0; j < NJ; j++) acc[x][i][j][0] = acc[x][i][j][1] = 0.0;
 
       for (int k = 0; k < d.nk; k++, kit++) {
         for (int j = 0; j < nmain; j++) {
@@ -339,29 +341,11 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
           if (active) {
             const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + rho) * KC;
             const c128 *sBw = sMain + s * P.main_units + TM * KC + (8 * noff + rho) * KC;
-            if (!narrow && njm == NJ) main_compute<NJ, 4, MT_W>(sAw, sBw, accr, acci, c, sw);
-            else if (!narrow && njm == NJ - 1) main_compute<NJ - 1, 4, MT_W>(sAw, sBw, accr, acci, c, sw);
-            else if (narrow && mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, accr, acci, c, sw);
-            else if (narrow && mtw == 1 && njm == 3) main_compute<3, 8, 1>(sAw, sBw, accr, acci, c, sw);
-            else if (narrow && mtw == 2 && njm == 4) main_compute<4, 8, 2>(sAw, sBw, accr, acci, c, sw);
-            else if (narrow && mtw == 2 && njm == 3) main_compute<3, 8, 2>(sAw, sBw, accr, acci, c, sw);
-            else {
-#pragma unroll
-              for (int ks = 0; ks < KC / 4; ks++) {
-                const int u = (4 * ks + c) ^ sw;
-                c128 a[MT_W];
-#pragma unroll
-                for (int i = 0; i < MT_W; i++) a[i] = sAw[i * 8 * KC + u];
-#pragma unroll
-                for (int jn = 0; jn < NJ; jn++) {
-                  if (jn < njm) {
-                    const c128 b = sBw[jn * nstride * 8 * KC + u];
-#pragma unroll
-                    for (int i = 0; i < MT_W; i++) cmma(accr[i][jn], acci[i][jn], a[i], b);
-                  }
-                }
-              }
-            }
+            // narrow panels: njm <= ceil(4 NJ / 8)
+            if (narrow) {
+              if (mtw == 1) main_dispatch<S3M, 8, 1, NJ, (NJ + 1) / 2>(njm, sAw, sBw, acc, c, sw);
+              else main_dispatch<S3M, 8, 2, NJ, (NJ + 1) / 2>(njm, sAw, sBw, acc, c, sw);
+            } else main_dispatch<S3M, 4, MT_W, NJ>(njm, sAw, sBw, acc, c, sw);
           }
           rm.release();
         }
@@ -391,8 +375,15 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
             if (jn < njm && Q < naux) {
               // accumulator columns 2c, 2c+1 hold matrix columns rho(2c) = c and rho(2c+1) = c + 4 of the n-tile
               const int ca = 8 * (noff + nstride * jn) + c, cb = ca + 4;
-              const c128 v0 = make_double2(pref * accr[i][jn][0], pref * acci[i][jn][0]);
-              const c128 v1 = make_double2(pref * accr[i][jn][1], pref * acci[i][jn][1]);
+              // 3M: Re = K1 - K2, Im = K3 - K1 - K2
+              c128 v0, v1;
+              if constexpr (S3M) {
+                v0 = make_double2(pref * (acc[0][i][jn][0] - acc[1][i][jn][0]), pref * (acc[2][i][jn][0] - acc[0][i][jn][0] - acc[1][i][jn][0]));
+                v1 = make_double2(pref * (acc[0][i][jn][1] - acc[1][i][jn][1]), pref * (acc[2][i][jn][1] - acc[0][i][jn][1] - acc[1][i][jn][1]));
+              } else {
+                v0 = make_double2(pref * acc[0][i][jn][0], pref * acc[1][i][jn][0]);
+                v1 = make_double2(pref * acc[0][i][jn][1], pref * acc[1][i][jn][1]);
+              }
               // element (Q, col) goes to [Q][col], or to [col][Q] in the transposed copy for -q; in Hermitian mode the elements
               // left of the diagonal block also fill their mirror image with the conjugate
 #pragma unroll
@@ -426,6 +417,7 @@ static int fill_qirr(const GwDims &d, short *qirr) {
 
 struct Plan {
   int main_off;
+  int s3m;               // 1: 3M scheme in the main GEMM (16 n-tiles per CTA), 0: 4-real-GEMM scheme (28 n-tiles per CTA)
   int cs, ncp, ksp_max, nqt, nitems, nteff, nqeff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
   size_t smem, slab_units, work_bytes;
   bool ok;
@@ -435,6 +427,10 @@ static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
   GwDims d = gw_dims(p);
   pl.nt = (d.naux + 7) / 8;
+  // scheme (measured, profiles/r02_3m_vs_4m.md): 3M while a panel fits one CTA or a 2-CTA cluster (naux <= 256); wider panels would need
+  // a 4-CTA cluster under 3M, which measured slower than the 2-CTA cluster of the 4-real-GEMM scheme with its 224-column tile
+  pl.s3m = pl.nt <= 8 * NJ_3M ? 1 : 0;
+  const int NJ = pl.s3m ? NJ_3M : NJ_4M;
   pl.cs = pl.nt <= 4 * NJ ? 1 : 2;
   pl.ncp = (pl.nt + pl.cs * 4 * NJ - 1) / (pl.cs * 4 * NJ);
   pl.ntc = (pl.nt + pl.cs * pl.ncp - 1) / (pl.cs * pl.ncp);
@@ -480,7 +476,7 @@ size_t gw_stage1_workspace(const gw_problem *p) {
   return pl.ok ? pl.work_bytes : 0;
 }
 
-// executed flops: every complex tile MMA is 4 DMMA.8x8x4 = 2048 flops
+// executed flops: a complex tile product is 4 DMMA.8x8x4 = 2048 flops in the two passes and 3 (1536 flops, 3M) in the main GEMM
 double gw_stage1_flops(const gw_problem *p) {
   s1::Plan pl = s1::make_plan(p);
   if (!pl.ok) return 0.0;
@@ -495,58 +491,28 @@ double gw_stage1_flops(const gw_problem *p) {
       if (rows < 0) rows = 0;
       mt_pass += (rows * d.nao + 7) / 8;
     }
-    const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp * pl.ncp;
+    const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp * pl.ncp * 2048.0;
     const int mtc = (tm_rows + 7) / 8;
     // main: warps whose first m-tile is valid execute MT_W m-tiles x their n-tiles x 2 k-steps per job
     const double mtiles = mtc <= 2 ? (double)mtc : (double)((mtc + s1::MT_W - 1) / s1::MT_W) * s1::MT_W;   // ragged panel: narrow ownership
     const double nmain = (d.nao * d.nao + s1::KC - 1) / s1::KC;
     int nt_eff = pl.nt;                         // Hermitian mode: n-tiles up to the panel's diagonal block
     if ((d.sym & GW_SYM_TR) && nt_eff > (qt * s1::TM + s1::TM + 7) / 8) nt_eff = (qt * s1::TM + s1::TM + 7) / 8;
-    const double mainv = mtiles * nt_eff * (s1::KC / 4) * nmain;
+    const double mainv = mtiles * nt_eff * (s1::KC / 4) * nmain * (pl.s3m ? 1536.0 : 2048.0);
     tiles += pass + mainv;
   }
-  return tiles * (double)d.nk * pl.nteff * pl.nqeff * 2048.0;
+  return tiles * (double)d.nk * pl.nteff * pl.nqeff;
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static EncodeTiledFn encode_tiled_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void *ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
-      cudaGetLastError();
-      return nullptr;
-    }
-    fn = (EncodeTiledFn)ptr;
-  }
-  return fn;
-}
-// rows x (nao² complex = 2 nao² doubles) matrix, box = 8 complex x box_rows, 128-byte swizzle, zero fill outside
-static int make_rows_map(CUtensorMap *map, const void *base, size_t rows, int n2, int box_rows) {
-  EncodeTiledFn enc = encode_tiled_fn();
-  if (!enc) return (int)cudaErrorNotSupported;
-  const cuuint64_t gdim[2] = {(cuuint64_t)2 * n2, (cuuint64_t)rows};
-  const cuuint64_t gstr[1] = {(cuuint64_t)n2 * 16};
-  const cuuint32_t box[2] = {(cuuint32_t)(2 * s1::KC), (cuuint32_t)box_rows};
-  const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
-}
-
-template <int KSP_MAX>
+template <int KSP_MAX, bool S3M>
 static int launch_p0(const s1::Plan &pl, const s1::Params &P, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(s1::p0_kernel<KSP_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  cudaError_t e = cudaFuncSetAttribute(s1::p0_kernel<KSP_MAX, S3M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
   const int n2 = P.d.nao * P.d.nao;
   CUtensorMap tmV, tmZ;
-  int rc = make_rows_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, n2, 8 * pl.ntc);
+  int rc = gwp::make_tensor_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, n2, 8 * pl.ntc);
   if (rc) return rc;
-  rc = make_rows_map(&tmZ, P.scratch, (size_t)gwp::gw_num_sms() * 2 * s1::TM, n2, s1::TM);
+  rc = gwp::make_tensor_map(&tmZ, P.scratch, (size_t)gwp::gw_num_sms() * 2 * s1::TM, n2, s1::TM);
   if (rc) return rc;
   cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof(cfg));
   cudaLaunchAttribute attr[1];
@@ -561,11 +527,11 @@ static int launch_p0(const s1::Plan &pl, const s1::Params &P, cudaStream_t st) {
     // co-resident clusters (a GPC with an odd number of free SMs leaves one unpaired)
     cfg.gridDim = dim3(pl.cs * ncl, 1, 1);
     int maxcl = 0;
-    if (cudaOccupancyMaxActiveClusters(&maxcl, s1::p0_kernel<KSP_MAX>, &cfg) == cudaSuccess && maxcl > 0 && maxcl < ncl) ncl = maxcl;
+    if (cudaOccupancyMaxActiveClusters(&maxcl, s1::p0_kernel<KSP_MAX, S3M>, &cfg) == cudaSuccess && maxcl > 0 && maxcl < ncl) ncl = maxcl;
     else cudaGetLastError();
   }
   cfg.gridDim = dim3(pl.cs * ncl, 1, 1);
-  e = cudaLaunchKernelEx(&cfg, s1::p0_kernel<KSP_MAX>, P, tmV, tmZ);
+  e = cudaLaunchKernelEx(&cfg, s1::p0_kernel<KSP_MAX, S3M>, P, tmV, tmZ);
   return (int)e;
 }
 
@@ -580,7 +546,12 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.main_off = pl.main_off; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
-  if (pl.ksp_max == 7) return launch_p0<7>(pl, P, st);
-  if (pl.ksp_max == 13) return launch_p0<13>(pl, P, st);
-  return launch_p0<16>(pl, P, st);
+  if (pl.s3m) {
+    if (pl.ksp_max == 7) return launch_p0<7, true>(pl, P, st);
+    if (pl.ksp_max == 13) return launch_p0<13, true>(pl, P, st);
+    return launch_p0<16, true>(pl, P, st);
+  }
+  if (pl.ksp_max == 7) return launch_p0<7, false>(pl, P, st);
+  if (pl.ksp_max == 13) return launch_p0<13, false>(pl, P, st);
+  return launch_p0<16, false>(pl, P, st);
 }

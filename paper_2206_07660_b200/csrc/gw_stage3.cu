@@ -9,7 +9,6 @@
 // A persistent CTA owns one (t,k): it loops over q and over Q panels, and keeps the nao x nao Sigma accumulator in
 // registers for the whole item, so the q-sum needs no cross-CTA reduction and the result is deterministic.
 // U and T live in two per-CTA slabs of the workspace (L2 resident); the raw V2 block is the only big stream.
-#include <cuda.h>
 #include "gw_pipe.cuh"
 
 // GW_SYM_TR bookkeeping shared by both stage-3 kernels: the k <= -k half of the mesh (only for the full q range, nk <= 128)
@@ -49,13 +48,7 @@ struct Params {
 // Main jobs are written by TMA with the 128-byte swizzle (16-byte unit u of row r sits at u ^ (r & 7)):
 //   A = W[TM rows][8 K]: 32 rows x 128 B;   B = one 1 KB box per n-tile of the chunk: [8 K rows][8 columns of V2].
 // Lane group g reads row / column rho(g) = (g >> 1) + 4 (g & 1) of its tile, so a quarter-warp touches eight different units.
-__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
-               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(gwp::smem_u32(bar)), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(gwp::smem_u32(bar)), "r"(bytes) : "memory");
-}
+using gwp::tma_load_2d; using gwp::mbar_expect_tx;
 
 template <int NJM>
 __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int rho) {
@@ -329,7 +322,7 @@ static Plan make_plan(const gw_problem *p) {
 }  // namespace s3
 
 
-double gw_stage3_flops(const gw_problem *p) {
+static double s3_generic_flops(const gw_problem *p) {
   s3::Plan pl = s3::make_plan(p);
   if (!pl.ok) return 0.0;
   GwDims d = gw_dims(p);
@@ -347,17 +340,15 @@ double gw_stage3_flops(const gw_problem *p) {
   return tiles * (double)d.nq * fill_kirr(d, tmp) * d.ntau * 2048.0;
 }
 
-namespace s3w { static int make_map(CUtensorMap *map, const void *base, size_t rows, int ncplx, int box_rows); }
-
 template <int KSP_MAX, int NCT>
 static int launch_sigma(const s3::Plan &pl, const s3::Params &P, cudaStream_t st) {
   cudaError_t e = cudaFuncSetAttribute(s3::sigma_kernel<KSP_MAX, NCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return (int)e;
   // tensor maps of the main jobs: Wt as [ntau*nq*naux rows][naux complex] (box 32 x 8), V as [nk*nk*naux rows][nao² complex] (box 8 x 8)
   CUtensorMap tmW, tmV;
-  int rc = s3w::make_map(&tmW, P.Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, s3::TM);
+  int rc = gwp::make_tensor_map(&tmW, P.Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, s3::TM);
   if (rc) return rc;
-  rc = s3w::make_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, s3::KC);
+  rc = gwp::make_tensor_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, s3::KC);
   if (rc) return rc;
   s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR_WS, pl.smem, st>>>(P, tmW, tmV);
   return (int)cudaGetLastError();
@@ -388,34 +379,51 @@ static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigm
 }  // namespace s3
 
 // =====================================================================================================================
-// s3w — warp-specialised variant of the stage-3 kernel for the nao = 25..28 class (ksp = 7, 4 x 4 tiles over nao).
-// Same algebra as s3::sigma_kernel; the work of one (q, Q-panel) unit is split between warp roles that run concurrently:
-//   main warps 0-7  : U = W·V2 (N chunk by N chunk, accumulators in registers), U^T stored to slabU[unit & 1]
+// s3w — warp-specialised stage-3 kernel for the production basis classes nao = 25..28 (KSP = 7 k-steps over nao, 4 x 4 Sigma
+// tiles) and nao = 49..52 (KSP = 13, 7 x 7 tiles).  Same algebra as s3::sigma_kernel; the work of one (q, Q-panel) unit is
+// split between warp roles that run concurrently:
+//   main warps 0-7  : U = W·V2 (N chunk by N chunk, accumulators in registers), U^T stored to slabU[unit & 1].
+//                     Complex tile products use the 3M scheme (three real DMMAs per complex 8x8x4 product instead of four):
+//                       K1 += Ar·Br,  K2 += Ai·Bi,  K3 += (Ar+Ai)·(Br+Bi);   Re U = K1 − K2,  Im U = K3 − K1 − K2
+//                     with three real accumulator sets per tile (warp tile 2 x 4 tiles = 96 registers) and the two operand sums
+//                     formed in registers after the fragment loads (one DADD per fragment) (measured against the 4-real-GEMM scheme in
+//                     profiles/r02_3m_vs_4m.md).
 //   aux warps 8-11  : for the PREVIOUS unit: pass A (T = G·U, slabU -> slabT) and the final contraction
-//                     Sigma += Σ_(Q,a) V1[Q][i][a] T[Q][a][j]; the nao x nao Sigma accumulator of the item lives in
-//                     their registers (warp w owns column tile w of all four row tiles)
-//   producer warps  : 12-14 feed the main ring (W panel + V2 chunk), 15 feeds the aux ring (G, slabU rows, V1 + slabT)
+//                     Sigma += Σ_(Q,a) V1[Q][i][a] T[Q][a][j] (4-real-GEMM scheme); the nao x nao Sigma accumulator of the item
+//                     lives in their registers (Sigma tile w + 4 i belongs to aux warp w)
+//   producer warps  : one thread of warp 12 feeds the main ring by TMA (W panel + V2 chunk), warp 15 feeds the aux ring
+//                     (G, slabU rows, V1 + slabT) with cp.async
 // so the DMMA pipe never drains at a phase change and the small-K phases run beside the big GEMM.
 // =====================================================================================================================
 namespace s3w {
 
 using gwp::FastDiv;
 constexpr int NMAINW = 8, NAUXW = 4, NTHR = 512;
-constexpr int T_MPROD = 384, N_MPROD = 96, T_APROD = 480, N_APROD = 32;
-constexpr int KC = 8, MT_W = 2, NJ = 7, TM = 32, KSP = 7, NDT = 4;
-constexpr int AMT = 1, AROWS = 32 * AMT;      // pass A: m-tiles per aux warp and rows per job (2 measured slower)
+constexpr int T_APROD = 480, N_APROD = 32;
+constexpr int KC = 8, MT_W = 2, NJ = 4, TM = 32;
+constexpr int AROWS = 32;                     // pass A: rows per job (one m-tile per aux warp)
 constexpr int NST_MAX = 8, AST_MAX = 4;
-constexpr int REG_MAIN = 176, REG_AUX = 120, REG_PROD = 40;
+constexpr int REG_MAIN = 152, REG_AUX = 168, REG_PROD = 40;   // 256*152 + 128*168 + 128*40 = 65536
+
+// compile-time geometry of a basis class: KSP = ceil(nao/4)
+template <int KSP> struct Geo {
+  static constexpr int NDT = (KSP + 1) / 2;                       // 8-wide tiles over nao
+  static constexpr int NTA = (NDT * NDT + NAUXW - 1) / NAUXW;     // Sigma tiles per aux warp
+  static constexpr int KH = KSP <= 8 ? 1 : 3;                     // K pieces of one Q's final contraction (shared-memory budget)
+  static constexpr int KSPF = (KSP + KH - 1) / KH;                // k-steps per piece (the last piece may have fewer)
+  static constexpr int LDP = (4 * KSP) % 8 == 0 ? 4 * KSP + 4 : 4 * KSP;       // ≡ 4 (mod 8): conflict-free K-contiguous fragments
+  static constexpr int LDPF = (4 * KSPF) % 8 == 0 ? 4 * KSPF + 4 : 4 * KSPF;
+  static constexpr int LDT = 8 * NDT + 2;                         // ≡ 2 (mod 8): conflict-free K-major fragments
+  static constexpr int AUX_UNITS = (AROWS * LDP > 8 * NDT * LDPF + 4 * KSPF * LDT + 8) ? AROWS * LDP : 8 * NDT * LDPF + 4 * KSPF * LDT + 8;
+};
 
 struct Params {
   GwDims d;
   const c128 *V, *G, *Wt;
   c128 *Sigma, *scratch;
   int nqt, nitems;
-  int ldp, ldt;           // row strides: pass / G / V1 tiles (K contiguous), T tiles (K major)
   int nnt, nchunk, cht;   // n-tiles over nao², N chunks, n-tiles per chunk
-  int ldb;                // row stride of the main-job B part
-  int main_units, aux_units, nstage, astage;
+  int main_units, nstage, astage;
   int main_off;           // offset of the main ring in the 1024-byte aligned dynamic shared memory (complex elements)
   size_t slab_units;      // complex elements per slab (three slabs per CTA: U0, U1, T)
   int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
@@ -424,58 +432,41 @@ struct Params {
   FastDiv fd_nao;
 };
 
-struct Ring {
-  uint64_t *full, *empty;
-  int nstage; unsigned it;     // `it` = stage index, `ph` = parity of the current round (no integer division per job)
-  unsigned ph;
-  __device__ __forceinline__ int stage() const { return (int)it; }
-  __device__ __forceinline__ void advance() { if (++it == (unsigned)nstage) { it = 0; ph ^= 1u; } }
-  __device__ __forceinline__ int acquire() { const int s = stage(); gwp::mbar_wait(empty + s, ph ^ 1u); return s; }
-  __device__ __forceinline__ void commit() { gwp::cp_async_arrive_noinc(full + stage()); advance(); }
-  __device__ __forceinline__ int wait() { const int s = stage(); gwp::mbar_wait(full + s, ph); return s; }
-  __device__ __forceinline__ void release() { __syncwarp(); if ((threadIdx.x & 31) == 0) gwp::mbar_arrive(empty + stage()); advance(); }
-};
-
-__device__ __forceinline__ void cpa(unsigned dst, const void *src, int nbytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(nbytes));
-}
-// with an L2 eviction policy: the V blocks are shared by the ~100 CTAs that work on the same k (evict last)
-__device__ __forceinline__ void cpa_hint(unsigned dst, const void *src, int nbytes, uint64_t pol) {
-  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;\n" ::"r"(dst), "l"(src), "r"(nbytes), "l"(pol));
-}
-__device__ __forceinline__ uint64_t policy_evict_last() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p)); return p; }
+using gwp::Ring;
 
 // main job in shared memory (both parts written by TMA with the 128-byte swizzle: 16-byte unit u of row r sits at u ^ (r & 7)):
 //   A = W[TM rows][8 K]                    32 rows x 128 B
 //   B = one 1 KB box per n-tile: [8 K rows][8 columns]
 // Lane group g reads row / column rho(g) = (g >> 1) + 4 (g & 1) of its tile, so a quarter-warp touches eight different units.
+// 3M: k1 += Ar Br, k2 += Ai Bi, k3 += (Ar+Ai)(Br+Bi).
 template <int NJM, int NSTRIDE = 4, int MTW = MT_W>
-__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&accr)[MT_W][NJ][2], double (&acci)[MT_W][NJ][2], int c, int rho) {
+__device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, double (&k1)[MT_W][NJ][2], double (&k2)[MT_W][NJ][2],
+                                             double (&k3)[MT_W][NJ][2], int c, int rho) {
 #pragma unroll
   for (int ks = 0; ks < KC / 4; ks++) {
     const int kr = 4 * ks + c;
     const int u = kr ^ rho;
     c128 a[MTW], b[NJM];
+    double as[MTW];
 #pragma unroll
     for (int i = 0; i < MTW; i++) a[i] = sAw[i * 8 * KC + u];
     const c128 *bk = sBw + kr * 8 + u;                  // row kr of the box, column rho swizzled by the row
 #pragma unroll
     for (int jn = 0; jn < NJM; jn++) b[jn] = bk[64 * NSTRIDE * jn];
 #pragma unroll
-    for (int jn = 0; jn < NJM; jn++)
+    for (int i = 0; i < MTW; i++) as[i] = a[i].x + a[i].y;
 #pragma unroll
-      for (int i = 0; i < MTW; i++) cmma(accr[i][jn], acci[i][jn], a[i], b[jn]);
+    for (int jn = 0; jn < NJM; jn++) {
+      const double bs = b[jn].x + b[jn].y;
+#pragma unroll
+      for (int i = 0; i < MTW; i++) {
+        dmma884(k1[i][jn][0], k1[i][jn][1], a[i].x, b[jn].x);
+        dmma884(k2[i][jn][0], k2[i][jn][1], a[i].y, b[jn].y);
+        dmma884(k3[i][jn][0], k3[i][jn][1], as[i], bs);
+      }
+    }
   }
 }
-
-__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t pol) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n"
-               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(gwp::smem_u32(bar)), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(gwp::smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ uint64_t policy_evict_normal() { uint64_t p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;\n" : "=l"(p)); return p; }
 
 // aux ring jobs (producer warp 15)
 __device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd) {
@@ -487,18 +478,29 @@ __device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row
     cp_async16(stage + r * ldp + a, s + i);
   }
 }
-// final job for one Q: A = V1[Q] (nao x nao, [i][a]) -> stage[i][ldp]; B = T[Q] ([a][j]) -> [a][ldt], K rows a >= nao zero filled
-__device__ __forceinline__ void issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldp, int ldt, FastDiv fd) {
-  const int n2 = nao * nao, lane = threadIdx.x - T_APROD;
-  for (int i = lane; i < n2; i += N_APROD) {
-    const int r = (int)fd.div((unsigned)i), a = i - r * nao;
-    cp_async16(stage + r * ldp + a, Aq + i);
+// final job for the K range [a0, a0 + 4 ksn) of one Q: A = V1[Q][i][a0..] -> stage[i][ldpf]; B = T[Q][a0..][j] -> [a - a0][ldt];
+// K beyond nao is zero filled
+template <int NDT>
+__device__ __forceinline__ void issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldpf, int ldt, int a0, int ksn, FastDiv fd) {
+  const int lane = threadIdx.x - T_APROD, kw = 4 * ksn;
+  if (a0 == 0 && kw >= nao) {                            // whole rows (one piece per Q)
+    for (int i = lane; i < nao * nao; i += N_APROD) {
+      const int r = (int)fd.div((unsigned)i), a = i - r * nao;
+      cp_async16(stage + r * ldpf + a, Aq + i);
+    }
+  } else {
+    const FastDiv fk((unsigned)kw);
+    for (int i = lane; i < nao * kw; i += N_APROD) {
+      const int r = (int)fk.div((unsigned)i), cc = i - r * kw;
+      const bool ok = a0 + cc < nao;
+      gwp::cp_async16_zfill(stage + r * ldpf + cc, ok ? Aq + r * nao + a0 + cc : Aq, ok);
+    }
   }
-  c128 *sB = stage + 8 * NDT * ldp;
-  for (int i = lane; i < 4 * KSP * nao; i += N_APROD) {
+  c128 *sB = stage + 8 * NDT * ldpf;
+  for (int i = lane; i < kw * nao; i += N_APROD) {
     const int r = (int)fd.div((unsigned)i);
-    const bool ok = r < nao;
-    gwp::cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + i : Bq, ok);
+    const bool ok = a0 + r < nao;
+    gwp::cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + (size_t)a0 * nao + i : Bq, ok);
   }
 }
 __device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao, int ldp, FastDiv fd) {
@@ -508,30 +510,55 @@ __device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao,
   }
 }
 
-// aux warps: Sigma tiles (mi, nj = w), mi = 0..3:  acc[mi] += A[mi rows][K] · B[K][8 w ..]; one B fragment per k-step
-__device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[NDT][2], double (&sgi)[NDT][2], int ldp, int ldt, int w) {
+// aux warps: Sigma tiles t = w + 4 i (row tile t / NDT, column tile t % NDT):  acc[i] += A[row tile][K] · B[K][column tile] over
+// the ksn k-steps of the job.  For NDT = 4 the warp's tiles share one column tile: one B fragment per k-step feeds four tiles.
+template <int KSP>
+__device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[Geo<KSP>::NTA][2], double (&sgi)[Geo<KSP>::NTA][2], int w, int ksn) {
+  using Gm = Geo<KSP>;
+  constexpr int NDT = Gm::NDT, NTA = Gm::NTA, ldpf = Gm::LDPF, ldt = Gm::LDT;
   const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
-  const c128 *ap = stage + g * ldp + c;
-  const c128 *bp = stage + 8 * NDT * ldp + c * ldt + 8 * w + g;
+  const c128 *ap = stage + g * ldpf + c;
+  const c128 *bp = stage + 8 * NDT * ldpf + c * ldt + g;
+  if constexpr (NDT == 4) {
 #pragma unroll
-  for (int ks = 0; ks < KSP; ks++) {
-    const c128 b = bp[4 * ks * ldt];
-    c128 a[NDT];
+    for (int ks = 0; ks < Gm::KSPF; ks++) {
+      const c128 b = bp[4 * ks * ldt + 8 * w];
+      c128 a[NDT];
 #pragma unroll
-    for (int mi = 0; mi < NDT; mi++) a[mi] = ap[8 * mi * ldp + 4 * ks];
+      for (int mi = 0; mi < NDT; mi++) a[mi] = ap[8 * mi * ldpf + 4 * ks];
 #pragma unroll
-    for (int mi = 0; mi < NDT; mi++) cmma(sgr[mi], sgi[mi], a[mi], b);
+      for (int mi = 0; mi < NDT; mi++) cmma(sgr[mi], sgi[mi], a[mi], b);
+    }
+  } else {
+    int aoff[NTA], boff[NTA];
+#pragma unroll
+    for (int i = 0; i < NTA; i++) {
+      const int t = min(w + NAUXW * i, NDT * NDT - 1), mi = t / NDT, nj = t - mi * NDT;
+      aoff[i] = 8 * mi * ldpf; boff[i] = 8 * nj;
+    }
+#pragma unroll
+    for (int ks = 0; ks < Gm::KSPF; ks++) {
+      if (ks < ksn) {
+#pragma unroll
+        for (int i = 0; i < NTA; i++) {
+          if (w + NAUXW * i < NDT * NDT) cmma(sgr[i], sgi[i], ap[aoff[i] + 4 * ks], bp[4 * ks * ldt + boff[i]]);
+        }
+      }
+    }
   }
 }
 
+template <int KSP>
 __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmV) {
+  using Gm = Geo<KSP>;
+  constexpr int NDT = Gm::NDT, NTA = Gm::NTA, ldp = Gm::LDP, ldpf = Gm::LDPF, ldt = Gm::LDT, AUXU = Gm::AUX_UNITS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   // the TMA destinations (128-byte swizzle) need 1024-byte alignment: the launch asks for 1 KB of slack
   c128 *smem = reinterpret_cast<c128 *>(smem_raw + ((1024u - (gwp::smem_u32(smem_raw) & 1023u)) & 1023u));
   const GwDims d = P.d;
-  const int nao = d.nao, naux = d.naux, n2 = nao * nao, ldp = P.ldp, ldt = P.ldt;
-  c128 *sG = smem;                                   // [32][ldp]: sG[a][b] = G[t][k-q][a][b]
-  c128 *sAux = sG + 8 * NDT * ldp;                   // astage x aux_units
+  const int nao = d.nao, naux = d.naux, n2 = nao * nao;
+  c128 *sG = smem;                                   // [8 NDT][ldp]: sG[a][b] = G[t][k-q][a][b]
+  c128 *sAux = sG + 8 * NDT * ldp;                   // astage x AUXU
   c128 *sMain = smem + P.main_off;                   // nstage x main_units, 1024-byte aligned stages
   __shared__ uint64_t bars[2 * NST_MAX + 2 * AST_MAX + 6];
   uint64_t *full_m = bars, *empty_m = bars + NST_MAX, *full_a = bars + 2 * NST_MAX, *empty_a = full_a + AST_MAX;
@@ -557,13 +584,11 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
   if (w >= NMAINW + NAUXW) {
     gwp::reg_dec<REG_PROD>();
     if (w < 15) {
-      // ---- main-ring producer: ONE thread issues the TMA box loads of a job (the W panel K slice; one 8 x 8 box of V2 per
-      //      n-tile of the chunk) and arms the stage's mbarrier with the byte count ----
+      // ---- main-ring producer: the 32 lanes of warp 12 issue the TMA box loads of a job in one go (lane 0 arms the stage's
+      //      mbarrier with the byte count, lanes < ntc load one 8 x 8 box of V2 each, lane 31 loads the W panel K slice) ----
       if (w == NMAINW + NAUXW) {
-        // the 32 lanes of this warp issue the boxes of a job in one go: lane 0 arms the barrier, lanes < ntc load one V box
-        // each, lane 31 loads the W box
         Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
-        const uint64_t polA = policy_evict_normal(), polB = policy_evict_last();
+        const uint64_t polA = gwp::policy_evict_normal(), polB = gwp::policy_evict_last();
         for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
           const int t = item % d.ntau, k = P.kof(item / d.ntau);
           for (int ql = 0; ql < d.nq; ql++) {
@@ -576,10 +601,10 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
                 for (int j = 0; j < nmain; j++) {
                   const int s = rm.acquire();
                   const unsigned dst = gwp::smem_u32(sMain + s * P.main_units);
-                  if (lane == 0) mbar_expect_tx(full_m + s, (unsigned)(TM * KC * 16 + ntc * 1024));
+                  if (lane == 0) gwp::mbar_expect_tx(full_m + s, (unsigned)(TM * KC * 16 + ntc * 1024));
                   __syncwarp();
-                  if (lane == 31) tma_load_2d(dst, &tmW, 2 * KC * j, yW + qt * TM, full_m + s, polA);
-                  if (lane < ntc) tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)lane, &tmV, 16 * (nt0 + lane), yV + KC * j, full_m + s, polB);
+                  if (lane == 31) gwp::tma_load_2d(dst, &tmW, 2 * KC * j, yW + qt * TM, full_m + s, polA);
+                  if (lane < ntc) gwp::tma_load_2d(dst + TM * KC * 16 + 1024u * (unsigned)lane, &tmV, 16 * (nt0 + lane), yV + KC * j, full_m + s, polB);
                   rm.advance();
                 }
               }
@@ -588,7 +613,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
         }
       }
     } else {
-      // ---- aux-ring producer: G per q, U^T rows of the finished unit (pass A), then V1[Q] + T[Q] per Q (final) ----
+      // ---- aux-ring producer: G per q, U^T rows of the finished unit (pass A), then V1[Q] + T[Q] per Q and K piece (final) ----
       Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
       unsigned un = 0;
       for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
@@ -605,15 +630,19 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
             gwp::mbar_wait(uready + (un & 1u), (un >> 1) & 1u);
             for (int j = 0; j < npass; j++) {
               const int s = ra.acquire();
-              issue_rows(sAux + s * P.aux_units, U, j * AROWS, rows, nao, ldp, P.fd_nao);
+              issue_rows(sAux + s * AUXU, U, j * AROWS, rows, nao, ldp, P.fd_nao);
               ra.commit();
             }
             gwp::mbar_wait(bar_phase, un & 1u);                     // T of this unit is in slabT
             const c128 *V1t = V1 + (size_t)Q0 * n2;
             for (int j = 0; j < tm_rows; j++) {
-              const int s = ra.acquire();
-              issue_final(sAux + s * P.aux_units, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldp, ldt, P.fd_nao);
-              ra.commit();
+#pragma unroll
+              for (int h = 0; h < Gm::KH; h++) {
+                const int s = ra.acquire();
+                issue_final<NDT>(sAux + s * AUXU, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldpf, ldt, 4 * Gm::KSPF * h,
+                                 min(Gm::KSPF, KSP - Gm::KSPF * h), P.fd_nao);
+                ra.commit();
+              }
             }
           }
         }
@@ -622,47 +651,53 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
     }
   } else if (w >= NMAINW) {
     // ============================================ aux warps ============================================
-    gwp::reg_dec<REG_AUX>();
+    gwp::reg_inc<REG_AUX>();
     const int wa = w - NMAINW, g = lane >> 2, c = lane & 3;
     Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
     unsigned un = 0;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
       const int t = item % d.ntau, k = P.kof(item / d.ntau);
-      double sgr[NDT][2], sgi[NDT][2];
+      double sgr[NTA][2], sgi[NTA][2];
 #pragma unroll
-      for (int i = 0; i < NDT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+      for (int i = 0; i < NTA; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
       for (int ql = 0; ql < d.nq; ql++) {
         for (int qt = 0; qt < P.nqt; qt++, un++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + AROWS - 1) / AROWS;
           gwp::mbar_wait(bar_g, un & 1u);
           for (int j = 0; j < npass; j++) {
             const int s = ra.wait();
-            gwp::pass_compute_exact_mt<KSP, true, AMT>(sAux + s * P.aux_units, sG, slabT, j * AROWS, rows, nao, ldp, wa, P.fd_nao);
+            gwp::pass_compute_exact_mt<KSP, true, 1>(sAux + s * AUXU, sG, slabT, j * AROWS, rows, nao, ldp, wa, P.fd_nao);
             ra.release();
           }
           __threadfence(); __syncwarp();
           if (lane == 0) { gwp::mbar_arrive(bar_phase); gwp::mbar_arrive(ufree + (un & 1u)); }
           for (int j = 0; j < tm_rows; j++) {
-            const int s = ra.wait();
-            final_compute(sAux + s * P.aux_units, sgr, sgi, ldp, ldt, wa);
-            ra.release();
+#pragma unroll
+            for (int h = 0; h < Gm::KH; h++) {
+              const int s = ra.wait();
+              final_compute<KSP>(sAux + s * AUXU, sgr, sgi, wa, min(Gm::KSPF, KSP - Gm::KSPF * h));
+              ra.release();
+            }
           }
         }
       }
-      // Sigma[t][k] = -(1/N_k) acc: this warp's column tile of the four row tiles
+      // Sigma[t][k] = -(1/N_k) acc: this warp's tiles
       const double pref = -1.0 / (double)d.nk;
       const int kn = gw_ksub(d, 0, k);
       const int ncopy = (P.nkeff < d.nk && kn != k) ? 2 : 1;  // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
-      const int j0 = 8 * wa + 2 * c;
       for (int cp = 0; cp < ncopy; cp++) {
         c128 *out = P.Sigma + ((size_t)t * d.nk + (cp ? kn : k)) * n2;
         const double prefi = cp ? -pref : pref;
 #pragma unroll
-        for (int mi = 0; mi < NDT; mi++) {
-          const int i = 8 * mi + g;
-          if (i < nao) {
-            if (j0 < nao) out[i * nao + j0] = make_double2(pref * sgr[mi][0], prefi * sgi[mi][0]);
-            if (j0 + 1 < nao) out[i * nao + j0 + 1] = make_double2(pref * sgr[mi][1], prefi * sgi[mi][1]);
+        for (int ti = 0; ti < NTA; ti++) {
+          const int tile = wa + NAUXW * ti;
+          if (tile < NDT * NDT) {
+            const int mi = tile / NDT, nj = tile - mi * NDT;
+            const int i = 8 * mi + g, j0 = 8 * nj + 2 * c;
+            if (i < nao) {
+              if (j0 < nao) out[i * nao + j0] = make_double2(pref * sgr[ti][0], prefi * sgi[ti][0]);
+              if (j0 + 1 < nao) out[i * nao + j0 + 1] = make_double2(pref * sgr[ti][1], prefi * sgi[ti][1]);
+            }
           }
         }
       }
@@ -679,8 +714,9 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
         for (int qt = 0; qt < P.nqt; qt++, un++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), mtc = (tm_rows + 7) / 8;
           c128 *U = slabU + (size_t)(un & 1u) * P.slab_units;
-          // tile ownership: full panels as in s3::sigma_kernel; the ragged last panel (<= 16 rows) is shared by all eight
-          // warps (m-tiles 0 (and 1), every 8th n-tile each), so it costs time in proportion to its rows
+          // tile ownership.  Full panels: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile of the chunk (the column
+          // group is rotated by mh, so the two main warps of a scheduler carry different groups).  The ragged last panel (<= 16 rows)
+          // is shared by all eight warps (m-tiles 0 (and 1), every 8th n-tile each): it costs time in proportion to its rows.
           const bool narrow = mtc <= 2;
           const int mh = narrow ? 0 : (w >> 2);
           const int noff = narrow ? w : (((w & 3) - mh + 4) & 3);
@@ -690,38 +726,32 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
             const int nt0 = ch * P.cht, ntc = min(P.cht, P.nnt - nt0), n0 = nt0 * 8;
             const int njm = (ntc > noff) ? (ntc - noff + nstride - 1) / nstride : 0;
             const bool active = (mh * MT_W < mtc) && njm > 0;
-            double accr[MT_W][NJ][2], acci[MT_W][NJ][2];
+            double k1[MT_W][NJ][2], k2[MT_W][NJ][2], k3[MT_W][NJ][2];
 #pragma unroll
             for (int i = 0; i < MT_W; i++)
 #pragma unroll
-              for (int j = 0; j < NJ; j++) { accr[i][j][0] = accr[i][j][1] = 0.0; acci[i][j][0] = acci[i][j][1] = 0.0; }
+              for (int j = 0; j < NJ; j++) { k1[i][j][0] = k1[i][j][1] = 0.0; k2[i][j][0] = k2[i][j][1] = 0.0; k3[i][j][0] = k3[i][j][1] = 0.0; }
             for (int jb = 0; jb < nmain; jb++) {
               const int s = rm.wait();
               if (active) {
                 const c128 *sAw = sMain + s * P.main_units + (8 * mh * MT_W + rho) * KC;
                 const c128 *sBw = sMain + s * P.main_units + TM * KC + 64 * noff;
                 if (narrow) {
-                  if (mtw == 1 && njm == 3) main_compute<3, 8, 1>(sAw, sBw, accr, acci, c, rho);
-                  else if (mtw == 1 && njm == 2) main_compute<2, 8, 1>(sAw, sBw, accr, acci, c, rho);
-                  else if (mtw == 1 && njm == 4) main_compute<4, 8, 1>(sAw, sBw, accr, acci, c, rho);
-                  else if (njm == 4) main_compute<4, 8, 2>(sAw, sBw, accr, acci, c, rho);
-                  else if (njm == 3) main_compute<3, 8, 2>(sAw, sBw, accr, acci, c, rho);
-                  else if (njm == 2) main_compute<2, 8, 2>(sAw, sBw, accr, acci, c, rho);
-                  else main_compute<1, 8, 2>(sAw, sBw, accr, acci, c, rho);
+                  if (mtw == 1 && njm == 2) main_compute<2, 8, 1>(sAw, sBw, k1, k2, k3, c, rho);
+                  else if (mtw == 1) main_compute<1, 8, 1>(sAw, sBw, k1, k2, k3, c, rho);
+                  else if (njm == 2) main_compute<2, 8, 2>(sAw, sBw, k1, k2, k3, c, rho);
+                  else main_compute<1, 8, 2>(sAw, sBw, k1, k2, k3, c, rho);
                 }
-                else if (njm == 7) main_compute<7>(sAw, sBw, accr, acci, c, rho);
-                else if (njm == 6) main_compute<6>(sAw, sBw, accr, acci, c, rho);
-                else if (njm == 5) main_compute<5>(sAw, sBw, accr, acci, c, rho);
-                else if (njm == 4) main_compute<4>(sAw, sBw, accr, acci, c, rho);
-                else if (njm == 3) main_compute<3>(sAw, sBw, accr, acci, c, rho);
-                else if (njm == 2) main_compute<2>(sAw, sBw, accr, acci, c, rho);
-                else main_compute<1>(sAw, sBw, accr, acci, c, rho);
+                else if (njm == 4) main_compute<4>(sAw, sBw, k1, k2, k3, c, rho);
+                else if (njm == 3) main_compute<3>(sAw, sBw, k1, k2, k3, c, rho);
+                else if (njm == 2) main_compute<2>(sAw, sBw, k1, k2, k3, c, rho);
+                else main_compute<1>(sAw, sBw, k1, k2, k3, c, rho);
               }
               rm.release();
             }
             // slabU[un & 1] was read by pass A of unit un-2
             if (ch == 0 && un >= 2) gwp::mbar_wait(ufree + (un & 1u), ((un >> 1) - 1u) & 1u);
-            // store U^T: element (Q, n=(b,j)) -> U[(Q*nao + j)*nao + b]
+            // store U^T: element (Q, n=(b,j)) -> U[(Q*nao + j)*nao + b];  Re U = K1 - K2, Im U = K3 - K1 - K2
 #pragma unroll
             for (int i = 0; i < MT_W; i++) {
               const int Ql = 8 * (mh * MT_W + i) + rho;            // accumulator row g holds panel row rho(g)
@@ -733,7 +763,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
                     const int n = n0 + 8 * (noff + nstride * jn) + c + 4 * e;   // accumulator columns 2c, 2c+1 hold columns c, c+4
                     if (n < n2) {
                       const int b = (int)P.fd_nao.div((unsigned)n), j = n - b * nao;
-                      U[((size_t)Ql * nao + j) * nao + b] = make_double2(accr[i][jn][e], acci[i][jn][e]);
+                      U[((size_t)Ql * nao + j) * nao + b] = make_double2(k1[i][jn][e] - k2[i][jn][e], k3[i][jn][e] - k1[i][jn][e] - k2[i][jn][e]);
                     }
                   }
                 }
@@ -748,31 +778,33 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
   }
 }
 
-struct Plan { int nqt, nitems, ldp, ldt, nnt, nchunk, cht, ldb, main_units, aux_units, nstage, astage, main_off, grid; size_t smem, slab_units, work_bytes; bool ok; };
+struct Plan { int ksp, nqt, nitems, nnt, nchunk, cht, main_units, nstage, astage, main_off, grid; size_t smem, slab_units, work_bytes; bool ok; };
 
-static Plan make_plan(const gw_problem *p) {
-  Plan pl; memset(&pl, 0, sizeof(pl));
-  GwDims d = gw_dims(p);
-  if ((d.nao + 3) / 4 != KSP) { pl.ok = false; return pl; }
-  pl.ldp = 4 * KSP;                         // 28 ≡ 4 (mod 8)
-  pl.ldt = 8 * NDT + 2;
-  pl.nnt = (d.nao * d.nao + 7) / 8;
-  pl.nchunk = (pl.nnt + 4 * NJ - 1) / (4 * NJ);
-  pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
-  pl.ldb = pl.cht * 8 + 2;
-  pl.nqt = (d.naux + TM - 1) / TM;
-  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
-  pl.main_units = TM * KC + 64 * pl.cht;      // A: 32 rows x 128 B; B: one 1 KB box per n-tile of the chunk
-  const int s_pass = AROWS * pl.ldp, s_fin = 8 * NDT * pl.ldp + 4 * KSP * pl.ldt + 8;
-  pl.aux_units = s_pass > s_fin ? s_pass : s_fin;
+template <int KSP>
+static void plan_smem(Plan &pl) {
+  using Gm = Geo<KSP>;
   pl.astage = 2;
   // 1 KB of the 227 KB is alignment slack: the main stages (TMA destinations, 128-byte swizzle) start 1024-byte aligned
   const size_t cap = 225 * 1024;
-  const size_t fixed = (((size_t)8 * NDT * pl.ldp + (size_t)pl.astage * pl.aux_units) * sizeof(c128) + 1023) / 1024 * 1024;
+  const size_t fixed = (((size_t)8 * Gm::NDT * Gm::LDP + (size_t)pl.astage * Gm::AUX_UNITS) * sizeof(c128) + 1023) / 1024 * 1024;
   pl.main_off = (int)(fixed / sizeof(c128));
   pl.nstage = (int)((cap - fixed) / ((size_t)pl.main_units * sizeof(c128)));
   if (pl.nstage > 6) pl.nstage = 6;
   pl.smem = fixed + (size_t)pl.nstage * pl.main_units * sizeof(c128) + 1024;
+}
+
+static Plan make_plan(const gw_problem *p) {
+  Plan pl; memset(&pl, 0, sizeof(pl));
+  GwDims d = gw_dims(p);
+  pl.ksp = (d.nao + 3) / 4;
+  if (pl.ksp != 7 && pl.ksp != 13) { pl.ok = false; return pl; }
+  pl.nnt = (d.nao * d.nao + 7) / 8;
+  pl.nchunk = (pl.nnt + 4 * NJ - 1) / (4 * NJ);
+  pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
+  pl.nqt = (d.naux + TM - 1) / TM;
+  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
+  pl.main_units = TM * KC + 64 * pl.cht;      // A: 32 rows x 128 B; B: one 1 KB box per n-tile of the chunk
+  if (pl.ksp == 7) plan_smem<7>(pl); else plan_smem<13>(pl);
   const int nsm = gwp::gw_num_sms();
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
@@ -781,28 +813,37 @@ static Plan make_plan(const gw_problem *p) {
   return pl;
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda):
-// [rows][ncplx complex] row-major matrix, box = box_rows x 8 complex, 128-byte swizzle
-static int make_map(CUtensorMap *map, const void *base, size_t rows, int ncplx, int box_rows) {
-  typedef CUresult (*Fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
-                         const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static Fn fn = nullptr;
-  if (!fn) {
-    void *ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
-      cudaGetLastError();
-      return (int)cudaErrorNotSupported;
-    }
-    fn = (Fn)ptr;
+// executed flops: a 3M tile product of the main GEMM is 3 DMMA.8x8x4 (1536 flops), a 4M one (pass A, final) 4 (2048)
+static double flops(const gw_problem *p, const Plan &pl) {
+  GwDims d = gw_dims(p);
+  const int ndt = (pl.ksp + 1) / 2;
+  const double nmain = (d.naux + KC - 1) / KC;
+  double fl = 0.0;
+  for (int qt = 0; qt < pl.nqt; qt++) {
+    const int tm_rows = (d.naux - qt * TM) < TM ? (d.naux - qt * TM) : TM;
+    const int mtc = (tm_rows + 7) / 8;
+    const double mtiles = (mtc <= 2) ? (double)mtc : (double)((mtc + MT_W - 1) / MT_W) * MT_W;
+    fl += mtiles * pl.nnt * (KC / 4) * nmain * 1536.0;                          // main (3M)
+    fl += (double)((tm_rows * d.nao + 7) / 8) * ndt * pl.ksp * 2048.0;           // pass A
+    fl += (double)tm_rows * ndt * ndt * pl.ksp * 2048.0;                         // final
   }
-  const cuuint64_t gdim[2] = {(cuuint64_t)2 * ncplx, (cuuint64_t)rows};
-  const cuuint64_t gstr[1] = {(cuuint64_t)ncplx * 16};
-  const cuuint32_t box[2] = {(cuuint32_t)(2 * KC), (cuuint32_t)box_rows};
-  const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
+  short tmp[128];
+  return fl * (double)d.nq * fill_kirr(d, tmp) * d.ntau;
+}
+
+template <int KSP>
+static int launch_k(const Plan &pl, const Params &P, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(sigma_ws_kernel<KSP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  if (e != cudaSuccess) return (int)e;
+  // tensor maps: Wt as [ntau*nq*naux rows][naux complex], box 32 rows x 8 complex; V as [nk*nk*naux rows][nao² complex],
+  // box 8 rows x 8 complex; 128-byte swizzle, zero fill outside the arrays
+  CUtensorMap tmW, tmV;
+  int rc = gwp::make_tensor_map(&tmW, P.Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, TM);
+  if (rc) return rc;
+  rc = gwp::make_tensor_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, KC);
+  if (rc) return rc;
+  sigma_ws_kernel<KSP><<<pl.grid, NTHR, pl.smem, st>>>(P, tmW, tmV);
+  return (int)cudaGetLastError();
 }
 
 static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
@@ -812,25 +853,20 @@ static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigm
   Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ldt = pl.ldt; P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht; P.ldb = pl.ldb;
-  P.main_units = pl.main_units; P.aux_units = pl.aux_units; P.nstage = pl.nstage; P.astage = pl.astage; P.slab_units = pl.slab_units;
+  P.nqt = pl.nqt; P.nitems = pl.nitems; P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht;
+  P.main_units = pl.main_units; P.nstage = pl.nstage; P.astage = pl.astage; P.slab_units = pl.slab_units;
   P.fd_nao = FastDiv((unsigned)P.d.nao);
   P.nkeff = fill_kirr(P.d, P.kirr);
   P.main_off = pl.main_off;
-  cudaError_t e = cudaFuncSetAttribute(sigma_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
-  if (e != cudaSuccess) return (int)e;
-  // tensor maps: Wt as [ntau*nq*naux rows][naux complex], box 32 rows x 8 complex; V as [nk*nk*naux rows][nao² complex],
-  // box 8 rows x 8 complex; 128-byte swizzle, zero fill outside the arrays
-  CUtensorMap tmW, tmV;
-  int rc = make_map(&tmW, Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, TM);
-  if (rc) return rc;
-  rc = make_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, KC);
-  if (rc) return rc;
-  sigma_ws_kernel<<<pl.grid, NTHR, pl.smem, st>>>(P, tmW, tmV);
-  return (int)cudaGetLastError();
+  return pl.ksp == 7 ? launch_k<7>(pl, P, st) : launch_k<13>(pl, P, st);
 }
 
 }  // namespace s3w
+
+double gw_stage3_flops(const gw_problem *p) {
+  s3w::Plan pw = s3w::make_plan(p);
+  return pw.ok ? s3w::flops(p, pw) : s3_generic_flops(p);
+}
 
 size_t gw_stage3_workspace(const gw_problem *p) {
   s3w::Plan pw = s3w::make_plan(p);
