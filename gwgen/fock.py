@@ -7,8 +7,9 @@ G^k(τ) = U diag(g(ε,τ)) U†,  g = −e^{−ετ}/(1+e^{−βε})   (single-p
 import numpy as np
 
 
-def make_fock(cfg, mesh):
-    rng = np.random.default_rng([cfg.seed, 1])
+def make_fock(cfg, mesh, channel=0):
+    """channel: spin channel of a spin-polarised problem (an independent spectrum per channel; channel 0 is the closed-shell one)."""
+    rng = np.random.default_rng([cfg.seed, 1] if channel == 0 else [cfg.seed, 1, int(channel)])
     nk, nao = mesh.nk, cfg.nao
     neg = mesh.neg()
     nocc = nao // 2

@@ -6,7 +6,7 @@ from .configs import GWConfig, get_config
 from .mesh import KMesh
 from .grids import make_grids
 from .fock import make_fock, greens_function, density_matrix
-from .vgen import make_V
+from .vgen import make_V, to_qslab
 
 
 @dataclass
@@ -23,6 +23,26 @@ class Problem:
     gamma: np.ndarray         # [nk][nao][nao]
     V: object = None          # torch complex128 [nk][nk][naux][nao][nao] on v_device, or None
     extras: dict = field(default_factory=dict)
+
+
+def make_spin_channels(p, ns=2):
+    """Spin-polarised inputs for ns collinear channels (include/gw.h "Spin channels"; the paper's AFM MnO case):
+    channel 0 is the problem's own G / gamma, the other channels get an independent seeded spectrum (a raw problem: independent
+    seeded non-Hermitian matrices).  Returns (G [ns][ntau][nk][nao][nao], gamma [ns][nk][nao][nao])."""
+    cfg, mesh = p.cfg, p.mesh
+    Gs, gs = [p.G], [p.gamma]
+    for ch in range(1, ns):
+        if "W" in p.extras:             # raw problem
+            rng = np.random.default_rng([cfg.seed, 7, ch])
+            cplx = lambda shape, sc: (rng.normal(size=shape) + 1j * rng.normal(size=shape)) * sc
+            scale = np.exp(-6.0 * np.minimum(p.tau, cfg.beta - p.tau) / cfg.beta).reshape(-1, 1, 1, 1)
+            Gs.append(cplx(p.G.shape, 1.0 / np.sqrt(cfg.nao)) * scale)
+            gs.append(cplx(p.gamma.shape, 1.0 / np.sqrt(cfg.nao)))
+        else:
+            eps, U = make_fock(cfg, mesh, channel=ch)
+            Gs.append(greens_function(eps, U, p.tau, cfg.beta))
+            gs.append(density_matrix(eps, U, cfg.beta))
+    return np.ascontiguousarray(np.stack(Gs)), np.ascontiguousarray(np.stack(gs))
 
 
 def make_problem(cfg, v_device="cpu", with_V=True, raw=False) -> Problem:

@@ -106,3 +106,17 @@ def make_V(cfg, mesh, device="cpu", out=None, raw=False):
                 out[m2, m1] = v.transpose(1, 2)
                 done[m2, m1] = True
     return out
+
+
+def to_qslab(V, mesh, q_begin, q_end):
+    """Layout conversion only: the q-slab view of V for the shard [q_begin, q_end) (include/gw.h "V layouts"):
+    out[q - q_begin][k][0] = V[k][k+q], out[q - q_begin][k][1] = V[k+q][k]."""
+    add = mesh.add_table()
+    nk = mesh.nk
+    out = torch.empty((q_end - q_begin, nk, 2) + tuple(V.shape[2:]), dtype=V.dtype, device=V.device)
+    for q in range(q_begin, q_end):
+        for k in range(nk):
+            kq = int(add[k][q])
+            out[q - q_begin, k, 0] = V[k, kq]
+            out[q - q_begin, k, 1] = V[kq, k]
+    return out

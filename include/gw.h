@@ -64,14 +64,37 @@ typedef struct {
   int32_t spin_deg;        /* s of the spin sum in Eq. 28b: 2 = closed shell, 1 = one spin channel */
   int32_t q_begin, q_end;  /* q shard [q_begin, q_end) */
   double beta;             /* inverse temperature (informational; the grids enter through T_wt/T_tw) */
-  const gw_c128 *V;        /* device [nk][nk][naux][nao][nao]: V^{k1 k2}_{ij}(Q), Eq. 6-7 */
+  const gw_c128 *V;        /* device [nk][nk][naux][nao][nao]: V^{k1 k2}_{ij}(Q), Eq. 6-7; or a q-slab (v_layout) */
   const gw_c128 *T_wt;     /* device [nw][ntau]: bosonic τ→iΩ transform matrix, Eq. 28a */
   const gw_c128 *T_tw;     /* device [ntau][nw]: bosonic iΩ→τ transform matrix, Eq. 30 */
   void *work;              /* device scratch shared by the four calls (L2-resident intermediates, solver copies), */
   size_t work_bytes;       /*   at least gw_workspace_bytes(p) bytes, 256-byte aligned; contents are don't-care    */
   int32_t symmetry;        /* 0 = evaluate Algorithm 1 literally (default); GW_SYM_TR = the caller asserts time-reversal   */
-  int32_t reserved;        /*   symmetric inputs (see GW_SYM_TR below); must be 0                                          */
+                           /*   symmetric inputs (see GW_SYM_TR below)                                                     */
+  int32_t ns;              /* spin channels (sums over sigma): 0 or 1 = one channel; 2 = two collinear  */
+                           /*   channels (spin-polarised, e.g. the paper's AFM MnO) — see "Spin channels" below */
+  int32_t v_layout;        /* GW_V_FULL (0) or GW_V_QSLAB: how p->V is laid out — see "V layouts" below                      */
+  int32_t reserved;        /* must be 0                                                                                    */
 } gw_problem;
+
+/* Spin channels.  With ns = 2 the Green's function has two collinear spin blocks G^{sigma sigma}, sigma = up, down (no spin-orbit
+ * coupling), stored with the channel as the LEADING index: G, Sigma : [ns][ntau][nk][nao][nao];  gamma, K : [ns][nk][nao][nao].
+ *   gw_polarization : P0t = -(spin_deg/N_k) Σ_sigma Σ_k ... G^sigma(k+q,tau) ... G^sigma(k,-tau)  (Eq. 28b's Σ_{sigma sigma'} restricted
+ *                     to the non-zero blocks; the sum runs inside the stage-1 k loop).  Pass spin_deg = 1 with ns = 2; two identical
+ *                     channels with spin_deg = 1 equal one channel with spin_deg = 2.
+ *   gw_selfenergy, gw_exchange : one Sigma^sigma / K^sigma per channel from G^sigma / gamma^sigma and the common Wt (Eq. 31, 22).
+ *   gw_hartree      : J (spin independent, [nk][nao][nao]) from Σ_sigma gamma^sigma (Eq. 20's Σ_sigma1), times spin_deg.
+ * P0t, Wt, V and the transforms carry no spin index. */
+
+/* V layouts.
+ *   GW_V_FULL  : p->V is the whole tensor [nk][nk][naux][nao][nao] (block (k1,k2) at index k1*nk + k2).
+ *   GW_V_QSLAB : p->V holds only the blocks the q shard [q_begin, q_end) touches, [nq][nk][2][naux][nao][nao]:
+ *                  slot (q - q_begin, k, 0) = V[k][k+q],   slot (q - q_begin, k, 1) = V[k+q][k].
+ *                Stage 1 reads V[k][k+q] and V[k+q][k]; stages 3 and 4 read V[k][k-q] = slot (q, k-q, 1) and V[k-q][k] = slot (q, k-q, 0):
+ *                the same 2 nk blocks per q serve every stage, which is what lets V be streamed through HBM one q-slab at a time
+ *                (gw_sigma_iteration_stream; the paper reads V "a k-batch at a time").  gw_hartree needs the
+ *                diagonal blocks V[k][k], i.e. a shard that contains q = 0 (else GW_EINVAL). */
+enum { GW_V_FULL = 0, GW_V_QSLAB = 1 };
 
 /* gw_problem.symmetry flag.  Time reversal: G[t][−k] = conj(G[t][k]) and V[−k1][−k2] = conj(V[k1][k2]) element-wise (the same
  * property that makes I − P̃0(iΩ) Hermitian for the Cholesky solve; the paper exploits k ↔ −k too), together with
@@ -89,7 +112,7 @@ enum { GW_SYM_TR = 1 };
 /* Stage 1 — Eq. 28b, Algorithm 1 first k loop:
  *   P0t[t][q-q_begin][Q][Q'] = -(s/N_k) Σ_k Σ_abcd V[k][k+q][Q][d][a] G[t][k+q][a][b] V[k+q][k][Q'][b][c] G[ntau-1-t][k][c][d]
  * (the printed "-1/N_k" is the antiperiodicity sign of G(−τ); reading R1).
- *   G   : device [ntau][nk][nao][nao]      in
+ *   G   : device [ntau][nk][nao][nao]      in   ([ns][ntau][nk][nao][nao] with ns = 2, summed over the channel)
  *   P0t : device [ntau][nq][naux][naux]    out */
 int gw_polarization(const gw_problem *p, const gw_c128 *G, gw_c128 *P0t, void *stream);
 
@@ -184,6 +207,17 @@ int gw_find_mu(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, const dou
 /* Y[i] = (a_re + i a_im) X[i] + (b_re + i b_im) Y[i], i < n (damping of two iterates, F = H0 + J + K, gamma = −G(beta^-)).
  * Y is not read when b == 0.  X, Y : device, may be equal. */
 int gw_axpby(size_t n, double a_re, double a_im, const gw_c128 *X, double b_re, double b_im, gw_c128 *Y, void *stream);
+
+/* Whole iteration with V OUT OF CORE (the paper keeps V on disk / in host memory and reads it a k-batch at a
+ * time): as gw_sigma_iteration_host (all pointers HOST memory, p->V in the GW_V_FULL layout, pinned memory
+ * recommended), but V never resides in HBM as a whole: the q shard is processed in slabs of nqs q-points; the 2 nk V blocks of each
+ * q are gathered into one of TWO device slab buffers (GW_V_QSLAB layout, together at most v_budget_bytes) by cudaMemcpyAsync on an
+ * internal copy stream while the previous slab computes; stages 1-4 run per slab and Sigma / K continue their q sums across slabs in
+ * the same order as the resident evaluation (bit-identical results).
+ *   stats : host float[4] or NULL = {total ms, GB copied host->device, number of slabs, q-points per slab}
+ * Returns GW_ENOMEM if v_budget_bytes does not hold two slabs of one q-point, GW_ENOTPD / launch errors as the host call. */
+int gw_sigma_iteration_stream(const gw_problem *p, const gw_c128 *G, const gw_c128 *gamma, gw_c128 *Sigma, gw_c128 *K,
+                              size_t v_budget_bytes, float *stats, void *stream);
 
 /* Executed FP64 flops of the last configuration of each stage kernel for `p` (what the kernels actually
  * issue, padding and recomputation included; 2 flops per real FMA).  out: host double[4] = stage 1..4. */

@@ -274,3 +274,46 @@ def scgw_iteration(cfg, vb, T_wt, T_tw, fg, H0, S, G, n_target, mu_lo, mu_hi, al
     G_new = transform(fg["T_tw_f"], G_w)
     G_mix = axpby(alpha, G_new, 1.0 - alpha, G.copy())
     return dict(gamma=gamma, J=J, K=K, P0t=P0t, Wt=Wt, Sigma_t=Sigma_t, Sigma_w=Sigma_w, F=F, mu=mu, ne=ne, G_w=G_w, G_new=G_new, G=G_mix)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# collinear spin channels (PAPER.md:41 spin-orbital indices, Eq. 28b's sum over sigma sigma')
+# With no spin-orbit coupling G is block diagonal in spin, G^{sigma sigma'} = delta_{sigma sigma'} G^sigma, so Eq. 28b's double
+# spin sum keeps the terms sigma = sigma' only: P0 = sum_sigma P0[G^sigma]; Eq. 31 and Eq. 22 hold per channel with the common W;
+# Eq. 20's sum over sigma_1 adds the channels' density matrices.  Each term is one call of the single-channel routine with
+# spin_deg = 1 (the literal sum, written out).
+# ---------------------------------------------------------------------------------------------------------------------
+def _one_channel(cfg):
+    import dataclasses
+    return dataclasses.replace(cfg, spin_deg=1)
+
+
+def polarization_spin(cfg, vb, Gs):
+    """Eq. 28b for ns collinear channels.  Gs: [ns][ntau][nk][nao][nao]; the prefactor is cfg.spin_deg (pass 1 for ns = 2)."""
+    c1 = _one_channel(cfg)
+    out = None
+    for sg in range(Gs.shape[0]):
+        term = polarization(c1, vb, np.ascontiguousarray(Gs[sg]))
+        out = term if out is None else out + term
+    return cfg.spin_deg * out
+
+
+def p0t_slice_spin(cfg, vb, Gs_t, Gs_tbar, q):
+    c1 = _one_channel(cfg)
+    return cfg.spin_deg * sum(p0t_slice(c1, vb, np.ascontiguousarray(Gs_t[sg]), np.ascontiguousarray(Gs_tbar[sg]), q) for sg in range(Gs_t.shape[0]))
+
+
+def selfenergy_spin(cfg, vb, Gs, Wt):
+    """Eq. 31 per channel with the common Wt."""
+    return np.stack([selfenergy(cfg, vb, np.ascontiguousarray(Gs[sg]), Wt) for sg in range(Gs.shape[0])])
+
+
+def exchange_spin(cfg, vb, gammas):
+    """Eq. 22 per channel."""
+    return np.stack([exchange(cfg, vb, np.ascontiguousarray(gammas[sg])) for sg in range(gammas.shape[0])])
+
+
+def hartree_spin(cfg, vb, gammas):
+    """Eq. 20: the sum over sigma_1 runs over the channels (times cfg.spin_deg)."""
+    c1 = _one_channel(cfg)
+    return cfg.spin_deg * sum(hartree(c1, vb, np.ascontiguousarray(gammas[sg])) for sg in range(gammas.shape[0]))

@@ -14,6 +14,7 @@ class GWError(RuntimeError):
 
 
 GW_SYM_TR = 1   # gw_problem.symmetry flag (include/gw.h)
+GW_V_FULL, GW_V_QSLAB = 0, 1   # gw_problem.v_layout
 
 
 class _CProblem(ctypes.Structure):
@@ -23,7 +24,7 @@ class _CProblem(ctypes.Structure):
                 ("beta", ctypes.c_double),
                 ("V", ctypes.c_void_p), ("T_wt", ctypes.c_void_p), ("T_tw", ctypes.c_void_p),
                 ("work", ctypes.c_void_p), ("work_bytes", ctypes.c_size_t),
-                ("symmetry", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("symmetry", ctypes.c_int32), ("ns", ctypes.c_int32), ("v_layout", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 def lib_path():
@@ -49,6 +50,7 @@ def lib():
         L.gw_workspace_bytes.argtypes = [P]
         L.gw_workspace_bytes.restype = sz
         L.gw_sigma_iteration_host.argtypes = [P, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.gw_sigma_iteration_stream.argtypes = [P, vp, vp, vp, vp, sz, vp, vp]
         L.gw_executed_flops.argtypes = [P, ctypes.POINTER(ctypes.c_double)]
         L.gw_launch_count.argtypes = [P]
         L.gw_fp64_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
@@ -64,7 +66,7 @@ def lib():
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version",
-                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby"):
+                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -102,8 +104,10 @@ class GWProblem:
 
     V, T_wt, T_tw: CUDA complex128 tensors for the device calls, or CPU tensors for gw_sigma_iteration_host."""
 
-    def __init__(self, mesh, nao, naux, ntau, nw, beta, V, T_wt, T_tw, spin_deg=2, q_begin=0, q_end=None, symmetry=0):
+    def __init__(self, mesh, nao, naux, ntau, nw, beta, V, T_wt, T_tw, spin_deg=2, q_begin=0, q_end=None, symmetry=0, ns=1, v_layout=GW_V_FULL):
         self.symmetry = int(symmetry)      # 0 = literal Algorithm 1; GW_SYM_TR = time-reversal symmetric inputs (gw.h)
+        self.ns = 2 if int(ns) == 2 else 1  # spin channels: G, Sigma [ns][ntau][nk][nao][nao], gamma, K [ns][nk][nao][nao] when ns = 2
+        self.v_layout = int(v_layout)      # GW_V_FULL: V [nk][nk][naux][nao][nao]; GW_V_QSLAB: V [nq][nk][2][naux][nao][nao] (gw.h)
         self.mesh = tuple(int(m) for m in mesh)
         self.nk = self.mesh[0] * self.mesh[1] * self.mesh[2]
         self.nao, self.naux, self.ntau, self.nw = int(nao), int(naux), int(ntau), int(nw)
@@ -112,16 +116,26 @@ class GWProblem:
         self.q_end = self.nk if q_end is None else int(q_end)
         self.nq = self.q_end - self.q_begin
         self.V, self.T_wt, self.T_tw = V, T_wt, T_tw
-        for name, t, shape in (("V", V, (self.nk, self.nk, naux, nao, nao)), ("T_wt", T_wt, (nw, ntau)),
-                               ("T_tw", T_tw, (ntau, nw))):
+        vshape = (self.nk, self.nk, naux, nao, nao) if self.v_layout == GW_V_FULL else (self.nq, self.nk, 2, naux, nao, nao)
+        for name, t, shape in (("V", V, vshape), ("T_wt", T_wt, (nw, ntau)), ("T_tw", T_tw, (ntau, nw))):
             if t.dtype != torch.complex128 or not t.is_contiguous() or tuple(t.shape) != shape:
                 raise GWError(f"{name}: need contiguous complex128 of shape {shape}, got {tuple(t.shape)} {t.dtype}")
         self.c = _CProblem(self.mesh[0], self.mesh[1], self.mesh[2], self.nao, self.naux, self.ntau, self.nw,
                            self.spin_deg, self.q_begin, self.q_end, self.beta,
-                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr(), None, 0, self.symmetry, 0)
+                           V.data_ptr(), T_wt.data_ptr(), T_tw.data_ptr(), None, 0, self.symmetry, self.ns, self.v_layout, 0)
         self.work = None
         if V.is_cuda:
             self.set_work(torch.empty(int(lib().gw_workspace_bytes(ctypes.byref(self.c))), dtype=torch.uint8, device=V.device))
+
+    def gshape(self):
+        """shape of G and Sigma"""
+        base = (self.ntau, self.nk, self.nao, self.nao)
+        return (2,) + base if self.ns == 2 else base
+
+    def kshape(self):
+        """shape of gamma and K"""
+        base = (self.nk, self.nao, self.nao)
+        return (2,) + base if self.ns == 2 else base
 
     def set_work(self, work):
         """Attach the device workspace (uint8 CUDA tensor of at least gw_workspace_bytes bytes)."""
@@ -134,8 +148,10 @@ class GWProblem:
         return self.V.is_cuda
 
     def shard(self, q_begin, q_end):
+        if self.v_layout != GW_V_FULL:
+            raise GWError("shard(): a q-slab problem is already a shard")
         return GWProblem(self.mesh, self.nao, self.naux, self.ntau, self.nw, self.beta, self.V, self.T_wt, self.T_tw,
-                         self.spin_deg, q_begin, q_end, self.symmetry)
+                         self.spin_deg, q_begin, q_end, self.symmetry, self.ns)
 
     def ref(self):
         return ctypes.byref(self.c)
@@ -147,7 +163,7 @@ def gw_workspace_bytes(prob):
 
 def gw_polarization(prob, G, P0t=None, stream=None):
     """Stage 1, Eq. 28b.  G [ntau][nk][nao][nao] -> P0t [ntau][nq][naux][naux]."""
-    g = _dev(G, (prob.ntau, prob.nk, prob.nao, prob.nao), "G")
+    g = _dev(G, prob.gshape(), "G")
     if P0t is None:
         P0t = torch.empty((prob.ntau, prob.nq, prob.naux, prob.naux), dtype=torch.complex128, device=G.device)
     _check(lib().gw_polarization(prob.ref(), g, _dev(P0t, (prob.ntau, prob.nq, prob.naux, prob.naux), "P0t"),
@@ -203,7 +219,7 @@ def gw_transform(T, X, Y=None, stream=None):
 
 def gw_selfenergy(prob, G, Wt, Sigma=None, stream=None):
     """Stage 3, Eq. 31."""
-    gshape = (prob.ntau, prob.nk, prob.nao, prob.nao)
+    gshape = prob.gshape()
     if Sigma is None:
         Sigma = torch.empty(gshape, dtype=torch.complex128, device=G.device)
     _check(lib().gw_selfenergy(prob.ref(), _dev(G, gshape, "G"),
@@ -214,7 +230,7 @@ def gw_selfenergy(prob, G, Wt, Sigma=None, stream=None):
 
 def gw_exchange(prob, gamma, K=None, stream=None):
     """Stage 4, Eq. 22."""
-    shape = (prob.nk, prob.nao, prob.nao)
+    shape = prob.kshape()
     if K is None:
         K = torch.empty(shape, dtype=torch.complex128, device=gamma.device)
     _check(lib().gw_exchange(prob.ref(), _dev(gamma, shape, "gamma"), _dev(K, shape, "K"), _stream(stream)), "gw_exchange")
@@ -241,9 +257,9 @@ def gw_sigma_iteration_host(prob, G, gamma, Sigma=None, K=None, want_P0t=False, 
     pin = G.is_pinned()
     mk = lambda shape: torch.empty(shape, dtype=torch.complex128, pin_memory=pin)
     if Sigma is None:
-        Sigma = mk((prob.ntau, prob.nk, prob.nao, prob.nao))
+        Sigma = mk(prob.gshape())
     if K is None:
-        K = mk((prob.nk, prob.nao, prob.nao))
+        K = mk(prob.kshape())
     pshape = (prob.ntau, prob.nq, prob.naux, prob.naux)
     P0t = mk(pshape) if want_P0t else None
     Wt = mk(pshape) if want_Wt else None
@@ -252,6 +268,27 @@ def gw_sigma_iteration_host(prob, G, gamma, Sigma=None, K=None, want_P0t=False, 
     _check(lib().gw_sigma_iteration_host(prob.ref(), vp(G), vp(gamma), vp(Sigma), vp(K), vp(P0t), vp(Wt),
                                          ctypes.cast(ms, ctypes.c_void_p), _stream(stream)), "gw_sigma_iteration_host")
     return {"Sigma": Sigma, "K": K, "P0t": P0t, "Wt": Wt, "stage_ms": list(ms)}
+
+
+def gw_sigma_iteration_stream(prob, G, gamma, v_budget_bytes, Sigma=None, K=None, stream=None):
+    """Out-of-core V (gw.h): the whole iteration with V in HOST memory (GW_V_FULL layout, pinned recommended), streamed through two
+    device q-slab buffers of at most v_budget_bytes together.  Returns dict(Sigma, K, stats)."""
+    if prob.on_device or prob.v_layout != GW_V_FULL:
+        raise GWError("gw_sigma_iteration_stream needs a GWProblem built from CPU tensors in the full V layout")
+    for name, t, shape in (("G", G, prob.gshape()), ("gamma", gamma, prob.kshape())):
+        if t.is_cuda or t.dtype != torch.complex128 or not t.is_contiguous() or tuple(t.shape) != shape:
+            raise GWError(f"{name}: need a contiguous CPU complex128 tensor of shape {shape}")
+    pin = G.is_pinned()
+    mk = lambda shape: torch.empty(shape, dtype=torch.complex128, pin_memory=pin)
+    if Sigma is None:
+        Sigma = mk(prob.gshape())
+    if K is None:
+        K = mk(prob.kshape())
+    st = (ctypes.c_float * 4)()
+    vp = lambda t: ctypes.c_void_p(t.data_ptr())
+    _check(lib().gw_sigma_iteration_stream(prob.ref(), vp(G), vp(gamma), vp(Sigma), vp(K), ctypes.c_size_t(int(v_budget_bytes)),
+                                           ctypes.cast(st, ctypes.c_void_p), _stream(stream)), "gw_sigma_iteration_stream")
+    return {"Sigma": Sigma, "K": K, "stats": {"ms": st[0], "h2d_gb": st[1], "slabs": int(st[2]), "q_per_slab": int(st[3])}}
 
 
 def gw_executed_flops(prob):
@@ -292,11 +329,11 @@ def _f64(t, name):
 
 
 def gw_hartree(prob, gamma, J=None, stream=None):
-    """Eq. 20: J[k] from gamma[k'] and the diagonal blocks V[k][k]."""
+    """Eq. 20: J[k] (spin independent) from gamma[k'] (summed over the spin channels) and the diagonal blocks V[k][k]."""
     shape = (prob.nk, prob.nao, prob.nao)
     if J is None:
         J = torch.empty(shape, dtype=torch.complex128, device=gamma.device)
-    _check(lib().gw_hartree(prob.ref(), _dev(gamma, shape, "gamma"), _dev(J, shape, "J"), _stream(stream)), "gw_hartree")
+    _check(lib().gw_hartree(prob.ref(), _dev(gamma, prob.kshape(), "gamma"), _dev(J, shape, "J"), _stream(stream)), "gw_hartree")
     return J
 
 

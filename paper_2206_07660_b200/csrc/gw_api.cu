@@ -26,7 +26,7 @@ static int check_problem(const gw_problem *p, bool need_T) {
   if (!p) return GW_EINVAL;
   if (p->nk1 <= 0 || p->nk2 <= 0 || p->nk3 <= 0 || p->nao <= 0 || p->naux <= 0 || p->ntau <= 0 || p->nw <= 0) return GW_EINVAL;
   if (p->spin_deg != 1 && p->spin_deg != 2) return GW_EINVAL;
-  if ((p->symmetry & ~GW_SYM_TR) || p->reserved) return GW_EINVAL;
+  if ((p->symmetry & ~GW_SYM_TR) || p->reserved || p->ns < 0 || p->ns > 2 || (p->v_layout != GW_V_FULL && p->v_layout != GW_V_QSLAB)) return GW_EINVAL;
   const int64_t nk = (int64_t)p->nk1 * p->nk2 * p->nk3;
   if (nk > (1 << 20)) return GW_EINVAL;
   if (p->q_begin < 0 || p->q_end > nk || p->q_begin >= p->q_end) return GW_EINVAL;
@@ -114,7 +114,7 @@ extern "C" int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, co
   cudaStream_t st = (cudaStream_t)stream;
   GwDims d = gw_dims(p);
   const size_t n2 = (size_t)d.nao * d.nao, a2 = (size_t)d.naux * d.naux;
-  const size_t bV = (size_t)d.nk * d.nk * d.naux * n2 * 16, bG = (size_t)d.ntau * d.nk * n2 * 16, bg = (size_t)d.nk * n2 * 16;
+  const size_t bV = gw_vblocks(d) * d.naux * n2 * 16, bG = (size_t)d.ns * d.ntau * d.nk * n2 * 16, bg = (size_t)d.ns * d.nk * n2 * 16;
   const size_t bP = (size_t)d.ntau * d.nq * a2 * 16, bT = (size_t)d.nw * d.ntau * 16;
   c128 *dV = 0, *dG = 0, *dg = 0, *dP = 0, *dS = 0, *dK = 0, *dTwt = 0, *dTtw = 0; void *dW = 0; int32_t *dinfo = 0;
   cudaEvent_t ev[7]; for (int i = 0; i < 7; i++) ev[i] = 0;
@@ -159,6 +159,86 @@ done:
   return rc;
 }
 
+
+// Out-of-core V: q-slabs of V are gathered from host memory into two device buffers on a copy stream while the previous slab
+// computes; Sigma and K continue their q sums across slabs (GW_ACC_CONTINUE / GW_ACC_PARTIAL), so the result is the resident one.
+extern "C" int gw_sigma_iteration_stream(const gw_problem *p, const gw_c128 *G, const gw_c128 *gamma, gw_c128 *Sigma, gw_c128 *K,
+                                         size_t v_budget_bytes, float *stats, void *stream) {
+  int rc = check_problem(p, true); if (rc) return rc;
+  if (!G || !gamma || !Sigma || !K || p->v_layout != GW_V_FULL) return GW_EINVAL;
+  if ((rc = check_arch())) return rc;
+  cudaStream_t st = (cudaStream_t)stream, cs = 0;
+  const GwDims d = gw_dims(p);
+  const size_t n2 = (size_t)d.nao * d.nao, a2 = (size_t)d.naux * d.naux;
+  const size_t blk = (size_t)d.naux * n2 * 16, perq = 2 * (size_t)d.nk * blk;          // one V block; the 2 nk blocks of one q
+  int nqs = (int)((v_budget_bytes / 2) / perq);
+  if (nqs < 1) return GW_ENOMEM;
+  if (nqs > d.nq) nqs = d.nq;
+  const int nslab = (d.nq + nqs - 1) / nqs;
+  const size_t bG = (size_t)d.ns * d.ntau * d.nk * n2 * 16, bg = (size_t)d.ns * d.nk * n2 * 16;
+  const size_t bP = (size_t)d.ntau * nqs * a2 * 16, bT = (size_t)d.nw * d.ntau * 16;
+  c128 *dV[2] = {0, 0}, *dG = 0, *dg = 0, *dP = 0, *dS = 0, *dK = 0, *dTwt = 0, *dTtw = 0; void *dW = 0; int32_t *dinfo = 0, *hinfo = 0;
+  cudaEvent_t ready[2] = {0, 0}, freed[2] = {0, 0}, e0 = 0, e1 = 0;
+  gw_problem sp = *p;
+  size_t wb = 0; double copied = 0.0; float ms = 0.f;
+  const char *hV = (const char *)p->V;
+  hinfo = (int32_t *)malloc(sizeof(int32_t) * 2 * nslab);
+  if (!hinfo) return GW_ENOMEM;
+  CU(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; i++) { CU(cudaEventCreateWithFlags(&ready[i], cudaEventDisableTiming)); CU(cudaEventCreateWithFlags(&freed[i], cudaEventDisableTiming)); }
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  for (int i = 0; i < 2; i++) CU(cudaMalloc(&dV[i], (size_t)nqs * perq));
+  CU(cudaMalloc(&dG, bG)); CU(cudaMalloc(&dg, bg)); CU(cudaMalloc(&dP, bP)); CU(cudaMalloc(&dS, bG)); CU(cudaMalloc(&dK, bg));
+  CU(cudaMalloc(&dTwt, bT)); CU(cudaMalloc(&dTtw, bT)); CU(cudaMalloc(&dinfo, 8 * (size_t)nslab));
+  sp.T_wt = (const gw_c128 *)dTwt; sp.T_tw = (const gw_c128 *)dTtw; sp.v_layout = GW_V_QSLAB; sp.V = (const gw_c128 *)dV[0];
+  sp.q_begin = p->q_begin; sp.q_end = p->q_begin + nqs;
+  wb = gw_workspace_bytes(&sp);
+  if (!wb) { rc = GW_ESHAPE; goto done; }
+  CU(cudaMalloc(&dW, wb));
+  sp.work = dW; sp.work_bytes = wb;
+  CU(cudaEventRecord(e0, st));
+  CU(cudaMemcpyAsync(dG, G, bG, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dg, gamma, bg, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dTwt, p->T_wt, bT, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(dTtw, p->T_tw, bT, cudaMemcpyHostToDevice, st));
+  for (int s = 0; s < nslab; s++) {
+    const int b = s & 1, q0 = p->q_begin + s * nqs, q1 = (q0 + nqs < p->q_end) ? q0 + nqs : p->q_end;
+    // gather the slab: slot (ql, k, 0) = V[k][k+q], slot (ql, k, 1) = V[k+q][k]; the buffer was last read by slab s-2
+    if (s >= 2) CU(cudaStreamWaitEvent(cs, freed[b], 0));
+    for (int q = q0; q < q1; q++)
+      for (int k = 0; k < d.nk; k++) {
+        const int kq = gw_kadd(d, k, q);
+        char *dst = (char *)dV[b] + (((size_t)(q - q0) * d.nk + k) * 2) * blk;
+        CU(cudaMemcpyAsync(dst, hV + ((size_t)k * d.nk + kq) * blk, blk, cudaMemcpyHostToDevice, cs));
+        CU(cudaMemcpyAsync(dst + blk, hV + ((size_t)kq * d.nk + k) * blk, blk, cudaMemcpyHostToDevice, cs));
+        copied += 2.0 * (double)blk;
+      }
+    CU(cudaEventRecord(ready[b], cs));
+    CU(cudaStreamWaitEvent(st, ready[b], 0));
+    sp.V = (const gw_c128 *)dV[b]; sp.q_begin = q0; sp.q_end = q1;
+    const int acc = (s > 0 ? GW_ACC_CONTINUE : 0) | (s < nslab - 1 ? GW_ACC_PARTIAL : 0);
+    if ((rc = gw_polarization(&sp, (gw_c128 *)dG, (gw_c128 *)dP, st))) goto done;
+    if ((rc = gw_screened_interaction(&sp, (gw_c128 *)dP, (gw_c128 *)dP, dinfo + 2 * s, st))) goto done;
+    if ((rc = gw_launch_stage3(&sp, dG, dP, dS, st, acc))) goto done;
+    if ((rc = gw_launch_stage4(&sp, dg, dK, st, acc))) goto done;
+    CU(cudaEventRecord(freed[b], st));
+  }
+  CU(cudaMemcpyAsync(Sigma, dS, bG, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(K, dK, bg, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(hinfo, dinfo, 8 * (size_t)nslab, cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(e1, st));
+  CU(cudaStreamSynchronize(st));
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  for (int s = 0; s < 2 * nslab; s++) if (hinfo[s] != -1) rc = GW_ENOTPD;
+  if (stats) { stats[0] = ms; stats[1] = (float)(copied * 1e-9); stats[2] = (float)nslab; stats[3] = (float)nqs; }
+done:
+  if (cs) { cudaStreamSynchronize(cs); cudaStreamDestroy(cs); }
+  cudaFree(dV[0]); cudaFree(dV[1]); cudaFree(dG); cudaFree(dg); cudaFree(dP); cudaFree(dS); cudaFree(dK); cudaFree(dTwt); cudaFree(dTtw); cudaFree(dW); cudaFree(dinfo);
+  for (int i = 0; i < 2; i++) { if (ready[i]) cudaEventDestroy(ready[i]); if (freed[i]) cudaEventDestroy(freed[i]); }
+  if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1);
+  free(hinfo);
+  return rc;
+}
 
 // ---- loop closure (gw_loop.cu) ----
 extern "C" int gw_hartree(const gw_problem *p, const gw_c128 *gamma, gw_c128 *J, void *stream) {

@@ -19,6 +19,8 @@ struct GwDims {
   int s;            // spin_deg
   int q0, nq;       // q shard
   int sym;          // gw_problem.symmetry
+  int ns;           // spin channels (1 or 2)
+  int vq;           // 1: p->V is a q-slab (GW_V_QSLAB), 0: the full tensor
 };
 
 static inline GwDims gw_dims(const gw_problem *p) {
@@ -26,6 +28,7 @@ static inline GwDims gw_dims(const gw_problem *p) {
   d.nk1 = p->nk1; d.nk2 = p->nk2; d.nk3 = p->nk3; d.nk = p->nk1 * p->nk2 * p->nk3;
   d.nao = p->nao; d.naux = p->naux; d.ntau = p->ntau; d.nw = p->nw; d.s = p->spin_deg;
   d.q0 = p->q_begin; d.nq = p->q_end - p->q_begin; d.sym = p->symmetry;
+  d.ns = p->ns == 2 ? 2 : 1; d.vq = p->v_layout == GW_V_QSLAB ? 1 : 0;
   return d;
 }
 
@@ -41,6 +44,17 @@ __host__ __device__ __forceinline__ int gw_kcombine(const GwDims &d, int k, int 
 }
 __host__ __device__ __forceinline__ int gw_kadd(const GwDims &d, int k, int q) { return gw_kcombine(d, k, q, +1); }
 __host__ __device__ __forceinline__ int gw_ksub(const GwDims &d, int k, int q) { return gw_kcombine(d, k, q, -1); }
+
+// V block index (in blocks of naux*nao² elements) for the shard-local q index ql, with kq = k + q:
+//   gw_vfwd = V[k][k+q],  gw_vbwd = V[k+q][k]   (gw.h "V layouts").  Stages 3/4 use them with k := k-q, kq := k.
+__host__ __device__ __forceinline__ size_t gw_vfwd(const GwDims &d, int ql, int k, int kq) {
+  return d.vq ? ((size_t)ql * d.nk + k) * 2 : (size_t)k * d.nk + kq;
+}
+__host__ __device__ __forceinline__ size_t gw_vbwd(const GwDims &d, int ql, int k, int kq) {
+  return d.vq ? ((size_t)ql * d.nk + k) * 2 + 1 : (size_t)kq * d.nk + k;
+}
+// number of V blocks behind p->V
+__host__ __device__ __forceinline__ size_t gw_vblocks(const GwDims &d) { return d.vq ? (size_t)d.nq * d.nk * 2 : (size_t)d.nk * d.nk; }
 
 __device__ __forceinline__ c128 cmul(c128 a, c128 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ void cfma(c128 &acc, c128 a, c128 b) {
@@ -76,8 +90,12 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t st);
 int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *info, double *phi, cudaStream_t st);
 int gw_launch_transform(int n_out, int n_in, const c128 *T, const c128 *X, c128 *Y, size_t len, cudaStream_t st);
-int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st);
-int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st);
+// acc_mode (stages 3 and 4; used by the out-of-core driver to continue the q sum across V slabs in the resident order):
+//   GW_ACC_CONTINUE : the accumulators start from the UNSCALED partial sums found in the output array
+//   GW_ACC_PARTIAL  : the output array receives UNSCALED partial sums (no -(1/N_k), no symmetry mirror copies)
+enum { GW_ACC_CONTINUE = 1, GW_ACC_PARTIAL = 2 };
+int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st, int acc_mode = 0);
+int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st, int acc_mode = 0);
 int gw_launch_hartree(const gw_problem *p, const c128 *gamma, c128 *J, cudaStream_t st);
 int gw_launch_dyson_update(int nk, int nao, int nwf, const double *omega, double mu, const c128 *S, const c128 *F, const c128 *Sigma_w, c128 *G_w,
                            int32_t *info, cudaStream_t st);

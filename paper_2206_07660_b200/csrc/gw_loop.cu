@@ -24,25 +24,26 @@ __device__ __forceinline__ c128 block_sum(c128 v, c128 *red) {
 }
 
 // ---- Hartree, Eq. 20:  rho[Q] = Σ_k' Σ_ab γ[k'][a][b] V[k'][k'][Q][b][a];   J[k][i][j] = (s/N_k) Σ_Q V[k][k][Q][i][j] rho[Q]
-__global__ void __launch_bounds__(NT) hartree_rho_kernel(const GwDims d, const c128 *__restrict__ V, const c128 *__restrict__ gamma, c128 *__restrict__ rho) {
+__global__ void __launch_bounds__(NT) hartree_rho_kernel(const GwDims d, int ql0, const c128 *__restrict__ V, const c128 *__restrict__ gamma, c128 *__restrict__ rho) {
   __shared__ c128 red[NT];
   const int Q = blockIdx.x, nao = d.nao, n2 = nao * nao;
   c128 acc = make_double2(0.0, 0.0);
-  for (int kp = 0; kp < d.nk; kp++) {
-    const c128 *Vq = V + (((size_t)kp * d.nk + kp) * d.naux + Q) * n2, *g = gamma + (size_t)kp * n2;
-    for (int e = threadIdx.x; e < n2; e += NT) {
-      const int b = e / nao, a = e - b * nao;
-      cfma(acc, g[a * nao + b], Vq[e]);
+  for (int sg = 0; sg < d.ns; sg++)                        // Σ_sigma1 of Eq. 20
+    for (int kp = 0; kp < d.nk; kp++) {
+      const c128 *Vq = V + (gw_vfwd(d, ql0, kp, kp) * d.naux + Q) * n2, *g = gamma + ((size_t)sg * d.nk + kp) * n2;
+      for (int e = threadIdx.x; e < n2; e += NT) {
+        const int b = e / nao, a = e - b * nao;
+        cfma(acc, g[a * nao + b], Vq[e]);
+      }
     }
-  }
   const c128 tot = block_sum(acc, red);
   if (threadIdx.x == 0) rho[Q] = tot;
 }
 
-__global__ void __launch_bounds__(NT) hartree_j_kernel(const GwDims d, const c128 *__restrict__ V, const c128 *__restrict__ rho, c128 *__restrict__ J) {
+__global__ void __launch_bounds__(NT) hartree_j_kernel(const GwDims d, int ql0, const c128 *__restrict__ V, const c128 *__restrict__ rho, c128 *__restrict__ J) {
   const int k = blockIdx.y, n2 = d.nao * d.nao, e = blockIdx.x * NT + threadIdx.x;
   if (e >= n2) return;
-  const c128 *Vk = V + ((size_t)k * d.nk + k) * d.naux * n2 + e;
+  const c128 *Vk = V + gw_vfwd(d, ql0, k, k) * d.naux * n2 + e;
   c128 acc = make_double2(0.0, 0.0);
   for (int Q = 0; Q < d.naux; Q++) cfma(acc, Vk[(size_t)Q * n2], rho[Q]);
   const double pref = (double)d.s / (double)d.nk;
@@ -165,9 +166,12 @@ int gw_launch_hartree(const gw_problem *p, const c128 *gamma, c128 *J, cudaStrea
   const GwDims d = gw_dims(p);
   if (!p->work || p->work_bytes < 256 + (size_t)d.naux * sizeof(c128) || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   c128 *rho = (c128 *)((char *)p->work + 256);
-  lp::hartree_rho_kernel<<<d.naux, lp::NT, 0, st>>>(d, (const c128 *)p->V, gamma, rho);
+  // the diagonal blocks V[k][k] = V[k][k+0]: in the q-slab layout they are slot (0 - q_begin, k, 0), present iff the shard holds q = 0
+  if (d.vq && !(d.q0 <= 0 && 0 < d.q0 + d.nq)) return GW_EINVAL;
+  const int ql0 = -d.q0;
+  lp::hartree_rho_kernel<<<d.naux, lp::NT, 0, st>>>(d, ql0, (const c128 *)p->V, gamma, rho);
   const int n2 = d.nao * d.nao;
-  lp::hartree_j_kernel<<<dim3((n2 + lp::NT - 1) / lp::NT, d.nk), lp::NT, 0, st>>>(d, (const c128 *)p->V, rho, J);
+  lp::hartree_j_kernel<<<dim3((n2 + lp::NT - 1) / lp::NT, d.nk), lp::NT, 0, st>>>(d, ql0, (const c128 *)p->V, rho, J);
   return (int)cudaGetLastError();
 }
 

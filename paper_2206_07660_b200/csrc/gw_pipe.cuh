@@ -239,6 +239,24 @@ __device__ __forceinline__ void final_store(c128 *out, const double (&sgr)[NCT][
   }
 }
 
+// load the warp-owned tiles of an nao x nao array into the accumulators (the inverse of final_store with pref = 1)
+template <int NCT>
+__device__ __forceinline__ void final_load(const c128 *in, double (&sgr)[NCT][2], double (&sgi)[NCT][2], int nao, int ndt) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+#pragma unroll
+  for (int ti = 0; ti < NCT; ti++) {
+    const int tile = w + 8 * ti;
+    if (tile < ndt * ndt) {
+      const int mi = tile / ndt, nj = tile - mi * ndt;
+      const int i = 8 * mi + g, j = 8 * nj + 2 * c;
+      if (i < nao) {
+        if (j < nao) { sgr[ti][0] = in[i * nao + j].x; sgi[ti][0] = in[i * nao + j].y; }
+        if (j + 1 < nao) { sgr[ti][1] = in[i * nao + j + 1].x; sgi[ti][1] = in[i * nao + j + 1].y; }
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // Warp-specialised pipeline: one producer warp fills a ring of stage buffers with cp.async (completion tracked by an
 // mbarrier per stage), NCONS consumer warps wait on "full", compute on FP64 tensor cores, and release "empty".

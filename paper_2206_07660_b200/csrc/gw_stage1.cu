@@ -164,6 +164,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
   c128 *slab0 = P.scratch + (size_t)cid * 2 * P.slab_units;
   const size_t vb = (size_t)naux * n2;
   const int nmain = (n2 + KC - 1) / KC;
+  const int nkk = d.nk * d.ns;                            // k loop of Eq. 28b with the spin sum inside
   const int rows_cta = TM / cs;                           // panel rows transformed by this CTA's pass warps
   const int r0 = (int)rank * rows_cta;
 
@@ -197,9 +198,10 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
         for (int item = cid; item < P.nitems; item += ncl) {
           const Item it = decode_item(P, item);
           const int q = d.q0 + it.ql;
-          for (int k = 0; k < d.nk; k++, kit++) {
+          for (int kk = 0; kk < nkk; kk++, kit++) {
+            const int k = d.ns == 2 ? kk >> 1 : kk;                    // spin channel innermost: the V blocks of (k, q) serve both
             const int kq = gw_kadd(d, k, q);
-            const int yB = (kq * d.nk + k) * naux + 8 * (it.cbase + (int)rank * P.ntc);   // row of V viewed as [nk*nk*naux][nao²]
+            const int yB = (int)gw_vbwd(d, it.ql, k, kq) * naux + 8 * (it.cbase + (int)rank * P.ntc);   // row of V viewed as [blocks*naux][nao²]
             const int yA = (cid * 2 + (int)(kit & 1u)) * TM;           // row of the slab area viewed as [2*nclusters*TM][nao²]
             if (cs > 1) gwp::mbar_wait_cluster(zready + (kit & 1u), (kit >> 1) & 1u);
             else gwp::mbar_wait(zready + (kit & 1u), (kit >> 1) & 1u);
@@ -223,11 +225,13 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
         const Item it = decode_item(P, item);
         const int q = d.q0 + it.ql;
         const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
-        for (int k = 0; k < d.nk; k++, kit++) {
+        for (int kk = 0; kk < nkk; kk++, kit++) {
+          const int k = d.ns == 2 ? kk >> 1 : kk, sg = d.ns == 2 ? kk & 1 : 0;
           const int kq = gw_kadd(d, k, q);
-          const c128 *Vt = P.V + ((size_t)k * d.nk + kq) * vb + (size_t)(it.Q0 + r0) * n2;
+          const c128 *Vt = P.V + gw_vfwd(d, it.ql, k, kq) * vb + (size_t)(it.Q0 + r0) * n2;
           const c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
-          const c128 *Gt = P.G + ((size_t)it.t * d.nk + kq) * n2, *Gm = P.G + ((size_t)(d.ntau - 1 - it.t) * d.nk + k) * n2;
+          const c128 *Gs = P.G + (size_t)sg * d.ntau * d.nk * n2;      // this spin channel's G[t][k]
+          const c128 *Gt = Gs + ((size_t)it.t * d.nk + kq) * n2, *Gm = Gs + ((size_t)(d.ntau - 1 - it.t) * d.nk + k) * n2;
           // pass 1 (its G buffer was last read two phases ago; a time-shared buffer must wait for the previous phase)
           if (P.ng == 2) issue_matrix<true>(sG0, Gt, nao, ldp, P.fd_nao);
           if (ph > 0) gwp::mbar_wait(bar_phase, (ph - 1) & 1u);
@@ -264,7 +268,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
     for (int item = cid; item < P.nitems; item += ncl) {
       const Item it = decode_item(P, item);
       const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
-      for (int k = 0; k < d.nk; k++, kit++) {
+      for (int kk = 0; kk < nkk; kk++, kit++) {
         c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
         // this slab was read by the main GEMM of iteration kit-2
         if (kit >= 2) {
@@ -335,7 +339,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
 #pragma unroll
           for (int j = 0; j < NJ; j++) acc[x][i][j][0] = acc[x][i][j][1] = 0.0;
 
-      for (int k = 0; k < d.nk; k++, kit++) {
+      for (int kk = 0; kk < nkk; kk++, kit++) {
         for (int j = 0; j < nmain; j++) {
           const int s = rm.wait();
           if (active) {
@@ -501,7 +505,7 @@ double gw_stage1_flops(const gw_problem *p) {
     const double mainv = mtiles * nt_eff * (s1::KC / 4) * nmain * (pl.s3m ? 1536.0 : 2048.0);
     tiles += pass + mainv;
   }
-  return tiles * (double)d.nk * pl.nteff * pl.nqeff;
+  return tiles * (double)d.nk * d.ns * pl.nteff * pl.nqeff;
 }
 
 template <int KSP_MAX, bool S3M>
@@ -510,7 +514,7 @@ static int launch_p0(const s1::Plan &pl, const s1::Params &P, cudaStream_t st) {
   if (e != cudaSuccess) return (int)e;
   const int n2 = P.d.nao * P.d.nao;
   CUtensorMap tmV, tmZ;
-  int rc = gwp::make_tensor_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, n2, 8 * pl.ntc);
+  int rc = gwp::make_tensor_map(&tmV, P.V, gw_vblocks(P.d) * P.d.naux, n2, 8 * pl.ntc);
   if (rc) return rc;
   rc = gwp::make_tensor_map(&tmZ, P.scratch, (size_t)gwp::gw_num_sms() * 2 * s1::TM, n2, s1::TM);
   if (rc) return rc;

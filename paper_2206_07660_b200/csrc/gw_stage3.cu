@@ -42,6 +42,7 @@ struct Params {
   int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
   short kirr[128];        // the evaluated k points when nkeff < nk
   __device__ __forceinline__ int kof(int i) const { return nkeff < d.nk ? (int)kirr[i] : i; }
+  int acc_mode;           // GW_ACC_CONTINUE / GW_ACC_PARTIAL (gw_common.cuh)
   FastDiv fd_nao;
 };
 
@@ -106,13 +107,13 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P, const
     asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;\n" : "=l"(polA));
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(polB));
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      const int t = item % d.ntau, k = P.kof(item / d.ntau);
+      const int t = item % d.ntau, ik = item / d.ntau, k = P.kof(ik % P.nkeff), sg = ik / P.nkeff;
+      const c128 *Gs = P.G + (size_t)sg * d.ntau * d.nk * n2;     // spin channel sg
       for (int ql = 0; ql < d.nq; ql++) {
         const int q = d.q0 + ql, kp = gw_ksub(d, k, q);
-        const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
-        const c128 *V2 = P.V + ((size_t)kp * d.nk + k) * vb;     // V[k-q][k][Q'][b][j]
-        const int yV = (kp * d.nk + k) * naux, yW = (t * d.nq + ql) * naux;   // first rows of V[k-q][k] and Wt[t][q] in the TMA views
-        gwp::ws_issue_matrix<false>(sG, P.G + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
+        const c128 *V1 = P.V + gw_vbwd(d, ql, kp, k) * vb;        // V[k][k-q][Q][i][a]
+        const int yV = (int)gw_vfwd(d, ql, kp, k) * naux, yW = (t * d.nq + ql) * naux;   // first rows of V[k-q][k] and Wt[t][q] in the TMA views
+        gwp::ws_issue_matrix<false>(sG, Gs + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
         gwp::cp_async_arrive_noinc(bar_g);
         for (int qt = 0; qt < P.nqt; qt++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0);
@@ -161,10 +162,12 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P, const
     const int g = lane >> 2, c = lane & 3;
     const int rho = (g >> 1) + 4 * (g & 1);            // fragment row / column of this lane group in the TMA-swizzled main jobs
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      const int t = item % d.ntau, k = P.kof(item / d.ntau);
+      const int t = item % d.ntau, ik = item / d.ntau, k = P.kof(ik % P.nkeff), sg = ik / P.nkeff;
+      c128 *Sout = P.Sigma + (((size_t)sg * d.ntau + t) * d.nk + k) * n2;
       double sgr[NCT][2], sgi[NCT][2];
 #pragma unroll
       for (int i = 0; i < NCT; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+      if (P.acc_mode & GW_ACC_CONTINUE) gwp::final_load<NCT>(Sout, sgr, sgi, nao, ndt);
       for (int ql = 0; ql < d.nq; ql++) {
         gwp::mbar_wait(bar_g, gpar); gpar ^= 1u;
         for (int qt = 0; qt < P.nqt; qt++) {
@@ -256,10 +259,11 @@ __global__ void __launch_bounds__(NTHR_WS, 1) sigma_kernel(const Params P, const
           }
         }
       }
-      gwp::final_store<NCT>(P.Sigma + ((size_t)t * d.nk + k) * n2, sgr, sgi, -1.0 / (double)d.nk, nao, ndt);
-      if (P.nkeff < d.nk) {                                   // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
+      const bool partial = (P.acc_mode & GW_ACC_PARTIAL) != 0;
+      gwp::final_store<NCT>(Sout, sgr, sgi, partial ? 1.0 : -1.0 / (double)d.nk, nao, ndt);
+      if (P.nkeff < d.nk && !partial) {                       // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
         const int kn = gw_ksub(d, 0, k);
-        if (kn != k) gwp::final_store<NCT>(P.Sigma + ((size_t)t * d.nk + kn) * n2, sgr, sgi, -1.0 / (double)d.nk, nao, ndt, true);
+        if (kn != k) gwp::final_store<NCT>(P.Sigma + (((size_t)sg * d.ntau + t) * d.nk + kn) * n2, sgr, sgi, -1.0 / (double)d.nk, nao, ndt, true);
       }
     }
   }
@@ -289,7 +293,7 @@ static Plan make_plan(const gw_problem *p) {
   pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
   pl.ldb = pl.cht * 8 + 2;
   pl.nqt = (d.naux + TM - 1) / TM;
-  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
+  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp) * d.ns; }
   const int s_pass = PASS_ROWS * pl.ldp, s_main = TM * KC + 64 * pl.cht;   // main: A 32 rows x 128 B + one 1 KB box per n-tile
   // the ring starts 1024-byte aligned and every stage is a multiple of 1024 bytes (TMA destinations, 128-byte swizzle)
   const size_t fixed = ((size_t)naop * pl.ldp * sizeof(c128) + 1023) / 1024 * 1024;
@@ -337,7 +341,7 @@ static double s3_generic_flops(const gw_problem *p) {
     tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.kspf * pl.kh;             // final
   }
   short tmp[128];
-  return tiles * (double)d.nq * fill_kirr(d, tmp) * d.ntau * 2048.0;
+  return tiles * (double)d.nq * fill_kirr(d, tmp) * d.ntau * d.ns * 2048.0;
 }
 
 template <int KSP_MAX, int NCT>
@@ -348,18 +352,19 @@ static int launch_sigma(const s3::Plan &pl, const s3::Params &P, cudaStream_t st
   CUtensorMap tmW, tmV;
   int rc = gwp::make_tensor_map(&tmW, P.Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, s3::TM);
   if (rc) return rc;
-  rc = gwp::make_tensor_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, s3::KC);
+  rc = gwp::make_tensor_map(&tmV, P.V, gw_vblocks(P.d) * P.d.naux, P.d.nao * P.d.nao, s3::KC);
   if (rc) return rc;
   s3::sigma_kernel<KSP_MAX, NCT><<<pl.grid, s3::NTHR_WS, pl.smem, st>>>(P, tmW, tmV);
   return (int)cudaGetLastError();
 }
 
 namespace s3 {
-static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
+static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st, int acc_mode) {
   Plan pl = make_plan(p);
   if (!pl.ok) return GW_ESHAPE;
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   s3::Params P;
+  P.acc_mode = acc_mode;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
   P.scratch = (c128 *)((char *)p->work + 256);
   P.nqt = pl.nqt; P.nitems = pl.nitems; P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.ldt = pl.ldt; P.kh = pl.kh; P.kspf = pl.kspf; P.ldpf = pl.ldpf; P.fd_kw = gwp::FastDiv((unsigned)(4 * pl.kspf));
@@ -429,6 +434,7 @@ struct Params {
   int nkeff;              // k points evaluated: nk, or the k <= -k half under GW_SYM_TR (Sigma[-k] = conj Sigma[k] is copied)
   short kirr[128];        // the evaluated k points when nkeff < nk
   __device__ __forceinline__ int kof(int i) const { return nkeff < d.nk ? (int)kirr[i] : i; }
+  int acc_mode;           // GW_ACC_CONTINUE / GW_ACC_PARTIAL (gw_common.cuh)
   FastDiv fd_nao;
 };
 
@@ -590,10 +596,10 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
         Ring rm; rm.full = full_m; rm.empty = empty_m; rm.nstage = P.nstage; rm.it = 0; rm.ph = 0;
         const uint64_t polA = gwp::policy_evict_normal(), polB = gwp::policy_evict_last();
         for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-          const int t = item % d.ntau, k = P.kof(item / d.ntau);
+          const int t = item % d.ntau, k = P.kof((item / d.ntau) % P.nkeff);
           for (int ql = 0; ql < d.nq; ql++) {
             const int kp = gw_ksub(d, k, d.q0 + ql);
-            const int yV = (kp * d.nk + k) * naux;                    // V[k-q][k] rows of V viewed as [nk*nk*naux][nao²]
+            const int yV = (int)gw_vfwd(d, ql, kp, k) * naux;         // V[k-q][k] rows of V viewed as [blocks*naux][nao²]
             const int yW = (t * d.nq + ql) * naux;                    // Wt[t][q] rows of Wt viewed as [ntau*nq*naux][naux]
             for (int qt = 0; qt < P.nqt; qt++) {
               for (int ch = 0; ch < P.nchunk; ch++) {
@@ -617,15 +623,16 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
       Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
       unsigned un = 0;
       for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-        const int t = item % d.ntau, k = P.kof(item / d.ntau);
+        const int t = item % d.ntau, ik = item / d.ntau, k = P.kof(ik % P.nkeff), sg = ik / P.nkeff;
+        const c128 *Gs = P.G + (size_t)sg * d.ntau * d.nk * n2;   // spin channel sg
         for (int ql = 0; ql < d.nq; ql++) {
           const int kp = gw_ksub(d, k, d.q0 + ql);
-          const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb;     // V[k][k-q][Q][i][a]
+          const c128 *V1 = P.V + gw_vbwd(d, ql, kp, k) * vb;      // V[k][k-q][Q][i][a]
           for (int qt = 0; qt < P.nqt; qt++, un++) {
             const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + AROWS - 1) / AROWS;
             const c128 *U = slabU + (size_t)(un & 1u) * P.slab_units;
             // sG is free: pass A of the previous unit completed before its final jobs were issued
-            if (qt == 0) issue_matrix(sG, P.G + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
+            if (qt == 0) issue_matrix(sG, Gs + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
             gwp::cp_async_arrive_noinc(bar_g);
             gwp::mbar_wait(uready + (un & 1u), (un >> 1) & 1u);
             for (int j = 0; j < npass; j++) {
@@ -656,10 +663,26 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
     Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
     unsigned un = 0;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
-      const int t = item % d.ntau, k = P.kof(item / d.ntau);
+      const int t = item % d.ntau, ik = item / d.ntau, k = P.kof(ik % P.nkeff), sg = ik / P.nkeff;
+      c128 *Sst = P.Sigma + ((size_t)sg * d.ntau + t) * d.nk * n2;       // Sigma[sg][t]
       double sgr[NTA][2], sgi[NTA][2];
 #pragma unroll
       for (int i = 0; i < NTA; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+      if (P.acc_mode & GW_ACC_CONTINUE) {                     // continue the q sum from the unscaled partial sums of the previous V slab
+        const c128 *in = Sst + (size_t)k * n2;
+#pragma unroll
+        for (int ti = 0; ti < NTA; ti++) {
+          const int tile = wa + NAUXW * ti;
+          if (tile < NDT * NDT) {
+            const int mi = tile / NDT, nj = tile - mi * NDT;
+            const int i = 8 * mi + g, j0 = 8 * nj + 2 * c;
+            if (i < nao) {
+              if (j0 < nao) { sgr[ti][0] = in[i * nao + j0].x; sgi[ti][0] = in[i * nao + j0].y; }
+              if (j0 + 1 < nao) { sgr[ti][1] = in[i * nao + j0 + 1].x; sgi[ti][1] = in[i * nao + j0 + 1].y; }
+            }
+          }
+        }
+      }
       for (int ql = 0; ql < d.nq; ql++) {
         for (int qt = 0; qt < P.nqt; qt++, un++) {
           const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + AROWS - 1) / AROWS;
@@ -682,11 +705,12 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
         }
       }
       // Sigma[t][k] = -(1/N_k) acc: this warp's tiles
-      const double pref = -1.0 / (double)d.nk;
+      const bool partial = (P.acc_mode & GW_ACC_PARTIAL) != 0;
+      const double pref = partial ? 1.0 : -1.0 / (double)d.nk;
       const int kn = gw_ksub(d, 0, k);
-      const int ncopy = (P.nkeff < d.nk && kn != k) ? 2 : 1;  // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
+      const int ncopy = (P.nkeff < d.nk && kn != k && !partial) ? 2 : 1;  // GW_SYM_TR: Sigma[t][-k] = conj(Sigma[t][k])
       for (int cp = 0; cp < ncopy; cp++) {
-        c128 *out = P.Sigma + ((size_t)t * d.nk + (cp ? kn : k)) * n2;
+        c128 *out = Sst + (size_t)(cp ? kn : k) * n2;
         const double prefi = cp ? -pref : pref;
 #pragma unroll
         for (int ti = 0; ti < NTA; ti++) {
@@ -802,7 +826,7 @@ static Plan make_plan(const gw_problem *p) {
   pl.nchunk = (pl.nnt + 4 * NJ - 1) / (4 * NJ);
   pl.cht = (pl.nnt + pl.nchunk - 1) / pl.nchunk;
   pl.nqt = (d.naux + TM - 1) / TM;
-  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp); }
+  { short tmp[128]; pl.nitems = d.ntau * fill_kirr(d, tmp) * d.ns; }
   pl.main_units = TM * KC + 64 * pl.cht;      // A: 32 rows x 128 B; B: one 1 KB box per n-tile of the chunk
   if (pl.ksp == 7) plan_smem<7>(pl); else plan_smem<13>(pl);
   const int nsm = gwp::gw_num_sms();
@@ -828,7 +852,7 @@ static double flops(const gw_problem *p, const Plan &pl) {
     fl += (double)tm_rows * ndt * ndt * pl.ksp * 2048.0;                         // final
   }
   short tmp[128];
-  return fl * (double)d.nq * fill_kirr(d, tmp) * d.ntau;
+  return fl * (double)d.nq * fill_kirr(d, tmp) * d.ntau * d.ns;
 }
 
 template <int KSP>
@@ -840,17 +864,18 @@ static int launch_k(const Plan &pl, const Params &P, cudaStream_t st) {
   CUtensorMap tmW, tmV;
   int rc = gwp::make_tensor_map(&tmW, P.Wt, (size_t)P.d.ntau * P.d.nq * P.d.naux, P.d.naux, TM);
   if (rc) return rc;
-  rc = gwp::make_tensor_map(&tmV, P.V, (size_t)P.d.nk * P.d.nk * P.d.naux, P.d.nao * P.d.nao, KC);
+  rc = gwp::make_tensor_map(&tmV, P.V, gw_vblocks(P.d) * P.d.naux, P.d.nao * P.d.nao, KC);
   if (rc) return rc;
   sigma_ws_kernel<KSP><<<pl.grid, NTHR, pl.smem, st>>>(P, tmW, tmV);
   return (int)cudaGetLastError();
 }
 
-static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
+static int launch(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st, int acc_mode) {
   Plan pl = make_plan(p);
   if (!pl.ok) return GW_ESHAPE;
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
   Params P;
+  P.acc_mode = acc_mode;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.Wt = Wt; P.Sigma = Sigma;
   P.scratch = (c128 *)((char *)p->work + 256);
   P.nqt = pl.nqt; P.nitems = pl.nitems; P.nnt = pl.nnt; P.nchunk = pl.nchunk; P.cht = pl.cht;
@@ -875,7 +900,7 @@ size_t gw_stage3_workspace(const gw_problem *p) {
   return pl.ok ? pl.work_bytes : 0;
 }
 
-int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st) {
-  if (s3w::make_plan(p).ok) return s3w::launch(p, G, Wt, Sigma, st);
-  return s3::launch(p, G, Wt, Sigma, st);
+int gw_launch_stage3(const gw_problem *p, const c128 *G, const c128 *Wt, c128 *Sigma, cudaStream_t st, int acc_mode) {
+  if (s3w::make_plan(p).ok) return s3w::launch(p, G, Wt, Sigma, st, acc_mode);
+  return s3::launch(p, G, Wt, Sigma, st, acc_mode);
 }

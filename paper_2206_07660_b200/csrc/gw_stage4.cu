@@ -48,10 +48,10 @@ __global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
     const int item = s_item;
     __syncthreads();
     if (item >= P.nitems) break;
-    const int ql = item % d.nq, k = item / d.nq;
+    const int ql = item % d.nq, ik = item / d.nq, k = ik % d.nk, sg = ik / d.nk;      // sg: spin channel
     const int kp = gw_ksub(d, k, d.q0 + ql);
-    const c128 *V1 = P.V + ((size_t)k * d.nk + kp) * vb, *V2 = P.V + ((size_t)kp * d.nk + k) * vb;
-    const c128 *gm = P.gamma + (size_t)kp * n2;
+    const c128 *V1 = P.V + gw_vbwd(d, ql, kp, k) * vb, *V2 = P.V + gw_vfwd(d, ql, kp, k) * vb;   // V[k][k-q], V[k-q][k]
+    const c128 *gm = P.gamma + ((size_t)sg * d.nk + kp) * n2;
     for (int i = threadIdx.x; i < n2; i += NTHR) { const int r = i / nao, cc = i - r * nao; sGt[cc * ldp + r] = gm[i]; }
     double sgr[NCT][2], sgi[NCT][2];
 #pragma unroll
@@ -94,18 +94,21 @@ __global__ void __launch_bounds__(NTHR, 1) exchange_kernel(const Params P) {
       cp_async_wait<0>();
       __syncthreads();
     }
-    gwp::final_store<NCT>(P.part + ((size_t)ql * d.nk + k) * n2, sgr, sgi, 1.0, nao, ndt);
+    gwp::final_store<NCT>(P.part + (((size_t)sg * d.nq + ql) * d.nk + k) * n2, sgr, sgi, 1.0, nao, ndt);
   }
 }
 
-// K[k] = -(1/N_k) Σ_ql part[ql][k]   (fixed summation order)
-__global__ void exchange_reduce_kernel(GwDims d, const c128 *__restrict__ part, c128 *__restrict__ K) {
+// K[sg][k] = -(1/N_k) Σ_ql part[sg][ql][k]   (fixed summation order).  acc_mode: GW_ACC_CONTINUE starts from the unscaled sums in K,
+// GW_ACC_PARTIAL stores unscaled sums (out-of-core V: the q sum continues across slabs in the resident order).
+__global__ void exchange_reduce_kernel(GwDims d, const c128 *__restrict__ part, c128 *__restrict__ K, int acc_mode) {
   const size_t n = (size_t)d.nk * d.nao * d.nao;
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+  if (i >= n * d.ns) return;
+  const size_t sg = i / n, e = i - sg * n;
   double re = 0.0, im = 0.0;
-  for (int ql = 0; ql < d.nq; ql++) { const c128 v = part[(size_t)ql * n + i]; re += v.x; im += v.y; }
-  const double pref = -1.0 / (double)d.nk;
+  if (acc_mode & GW_ACC_CONTINUE) { re = K[i].x; im = K[i].y; }
+  for (int ql = 0; ql < d.nq; ql++) { const c128 v = part[(sg * d.nq + ql) * n + e]; re += v.x; im += v.y; }
+  const double pref = (acc_mode & GW_ACC_PARTIAL) ? 1.0 : -1.0 / (double)d.nk;
   K[i] = make_double2(pref * re, pref * im);
 }
 
@@ -116,7 +119,7 @@ static Plan make_plan(const gw_problem *p) {
   GwDims d = gw_dims(p);
   pl.g = gwp::pass_geom(d.nao);
   if (!pl.g.ok) { pl.ok = false; return pl; }
-  pl.nitems = d.nk * d.nq;
+  pl.nitems = d.nk * d.nq * d.ns;
   const int s_pass = PASS_ROWS * pl.g.ldp;
   // a final job covers one Q, or 1/kh of its K range if a whole Q does not fit; the ring is 3 deep, or 2 for the widest bases
   pl.ok = false;
@@ -135,7 +138,7 @@ static Plan make_plan(const gw_problem *p) {
   const int nsm = gwp::gw_num_sms();
   pl.grid = pl.nitems < nsm ? pl.nitems : nsm;
   pl.slab_units = (((size_t)TM * d.nao * d.nao) + 15) / 16 * 16;
-  pl.part_units = (size_t)d.nq * d.nk * d.nao * d.nao;
+  pl.part_units = (size_t)d.ns * d.nq * d.nk * d.nao * d.nao;
   pl.work_bytes = 256 + ((size_t)nsm * pl.slab_units + pl.part_units) * sizeof(c128);
   return pl;
 }
@@ -156,7 +159,7 @@ double gw_stage4_flops(const gw_problem *p) {
     const int tm_rows = (d.naux - Q0) < s4::TM ? (d.naux - Q0) : s4::TM;
     tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.g.ndt * pl.g.ksp + (double)tm_rows * pl.g.ndt * pl.g.ndt * pl.kspf * pl.kh;
   }
-  return tiles * (double)d.nk * d.nq * 2048.0;
+  return tiles * (double)d.nk * d.nq * d.ns * 2048.0;
 }
 
 template <int KSP_MAX, int NCT>
@@ -167,7 +170,7 @@ static int launch_exchange(const s4::Plan &pl, const s4::Params &P, cudaStream_t
   return (int)cudaGetLastError();
 }
 
-int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st) {
+int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream_t st, int acc_mode) {
   s4::Plan pl = s4::make_plan(p);
   if (!pl.ok) return GW_ESHAPE;
   if (!p->work || p->work_bytes < pl.work_bytes || (((uintptr_t)p->work) & 255)) return GW_ENOMEM;
@@ -191,7 +194,7 @@ int gw_launch_stage4(const gw_problem *p, const c128 *gamma, c128 *K, cudaStream
     else rc = launch_exchange<16, 8>(pl, P, st);
   }
   if (rc) return rc;
-  const size_t n = (size_t)P.d.nk * P.d.nao * P.d.nao;
-  s4::exchange_reduce_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(P.d, P.part, K);
+  const size_t n = (size_t)P.d.ns * P.d.nk * P.d.nao * P.d.nao;
+  s4::exchange_reduce_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(P.d, P.part, K, acc_mode);
   return (int)cudaGetLastError();
 }

@@ -6,6 +6,8 @@ transposed operand, wrong k±q table, wrong normalisation) fails at least one of
 import numpy as np
 import pytest
 
+import torch
+
 import gwgen
 from gwgen.configs import GWConfig
 from gwgen.fock import fermi
@@ -525,3 +527,61 @@ def test_P17_scgw_iteration_noninteracting_limit(problems, oracle_lib):
         g = -np.exp(-np.outer(p.tau, x)) / (1.0 + np.exp(-cfg.beta * x))
         ref = np.einsum("in,tn,jn->tij", C, g, C.conj())
         assert np.max(np.abs(r["G_new"][:, k] - ref)) < 1e-7
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# Collinear spin channels: the oracle's spin routines are the literal sum over sigma of the
+# single-channel ones.  Pins: two identical channels == closed shell; two different channels == the Lindhard closed form summed
+# over the channels' own spectra; Eq. 20's sigma_1 sum by einsum.
+# ----------------------------------------------------------------------------------------------------------------
+def test_P18_two_identical_channels_equal_closed_shell(problems, oracle_results, oracle_lib):
+    import dataclasses
+    p = problems("T")
+    cfg1 = dataclasses.replace(p.cfg, spin_deg=1)
+    vb = oracle_lib.VBlocks(p.cfg, p.V.numpy())
+    ref = oracle_results("T")
+    G2 = np.ascontiguousarray(np.stack([p.G, p.G])); g2 = np.ascontiguousarray(np.stack([p.gamma, p.gamma]))
+    assert relerr(oracle_lib.polarization_spin(cfg1, vb, G2), ref["P0t"]) < 1e-15          # spin_deg = 2 of the closed shell
+    S2 = oracle_lib.selfenergy_spin(cfg1, vb, G2, ref["Wt"])
+    K2 = oracle_lib.exchange_spin(cfg1, vb, g2)
+    for sg in range(2):
+        assert np.array_equal(S2[sg], ref["Sigma"]) and np.array_equal(K2[sg], ref["K"])
+    assert relerr(oracle_lib.hartree_spin(cfg1, vb, g2), oracle_lib.hartree(p.cfg, vb, p.gamma)) < 1e-15
+
+
+def test_P19_spin_polarised_lindhard_and_hartree(problems, oracle_lib):
+    import copy
+    import dataclasses
+    p = problems("T")
+    cfg1 = dataclasses.replace(p.cfg, spin_deg=1)
+    Gs, gs = gwgen.make_spin_channels(p, 2)
+    assert relerr(Gs[1], Gs[0]) > 0.1                                                      # the channels really differ
+    vb = oracle_lib.VBlocks(p.cfg, p.V.numpy())
+    P0 = oracle_lib.polarization_spin(cfg1, vb, Gs)
+    chans = []
+    for ch in range(2):
+        pc = copy.copy(p)
+        pc.cfg = cfg1
+        pc.eps, pc.U = gwgen.make_fock(p.cfg, p.mesh, channel=ch)
+        chans.append(pc)
+    rng = np.random.default_rng(8)
+    for _ in range(4):
+        q, t = int(rng.integers(p.cfg.nk)), int(rng.integers(p.cfg.ntau))
+        ref = lindhard_tau(chans[0], q, t) + lindhard_tau(chans[1], q, t)
+        assert relerr(P0[t, q], ref) < 1e-12
+        assert relerr(oracle_lib.p0t_slice_spin(cfg1, vb, Gs[:, t], Gs[:, p.cfg.ntau - 1 - t], q), P0[t, q]) < 1e-15
+    V = p.V.numpy()
+    Vd = np.stack([V[k, k] for k in range(p.cfg.nk)])
+    rho = np.einsum("skab,kQba->Q", gs, Vd)
+    assert relerr(oracle_lib.hartree_spin(cfg1, vb, gs), np.einsum("kQij,Q->kij", Vd, rho) / p.cfg.nk) < 1e-13
+
+
+def test_qslab_layout_is_a_pure_gather(problems):
+    """gwgen.to_qslab (the GW_V_QSLAB layout of include/gw.h) only moves blocks: slot (q, k, 0) = V[k][k+q], slot (q, k, 1) = V[k+q][k]."""
+    p = problems("R")
+    add = p.mesh.add_table()
+    S = gwgen.to_qslab(p.V, p.mesh, 3, 9)
+    for q in (3, 5, 8):
+        for k in (0, 4, p.cfg.nk - 1):
+            kq = int(add[k][q])
+            assert torch.equal(S[q - 3, k, 0], p.V[k, kq]) and torch.equal(S[q - 3, k, 1], p.V[kq, k])
