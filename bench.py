@@ -35,6 +35,8 @@ def parse_args():
     ap.add_argument("--no-tr-mode", action="store_true", help="skip the extra GW_SYM_TR measurement")
     ap.add_argument("--no-largest", action="store_true", help="skip the largest_config leg (config 4) of the default run")
     ap.add_argument("--largest-steps", type=int, default=2)
+    ap.add_argument("--no-out-of-core", action="store_true", help="skip the out-of-core leg (config 4 with V streamed from host memory)")
+    ap.add_argument("--v-budget-gb", type=float, default=24.0, help="HBM budget of the two V slab buffers in the out-of-core leg")
     ap.add_argument("--traffic-from-ncu", default=None, metavar="CSV",
                     help="no benchmark: read an ncu --csv log with dram__bytes_read.sum / dram__bytes_write.sum per launch and "
                          "record it in profiles/traffic.json under --config, with the hash of the kernel sources")
@@ -235,8 +237,10 @@ def traffic_from_ncu(csv_path, cfg_name):
 
 
 def stage_names(cfg):
-    return {0: "s1::p0_kernel (stage 1, Eq. 28b)",
-            2: ("s3w::sigma_ws_kernel" if (cfg.nao + 3) // 4 == 7 else "s3::sigma_kernel") + " (stage 3, Eq. 31)"}
+    ksp = (cfg.nao + 3) // 4
+    s1 = "s1::p0_kernel<3M>" if (cfg.naux + 7) // 8 <= 32 else "s1::p0_kernel<4M>"
+    return {0: s1 + " (stage 1, Eq. 28b)",
+            2: ("s3w::sigma_ws_kernel<3M main>" if ksp in (7, 13) else "s3::sigma_kernel") + " (stage 3, Eq. 31)"}
 
 
 def roofline_of(cfg, nq, stage_ms, executed, peak, peak_note):
@@ -439,6 +443,30 @@ def run_ours(args):
                    "stage_ms": {"polarization": b_stage[0], "screened_interaction": b_stage[1], "selfenergy": b_stage[2], "exchange": b_stage[3]},
                    "roofline": roofline_of(big, brun.nq, b_stage, b_exec, peak, peak_note), "clocks": b_clocks, "info": [-1, -1],
                    "gpu_launches": gw.gw_launch_count(brun.prob) * args.largest_steps}
+        # ---- out_of_core: the same config-4 iteration with V in pinned HOST memory, streamed through two device q-slab buffers of
+        #      --v-budget-gb in total (gw_sigma_iteration_stream; the paper reads V a k-batch at a time).  One timed
+        #      iteration through the C ABI, host buffers in and out; Sigma must equal the resident run bit for bit. ----
+        if not args.no_out_of_core:
+            try:
+                S_res = brun.Sigma.cpu()
+                bp = brun.p
+                hV = torch.empty(bp.V.shape, dtype=torch.complex128, pin_memory=True); hV.copy_(bp.V)
+                hG = torch.from_numpy(bp.G).pin_memory(); hg = torch.from_numpy(bp.gamma).pin_memory()
+                hTw = torch.from_numpy(bp.T_wt).pin_memory(); hTt = torch.from_numpy(bp.T_tw).pin_memory()
+                brun = None; bp.V = None
+                torch.cuda.empty_cache()
+                hprob = gw.GWProblem(big.mesh, big.nao, big.naux, big.ntau, big.nw, big.beta, hV, hTw, hTt, big.spin_deg)
+                t0 = time.perf_counter()
+                r = gw.gw_sigma_iteration_stream(hprob, hG, hg, int(args.v_budget_gb * 1e9))
+                torch.cuda.synchronize()
+                ooc_s = time.perf_counter() - t0
+                largest["out_of_core"] = {"value": ooc_s, "unit": "s", "steps": 1, "v_budget_bytes": int(args.v_budget_gb * 1e9),
+                                          "V_bytes_host": big.bytes_V(), "h2d_gb": r["stats"]["h2d_gb"], "slabs": r["stats"]["slabs"],
+                                          "q_per_slab": r["stats"]["q_per_slab"], "ratio_to_resident": ooc_s / b_s,
+                                          "sigma_bit_identical_to_resident": bool(torch.equal(r["Sigma"], S_res))}
+                del hV, hG, hg, hprob, r, S_res
+            except Exception as e:       # e.g. not enough pinned host memory on this box: reported, never fatal for the headline
+                largest["out_of_core"] = {"error": str(e)[:300]}
         brun = None
         torch.cuda.empty_cache()
 
