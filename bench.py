@@ -40,6 +40,9 @@ def parse_args():
     ap.add_argument("--traffic-from-ncu", default=None, metavar="CSV",
                     help="no benchmark: read an ncu --csv log with dram__bytes_read.sum / dram__bytes_write.sum per launch and "
                          "record it in profiles/traffic.json under --config, with the hash of the kernel sources")
+    ap.add_argument("--traffic-scale-to", default=None, metavar="CFG",
+                    help="with --traffic-from-ncu: also record the capture under CFG, scaled by ntau(CFG)/ntau(--config) (the per-launch "
+                         "traffic of stages 1 and 3 is proportional to the number of tau nodes; e.g. the cfgQ capture stands in for cfg4)")
     return ap.parse_args()
 
 
@@ -205,7 +208,7 @@ def traffic_lookup(cfg_name, stage):
     return rec.get("stage1_bytes" if stage == 0 else "stage3_bytes")
 
 
-def traffic_from_ncu(csv_path, cfg_name):
+def traffic_from_ncu(csv_path, cfg_name, scale_to=None):
     """Parse `ncu --csv --metrics dram__bytes_read.sum,dram__bytes_write.sum,...` output: one row per (launch, metric)."""
     import csv
     rows = [r for r in csv.reader(open(csv_path)) if len(r) > 5]
@@ -231,6 +234,17 @@ def traffic_from_ncu(csv_path, cfg_name):
     out["kernel_revision"] = kernel_revision()
     out["source"] = os.path.basename(csv_path)
     allrec[cfg_name] = out
+    if scale_to:
+        import gwgen
+        src = next(c for c in gwgen.CONFIGS.values() if c.name == cfg_name)
+        dst = gwgen.get_config(scale_to)
+        f = dst.ntau / src.ntau
+        sc = dict(out)
+        for k in ("stage1_bytes", "stage3_bytes"):
+            if k in sc:
+                sc[k] = sc[k] * f
+        sc["scaled_from"] = f"{cfg_name} x {f:g} (ntau {src.ntau} -> {dst.ntau}, same mesh, basis and kernels)"
+        allrec[dst.name] = sc
     json.dump(allrec, open(TRAFFIC_JSON, "w"), indent=1, sort_keys=True)
     print(json.dumps({cfg_name: out}))
     return 0
@@ -274,12 +288,20 @@ class DeviceRun:
         import gwgen
         from paper_2206_07660_b200.dist import shard_range
         self.gw, self.cfg, self.world = gw, cfg, world
-        self.p = gwgen.make_problem(cfg, v_device=dev)
         q0, q1 = shard_range(cfg.nk, world, rank)
         self.q0, self.q1, self.nq = q0, q1, q1 - q0
+        if world > 1:
+            # one rank holds only its q-slab of V: the 2 nk blocks per q of its shard serve all four stages (gw.h "V layouts")
+            self.p = gwgen.make_problem(cfg, with_V=False)
+            self.p.V = gwgen.make_V_qslab(cfg, self.p.mesh, q0, q1, device=dev)
+            layout = gw.GW_V_QSLAB
+        else:
+            self.p = gwgen.make_problem(cfg, v_device=dev)
+            layout = gw.GW_V_FULL
         p = self.p
         self.T_wt, self.T_tw = torch.from_numpy(p.T_wt).to(dev), torch.from_numpy(p.T_tw).to(dev)
-        self.prob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, p.V, self.T_wt, self.T_tw, cfg.spin_deg, q0, q1, symmetry)
+        self.prob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, p.V, self.T_wt, self.T_tw, cfg.spin_deg, q0, q1, symmetry,
+                                 v_layout=layout)
         self.G = torch.from_numpy(p.G).to(dev)
         self.gamma = torch.from_numpy(p.gamma).to(dev)
         self.P = torch.empty((cfg.ntau, self.nq, cfg.naux, cfg.naux), dtype=torch.complex128, device=dev)   # P0t, then Wt in place
@@ -512,7 +534,7 @@ def main():
     args = parse_args()
     if args.traffic_from_ncu:
         import gwgen
-        return traffic_from_ncu(args.traffic_from_ncu, gwgen.get_config(args.config).name)
+        return traffic_from_ncu(args.traffic_from_ncu, gwgen.get_config(args.config).name, args.traffic_scale_to)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -120,3 +120,19 @@ def to_qslab(V, mesh, q_begin, q_end):
             out[q - q_begin, k, 0] = V[k, kq]
             out[q - q_begin, k, 1] = V[kq, k]
     return out
+
+
+def make_V_qslab(cfg, mesh, q_begin, q_end, device="cpu", raw=False):
+    """The q-slab of V for the shard [q_begin, q_end) generated directly (only the 2 nk blocks per q a rank needs, SURVEY.md §8e:
+    "V slice {V[k][k+q] : q mine}"): out[q - q_begin][k][0] = V[k][k+q], out[q - q_begin][k][1] = V[k+q][k].  Same values as
+    to_qslab(make_V(...)) up to the rounding order of the four-term group average (every block is a pure function of (seed, k1, k2))."""
+    add = mesh.add_table()
+    neg = mesh.neg()
+    nk = mesh.nk
+    out = torch.empty((q_end - q_begin, nk, 2, cfg.naux, cfg.nao, cfg.nao), dtype=torch.complex128, device=device)
+    for q in range(q_begin, q_end):
+        for k in range(nk):
+            kq = int(add[k][q])
+            out[q - q_begin, k, 0] = make_V_block(cfg, mesh, k, kq, device, neg, raw)
+            out[q - q_begin, k, 1] = make_V_block(cfg, mesh, kq, k, device, neg, raw)
+    return out

@@ -153,3 +153,28 @@ def test_streamed_iteration_equals_resident(problems, oracle_results, name, ns, 
         assert relerr(out["Sigma"].numpy(), ref["Sigma"]) <= TOL and relerr(out["K"].numpy(), ref["K"]) <= TOL
     with pytest.raises(gw.GWError):
         gw.gw_sigma_iteration_stream(hprob, G.pin_memory(), gamma.pin_memory(), perq)      # budget below two one-q slabs: GW_ENOMEM
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two GPUs")
+def test_two_gpu_q_shards_sum_to_oracle(problems, oracle_results):
+    """Each of two GPUs evaluates its q shard from its own V q-slab (generated per rank, as bench.py --gpus N does); the partial
+    Sigma and K add up to the oracle's full result (the NCCL all-reduce of dist.py is a plain sum of these partials)."""
+    import paper_2206_07660_b200 as gw
+    from paper_2206_07660_b200.dist import shard_range
+    p = problems("R")
+    cfg = p.cfg
+    ref = oracle_results("R")
+    S_tot, K_tot = None, None
+    for rank in range(2):
+        dev = torch.device("cuda", rank)
+        with torch.cuda.device(dev):
+            q0, q1 = shard_range(cfg.nk, 2, rank)
+            V = gwgen.make_V_qslab(cfg, p.mesh, q0, q1, device=dev)
+            prob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, V, torch.from_numpy(p.T_wt).to(dev), torch.from_numpy(p.T_tw).to(dev),
+                                cfg.spin_deg, q0, q1, 0, 1, gw.GW_V_QSLAB)
+            out = gw.gw_sigma_iteration(prob, torch.from_numpy(p.G).to(dev), torch.from_numpy(p.gamma).to(dev))
+            torch.cuda.synchronize()
+            assert relerr(out["Wt"].cpu().numpy(), ref["Wt"][:, q0:q1]) <= TOL
+            S_tot = out["Sigma"].cpu() if S_tot is None else S_tot + out["Sigma"].cpu()
+            K_tot = out["K"].cpu() if K_tot is None else K_tot + out["K"].cpu()
+    assert relerr(S_tot.numpy(), ref["Sigma"]) <= TOL and relerr(K_tot.numpy(), ref["K"]) <= TOL
