@@ -133,6 +133,13 @@ int gw_screened_interaction(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt
  *   an entry whose factorisation failed (see info) is unspecified. */
 int gw_screened_interaction_phi(const gw_problem *p, const gw_c128 *P0t, gw_c128 *Wt, int32_t *info, double *phi, void *stream);
 
+/* Phi~_GW itself, Eq. 37, from the summand above and the caller's quadrature weights of the Matsubara sum
+ * (the paper prints none for its sparse grid; reading R18; on an n >= 0 grid the weights carry the factor 2 of
+ * the mirror images n < 0):
+ *   *out = (1/(2 N_k beta)) Σ_q Σ_n w[n] phi[n][q]          (a q shard yields its partial sum: add the shards)
+ *   nk = N_k of the whole mesh;  w : device double [nw];  phi : device double [nw][nq];  out : device double.  Fixed summation order. */
+int gw_phi_gw(int32_t nk, int32_t nq, int32_t nw, double beta, const double *w, const double *phi, double *out, void *stream);
+
 /* Generic imaginary-axis grid transform — the kernel of Eq. 28a / Eq. 30 exposed for the next workflow step, the fermionic
  * τ→iω_n transform of Σ̃ (Eq. 13; Fig. 4 step after the hot path):
  *   Y[o][m] = Σ_i T[o][i] X[i][m],   o < n_out, i < n_in, m < len      (complex T; n_out, n_in <= 200)

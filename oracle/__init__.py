@@ -317,3 +317,11 @@ def hartree_spin(cfg, vb, gammas):
     """Eq. 20: the sum over sigma_1 runs over the channels (times cfg.spin_deg)."""
     c1 = _one_channel(cfg)
     return cfg.spin_deg * sum(hartree(c1, vb, np.ascontiguousarray(gammas[sg])) for sg in range(gammas.shape[0]))
+
+
+def phi_gw(nk, beta, w, phi):
+    """Eq. 37 with quadrature weights w[n]: (1/(2 N_k beta)) sum_q sum_n w[n] phi[n][q]."""
+    w = np.ascontiguousarray(w, dtype=np.float64); phi = np.ascontiguousarray(phi, dtype=np.float64)
+    lib().gwref_phi_gw.restype = ctypes.c_double
+    lib().gwref_phi_gw.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p]
+    return float(lib().gwref_phi_gw(int(nk), int(phi.shape[1]), int(phi.shape[0]), float(beta), _pd(w), _pd(phi)))

@@ -507,6 +507,18 @@ int gwref_find_mu(const gwref_dims *d, int nwf, const double *omega, const c128 
   return fail;
 }
 
+/* ---- Dynamical part of the GW Luttinger-Ward functional, Eq. 37:
+ *   Phi~_GW = (1/(2 N_k)) sum_q (1/beta) sum_n tr{ ln[I - P0^q(i Omega_n)] + P0^q(i Omega_n) }
+ * evaluated on the sampled frequencies with the caller's quadrature weights w[n] for the Matsubara sum (reading R18: the
+ * paper prints none; for n >= 0 grids the weights carry the factor 2 of the n < 0 mirror images):
+ *   Phi~_GW = (1/(2 N_k beta)) sum_q sum_n w[n] phi[n][q],   phi from gwref_phi.   phi: [nw][nq] (nq = nk for the full mesh). */
+double gwref_phi_gw(int nk, int nq, int nw, double beta, const double *w, const double *phi) {
+  double tot = 0.0;
+  for (int q = 0; q < nq; q++)
+    for (int n = 0; n < nw; n++) tot += w[n] * phi[(size_t)n * nq + q];
+  return tot / (2.0 * (double)nk * beta);
+}
+
 /* Y = a X + b Y (simple mixing of two iterates, PAPER.md:326-330 mentions DIIS; plain damping is the baseline it improves on) */
 void gwref_axpby(size_t n, c128 a, const c128 *X, c128 b, c128 *Y) {
   for (size_t i = 0; i < n; i++) Y[i] = a * X[i] + b * Y[i];

@@ -62,11 +62,12 @@ def lib():
         L.gw_find_mu.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, vp,
                                  ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(i32), vp]
         L.gw_axpby.argtypes = [sz, dbl, dbl, vp, dbl, dbl, vp, vp]
+        L.gw_phi_gw.argtypes = [i32, i32, i32, dbl, vp, vp, vp, vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version",
-                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream"):
+                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -198,6 +199,15 @@ def gw_screened_interaction_phi(prob, P0t, Wt=None, info=None, phi=None, stream=
                                              ctypes.c_void_p(info.data_ptr()), ctypes.c_void_p(phi.data_ptr()),
                                              _stream(stream)), "gw_screened_interaction_phi")
     return Wt, info, phi
+
+
+def gw_phi_gw(prob, w, phi, stream=None):
+    """Eq. 37: Phi~_GW = (1/(2 N_k beta)) sum_q sum_n w[n] phi[n][q] (1-element CUDA float64 tensor; a q shard gives its partial sum)."""
+    out = torch.empty(1, dtype=torch.float64, device=phi.device)
+    if tuple(phi.shape) != (prob.nw, prob.nq) or tuple(w.shape) != (prob.nw,):
+        raise GWError("gw_phi_gw: need w [nw] and phi [nw][nq]")
+    _check(lib().gw_phi_gw(prob.nk, prob.nq, prob.nw, prob.beta, _f64(w, "w"), _f64(phi, "phi"), _f64(out, "out"), _stream(stream)), "gw_phi_gw")
+    return out
 
 
 def gw_transform(T, X, Y=None, stream=None):

@@ -322,6 +322,12 @@ done:
   return rc;
 }
 
+extern "C" int gw_phi_gw(int32_t nk, int32_t nq, int32_t nw, double beta, const double *w, const double *phi, double *out, void *stream) {
+  if (nk <= 0 || nq <= 0 || nw <= 0 || !(beta > 0) || !w || !phi || !out || (((uintptr_t)w | (uintptr_t)phi | (uintptr_t)out) & 7)) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  return gw_launch_phi_gw(nk, nq, nw, beta, w, phi, out, (cudaStream_t)stream);
+}
+
 extern "C" int gw_axpby(size_t n, double a_re, double a_im, const gw_c128 *X, double b_re, double b_im, gw_c128 *Y, void *stream) {
   if (!aligned16(X) || !aligned16(Y)) return GW_EINVAL;
   int rc = check_arch(); if (rc) return rc;

@@ -101,6 +101,7 @@ int gw_launch_dyson_update(int nk, int nao, int nwf, const double *omega, double
                            int32_t *info, cudaStream_t st);
 int gw_launch_electron_count(int nk, int nao, int nwf, int spin_deg, const c128 *t_beta, const c128 *S, const c128 *G_w, c128 *partial, double *ne,
                              cudaStream_t st);
+int gw_launch_phi_gw(int nk, int nq, int nw, double beta, const double *w, const double *phi, double *out, cudaStream_t st);
 int gw_launch_axpby(size_t n, c128 a, const c128 *X, c128 b, c128 *Y, cudaStream_t st);
 size_t gw_stage1_workspace(const gw_problem *p);
 size_t gw_stage2_workspace(const gw_problem *p);

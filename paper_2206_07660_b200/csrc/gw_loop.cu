@@ -158,6 +158,17 @@ __global__ void __launch_bounds__(NT) axpby_kernel(size_t n, c128 a, const c128 
   }
 }
 
+// ---- Eq. 37 with quadrature weights: out = (1/(2 N_k beta)) Σ_q Σ_n w[n] phi[n][q]; one CTA, fixed order
+__global__ void __launch_bounds__(NT) phi_gw_kernel(int nk, int nq, int nw, double beta, const double *__restrict__ w, const double *__restrict__ phi,
+                                                    double *__restrict__ out) {
+  __shared__ c128 red[NT];
+  double acc = 0.0;
+  for (int q = threadIdx.x; q < nq; q += NT)
+    for (int n = 0; n < nw; n++) acc = fma(w[n], phi[(size_t)n * nq + q], acc);
+  const c128 tot = block_sum(make_double2(acc, 0.0), red);
+  if (threadIdx.x == 0) *out = tot.x / (2.0 * (double)nk * beta);
+}
+
 static size_t dyson_smem(int nao) { return ((size_t)nao * (nao + 1) + nao) * sizeof(c128) + (size_t)nao * sizeof(int); }
 
 }  // namespace lp
@@ -197,5 +208,10 @@ int gw_launch_axpby(size_t n, c128 a, const c128 *X, c128 b, c128 *Y, cudaStream
   size_t blocks = (n + lp::NT - 1) / lp::NT;
   if (blocks > 148 * 16) blocks = 148 * 16;
   lp::axpby_kernel<<<(unsigned)blocks, lp::NT, 0, st>>>(n, a, X, b, Y, !(b.x == 0.0 && b.y == 0.0));
+  return (int)cudaGetLastError();
+}
+
+int gw_launch_phi_gw(int nk, int nq, int nw, double beta, const double *w, const double *phi, double *out, cudaStream_t st) {
+  lp::phi_gw_kernel<<<1, lp::NT, 0, st>>>(nk, nq, nw, beta, w, phi, out);
   return (int)cudaGetLastError();
 }

@@ -120,3 +120,21 @@ def test_scgw_iteration_parity(problems, oracle_lib, name):
         assert report(name, "scgw " + key, got[key].cpu().numpy(), ref[key]) <= (TOL if key not in ("G_w", "G_new", "G") else 1e-9), key
     print(f"scgw {name}: mu {got['mu']:.12f} (oracle {ref['mu']:.12f}), N_e {got['ne']:.12f}, {got['n_eval']} N_e evaluations")
     assert abs(got["mu"] - ref["mu"]) < 1e-9 and abs(got["ne"] - target) < 1e-9
+
+
+def test_phi_gw_parity(problems, oracle_lib):
+    """Eq. 37: the Matsubara / q sum of the summand returned by gw_screened_interaction_phi, with quadrature weights."""
+    import paper_2206_07660_b200 as gw
+    p = problems("R")
+    cfg = p.cfg
+    prob, G, _ = device_problem(p)
+    P0t = gw.gw_polarization(prob, G)
+    _, _, phi = gw.gw_screened_interaction_phi(prob, P0t)
+    w = np.where(p.nbos == 0, 1.0, 2.0)                      # n >= 0 grid: mirror images n < 0 folded in
+    got = float(gw.gw_phi_gw(prob, torch.from_numpy(w).cuda(), phi).cpu())
+    ref = oracle_lib.phi_gw(cfg.nk, cfg.beta, w, phi.cpu().numpy())
+    assert abs(got - ref) <= 1e-13 * abs(ref)
+    P0 = oracle_lib.polarization(cfg, oracle_lib.VBlocks(cfg, p.V.numpy()), p.G)
+    _, P0w, _ = oracle_lib.screened_interaction(cfg, p.T_wt, p.T_tw, P0, want_freq=True)
+    phi_ref = np.array([[oracle_lib.phi(P0w[n, q]) for q in range(cfg.nk)] for n in range(cfg.nw)])
+    assert abs(got - oracle_lib.phi_gw(cfg.nk, cfg.beta, w, phi_ref)) <= 1e-10 * abs(ref)

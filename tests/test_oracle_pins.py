@@ -585,3 +585,20 @@ def test_qslab_layout_is_a_pure_gather(problems):
         for k in (0, 4, p.cfg.nk - 1):
             kq = int(add[k][q])
             assert torch.equal(S[q - 3, k, 0], p.V[k, kq]) and torch.equal(S[q - 3, k, 1], p.V[kq, k])
+
+
+def test_P20_phi_gw_scalar_closed_form_and_definition(oracle_lib):
+    """Eq. 37 summed with quadrature weights.  Scalar model of P1 (nk = nao = naux = 1, single pole): P0(i Omega_n) = p delta_n0 with
+    p = -s v^2 beta f (1 - f), so Phi~_GW = (1/(2 beta)) w_0 [ln(1 - p) + p]; and the plain double sum on random data."""
+    beta, eps, v, s = 10.0, 0.3, 0.7, 2
+    f = 1.0 / (1.0 + np.exp(beta * eps))
+    p = -s * v * v * beta * f * (1.0 - f)
+    nw = 5
+    w = np.array([1.0, 2.0, 2.0, 2.0, 2.0])
+    phi = np.zeros((nw, 1))
+    for n in range(nw):
+        phi[n, 0] = oracle_lib.phi(np.array([[p if n == 0 else 0.0]], dtype=np.complex128))
+    assert abs(oracle_lib.phi_gw(1, beta, w, phi) - (np.log(1.0 - p) + p) / (2.0 * beta)) < 1e-15
+    rng = np.random.default_rng(4)
+    w = rng.uniform(0.5, 2.0, 7); phi = rng.normal(size=(7, 11))
+    assert abs(oracle_lib.phi_gw(12, 3.0, w, phi) - np.einsum("n,nq->", w, phi) / (2 * 12 * 3.0)) < 1e-14
