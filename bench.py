@@ -35,6 +35,7 @@ def parse_args():
     ap.add_argument("--no-tr-mode", action="store_true", help="skip the extra GW_SYM_TR measurement")
     ap.add_argument("--no-largest", action="store_true", help="skip the largest_config leg (config 4) of the default run")
     ap.add_argument("--largest-steps", type=int, default=2)
+    ap.add_argument("--no-closure", action="store_true", help="skip the loop-closure leg (Sigma -> G' on the headline config)")
     ap.add_argument("--no-out-of-core", action="store_true", help="skip the out-of-core leg (config 4 with V streamed from host memory)")
     ap.add_argument("--v-budget-gb", type=float, default=24.0, help="HBM budget of the two V slab buffers in the out-of-core leg")
     ap.add_argument("--traffic-from-ncu", default=None, metavar="CSV",
@@ -382,6 +383,9 @@ def run_ours(args):
     peak_note = ("measured in this run: max of the register-resident DMMA.8x8x4 loop (%.2f TFLOP/s) and DFMA loop (%.2f TFLOP/s) on all "
                  "SMs (gw_fp64_peak, gw_fp64_peak_dfma); MEASURED_PEAKS.json has no FP64 entry" % (peak_dmma, peak_dfma))
 
+    # the three complex tile-product schemes in the bare inner loop (context for the 3M / 4M choice, profiles/r02_3m_vs_4m.md)
+    cmma = {k: gw.gw_complex_mma_probe(m, 100.0) for m, k in ((0, "4m"), (1, "3m_sums_in_registers"), (2, "3m_presummed_b"))}
+
     # ---- synthetic inputs, resident in HBM (generation is not timed) ----
     run = DeviceRun(gw, cfg, dev, world, rank)
     nq = run.nq
@@ -418,6 +422,45 @@ def run_ours(args):
                    "symmetry": "GW_SYM_TR: tau <-> beta-tau, q <-> -q and Hermitian tiles in stage 1, k <-> -k in stage 3 (exact for these inputs)",
                    "sigma_rel_diff_vs_literal": dev_rel, "tflops_executed": sum(ex_tr) / tr_s * 1e-12}
         del S_lit, prob_tr
+
+    # ---- loop closure (Fig. 4 steps 3-4): from the Sigma(tau), K just computed to the next G(tau), every step a C-ABI
+    #      call, timed with CUDA events (gw_find_mu by wall clock: it synchronises after every N_e evaluation).  Reported beside. ----
+    closure = None
+    if world == 1 and not args.no_closure:
+        mesh = run.p.mesh
+        H0n, Sn = gwgen.make_h0_s(cfg, mesh, run.p.eps, run.p.U)
+        fgn = gwgen.make_fermionic_grids(cfg.ntau, cfg.beta)
+        fg = {k: torch.from_numpy(np.ascontiguousarray(fgn[k])).to(dev) for k in ("omega", "T_wt_f", "T_tw_f", "t_beta", "e_beta")}
+        H0, S = torch.from_numpy(H0n).to(dev), torch.from_numpy(Sn).to(dev)
+        n_target = cfg.spin_deg * (cfg.nao // 2)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(8)]
+        st = run.stream
+        ev[0].record(st)
+        Gb = gw.gw_transform(fg["e_beta"].reshape(1, -1), run.G, stream=st)[0].contiguous()
+        gam = gw.gw_axpby(-1.0, Gb, 0.0, torch.empty_like(Gb), st)
+        ev[1].record(st)
+        J = gw.gw_hartree(run.prob, gam, stream=st)
+        ev[2].record(st)
+        Sw = gw.gw_transform(fg["T_wt_f"], run.Sigma, stream=st)
+        ev[3].record(st)
+        F = gw.gw_axpby(1.0, J, 1.0, gw.gw_axpby(1.0, run.K, 1.0, H0.clone(), st), st)
+        ev[4].record(st)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        mu, ne, G_w, n_eval = gw.gw_find_mu(fg["omega"], fg["t_beta"], S, F, Sw, n_target, -1.0, 1.0, 1e-12, cfg.spin_deg, stream=st)
+        mu_ms = (time.perf_counter() - t0) * 1e3
+        ev[5].record(st)
+        G_new = gw.gw_transform(fg["T_tw_f"], G_w, stream=st)
+        ev[6].record(st)
+        gw.gw_axpby(0.7, G_new, 0.3, run.G.clone(), st)
+        ev[7].record(st)
+        torch.cuda.synchronize()
+        el = lambda a, b: ev[a].elapsed_time(ev[b])
+        closure = {"unit": "ms", "gamma_from_G_beta": el(0, 1), "hartree_J": el(1, 2), "sigma_tau_to_iw": el(2, 3), "fock_assembly": el(3, 4),
+                   "find_mu": mu_ms, "find_mu_evaluations": n_eval, "mu": mu, "n_e_minus_target": ne - n_target,
+                   "g_iw_to_tau": el(5, 6), "damping": el(6, 7),
+                   "total": el(0, 4) + mu_ms + el(5, 7), "fraction_of_sigma_build": (el(0, 4) + mu_ms + el(5, 7)) / ms_per_step}
+        del H0, S, fg, Gb, gam, J, Sw, F, G_w, G_new
 
     # ---- e2e: the same iteration through the C ABI with HOST buffers (copies inside the timed region) ----
     e2e = None
@@ -507,10 +550,12 @@ def run_ours(args):
            "tflops_executed_per_gpu": sum(executed) / (ms_per_step * 1e-3) * 1e-12,
            "frac_of_fp64_peak_nominal": total_nom / (ms_per_step * 1e-3) * 1e-12 / peak / world,
            "fp64_peak_tflops_measured": peak, "fp64_peak_dmma": peak_dmma, "fp64_peak_dfma": peak_dfma,
+           "complex_mma_inner_loop_algorithmic_tflops": cmma,
            "stage_ms": {"polarization": stage_ms[0], "screened_interaction": stage_ms[1], "selfenergy": stage_ms[2],
                         "exchange": stage_ms[3], "allreduce": stage_ms[4]},
            "roofline": roof, "gpu_launches": launches * args.steps,
            "clocks": clocks, "info": [-1, -1], "kernel_revision": kernel_revision()}
+    out["loop_closure"] = closure
     out["time_reversal_mode"] = tr_mode
     out["largest_config"] = largest
     out["e2e"] = e2e

@@ -241,6 +241,13 @@ int gw_fp64_peak(double ms, double *tflops, void *stream);
  * bench.py is the larger of the two. */
 int gw_fp64_peak_dfma(double ms, double *tflops, void *stream);
 
+/* Inner loop of the main GEMMs alone (operands resident in shared memory, 8 warps per CTA, one CTA per SM) for about `ms` milliseconds, for
+ * the three ways of forming a complex 8x8x4 tile product on DMMA.8x8x4 that profiles/r02_3m_vs_4m.md compares:
+ *   mode 0: 4M (four real DMMAs);  mode 1: 3M Karatsuba with the operand sums formed by DADD in registers (what the kernels run);
+ *   mode 2: 3M with the B operand's sums pre-formed in shared memory.
+ * *tflops = ALGORITHMIC TFLOP/s, 8 flops per complex multiply-add. */
+int gw_complex_mma_probe(int32_t mode, double ms, double *tflops, void *stream);
+
 const char *gw_strerror(int code);
 int gw_version(void);
 

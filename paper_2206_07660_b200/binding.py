@@ -63,11 +63,12 @@ def lib():
                                  ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(i32), vp]
         L.gw_axpby.argtypes = [sz, dbl, dbl, vp, dbl, dbl, vp, vp]
         L.gw_phi_gw.argtypes = [i32, i32, i32, dbl, vp, vp, vp, vp]
+        L.gw_complex_mma_probe.argtypes = [i32, dbl, ctypes.POINTER(dbl), vp]
         L.gw_strerror.argtypes = [ctypes.c_int]
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version",
-                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw"):
+                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -314,6 +315,13 @@ def gw_launch_count(prob):
 def gw_fp64_peak(ms=200.0, stream=None):
     out = ctypes.c_double(0.0)
     _check(lib().gw_fp64_peak(ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_fp64_peak")
+    return out.value
+
+
+def gw_complex_mma_probe(mode, ms=100.0, stream=None):
+    """Algorithmic TFLOP/s of the main-GEMM inner loop alone: mode 0 = 4M, 1 = 3M with sums in registers, 2 = 3M with pre-summed B."""
+    out = ctypes.c_double(0.0)
+    _check(lib().gw_complex_mma_probe(int(mode), ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_complex_mma_probe")
     return out.value
 
 

@@ -414,6 +414,111 @@ done:
   return rc;
 }
 
+
+// ---- complex tile-product probe: the inner loop of the main GEMMs alone (operands resident in shared memory, 8 warps per CTA, one CTA
+//      per SM), for the three ways of forming a complex 8x8x4 product on DMMA (profiles/r02_3m_vs_4m.md):
+//        mode 0: 4M (four real DMMAs, warp tile 2 x 7);  mode 1: 3M Karatsuba, operand sums by DADD in registers (warp tile 2 x 4);
+//        mode 2: 3M with the B sums pre-formed as a third plane in shared memory
+template <int MODE, int MT, int NJ>
+__global__ void __launch_bounds__(256, 1) cmma_probe_kernel(double *out, int iters) {
+  constexpr int KC = 8, TM = 32, NCG = 8 / (TM / (8 * MT)), NCOLS = 8 * NCG * NJ, NACC = MODE == 0 ? 2 : 3;
+  extern __shared__ __align__(128) unsigned char raw[];
+  c128 *sA = reinterpret_cast<c128 *>(raw), *sB = sA + TM * KC;
+  double *sB3 = reinterpret_cast<double *>(sB + NCOLS * KC);
+  for (int i = threadIdx.x; i < TM * KC; i += blockDim.x) sA[i] = make_double2(1e-3 * (i % 7), -1e-3 * (i % 5));
+  for (int i = threadIdx.x; i < NCOLS * KC; i += blockDim.x) { sB[i] = make_double2(1e-3 * (i % 3), 1e-3 * (i % 11)); sB3[i] = 1e-3; }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3, rho = (g >> 1) + 4 * (g & 1);
+  double acc[MT][NJ][NACC][2];
+#pragma unroll
+  for (int i = 0; i < MT; i++)
+#pragma unroll
+    for (int j = 0; j < NJ; j++)
+#pragma unroll
+      for (int x = 0; x < NACC; x++) acc[i][j][x][0] = acc[i][j][x][1] = 0.0;
+  constexpr int MG = TM / (8 * MT);
+  const c128 *sAw = sA + (8 * (w % MG) * MT + rho) * KC, *sBw = sB + (8 * (w / MG) + rho) * KC;
+  const double *sB3w = sB3 + (8 * (w / MG) + rho) * KC;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int ks = 0; ks < KC / 4; ks++) {
+      const int u = (4 * ks + c) ^ rho;
+      c128 a[MT], b[NJ];
+      double b3[NJ];
+#pragma unroll
+      for (int i = 0; i < MT; i++) a[i] = sAw[i * 8 * KC + u];
+#pragma unroll
+      for (int j = 0; j < NJ; j++) { b[j] = sBw[j * NCG * 8 * KC + u]; if (MODE == 2) b3[j] = sB3w[j * NCG * 8 * KC + u]; }
+      if (MODE == 0) {
+#pragma unroll
+        for (int j = 0; j < NJ; j++)
+#pragma unroll
+          for (int i = 0; i < MT; i++) cmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+      } else {
+        double as[MT];
+#pragma unroll
+        for (int i = 0; i < MT; i++) as[i] = a[i].x + a[i].y;
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+          const double bs = MODE == 1 ? b[j].x + b[j].y : b3[j];
+#pragma unroll
+          for (int i = 0; i < MT; i++) {
+            dmma884(acc[i][j][0][0], acc[i][j][0][1], a[i].x, b[j].x);
+            dmma884(acc[i][j][1][0], acc[i][j][1][1], a[i].y, b[j].y);
+            dmma884(acc[i][j][2][0], acc[i][j][2][1], as[i], bs);
+          }
+        }
+      }
+    }
+    __syncwarp();
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < MT; i++)
+#pragma unroll
+    for (int j = 0; j < NJ; j++)
+#pragma unroll
+      for (int x = 0; x < NACC; x++) s += acc[i][j][x][0] + acc[i][j][x][1];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+template <int MODE, int MT, int NJ>
+static int run_cmma_probe(double ms, double *tflops, cudaStream_t st) {
+  constexpr int NCOLS = 8 * (8 / (32 / (8 * MT))) * NJ;
+  const size_t smem = (size_t)(32 * 8 + NCOLS * 8) * 16 + (size_t)NCOLS * 8 * 8;
+  int rc = 0;
+  const int nsm = gw_sm_count(), iters = 4000;
+  double *out = 0; cudaEvent_t e0 = 0, e1 = 0; float t = 0; int reps = 1;
+  CU(cudaFuncSetAttribute(cmma_probe_kernel<MODE, MT, NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CU(cudaMalloc(&out, sizeof(double) * nsm * 256));
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  cmma_probe_kernel<MODE, MT, NJ><<<nsm, 256, smem, st>>>(out, iters);
+  CU(cudaEventRecord(e0, st));
+  cmma_probe_kernel<MODE, MT, NJ><<<nsm, 256, smem, st>>>(out, iters);
+  CU(cudaEventRecord(e1, st));
+  CU(cudaEventSynchronize(e1));
+  CU(cudaEventElapsedTime(&t, e0, e1));
+  reps = (int)(ms / (t > 0.01f ? t : 0.01f)) + 1;
+  CU(cudaEventRecord(e0, st));
+  for (int r = 0; r < reps; r++) cmma_probe_kernel<MODE, MT, NJ><<<nsm, 256, smem, st>>>(out, iters);
+  CU(cudaEventRecord(e1, st));
+  CU(cudaEventSynchronize(e1));
+  CU(cudaEventElapsedTime(&t, e0, e1));
+  *tflops = 8.0 * 32.0 * NCOLS * 8.0 * iters * nsm * reps / (t * 1e-3) * 1e-12;   // 8 flops per complex multiply-add
+done:
+  cudaFree(out); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1);
+  return rc;
+}
+
+extern "C" int gw_complex_mma_probe(int32_t mode, double ms, double *tflops, void *stream) {
+  if (!tflops || !(ms > 0) || mode < 0 || mode > 2) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (mode == 0) return run_cmma_probe<0, 2, 7>(ms, tflops, st);
+  if (mode == 1) return run_cmma_probe<1, 2, 4>(ms, tflops, st);
+  return run_cmma_probe<2, 2, 4>(ms, tflops, st);
+}
+
 extern "C" const char *gw_strerror(int code) {
   switch (code) {
     case GW_OK: return "ok";
