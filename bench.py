@@ -427,6 +427,7 @@ def run_ours(args):
     #      call, timed with CUDA events (gw_find_mu by wall clock: it synchronises after every N_e evaluation).  Reported beside. ----
     closure = None
     if world == 1 and not args.no_closure:
+      try:
         mesh = run.p.mesh
         H0n, Sn = gwgen.make_h0_s(cfg, mesh, run.p.eps, run.p.U)
         fgn = gwgen.make_fermionic_grids(cfg.ntau, cfg.beta)
@@ -445,10 +446,9 @@ def run_ours(args):
         ev[3].record(st)
         F = gw.gw_axpby(1.0, J, 1.0, gw.gw_axpby(1.0, run.K, 1.0, H0.clone(), st), st)
         ev[4].record(st)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        mu, ne, G_w, n_eval = gw.gw_find_mu(fg["omega"], fg["t_beta"], S, F, Sw, n_target, -1.0, 1.0, 1e-12, cfg.spin_deg, stream=st)
-        mu_ms = (time.perf_counter() - t0) * 1e3
+        # one N_e(mu) evaluation = Eq. 16 for all (n, k) + Eq. 15 (what the chemical-potential search repeats)
+        G_w, _ = gw.gw_dyson_update(fg["omega"], 0.0, S, F, Sw, stream=st)
+        gw.gw_electron_count(fg["t_beta"], S, G_w, cfg.spin_deg, stream=st)
         ev[5].record(st)
         G_new = gw.gw_transform(fg["T_tw_f"], G_w, stream=st)
         ev[6].record(st)
@@ -457,10 +457,21 @@ def run_ours(args):
         torch.cuda.synchronize()
         el = lambda a, b: ev[a].elapsed_time(ev[b])
         closure = {"unit": "ms", "gamma_from_G_beta": el(0, 1), "hartree_J": el(1, 2), "sigma_tau_to_iw": el(2, 3), "fock_assembly": el(3, 4),
-                   "find_mu": mu_ms, "find_mu_evaluations": n_eval, "mu": mu, "n_e_minus_target": ne - n_target,
-                   "g_iw_to_tau": el(5, 6), "damping": el(6, 7),
-                   "total": el(0, 4) + mu_ms + el(5, 7), "fraction_of_sigma_build": (el(0, 4) + mu_ms + el(5, 7)) / ms_per_step}
+                   "one_ne_evaluation_dyson_plus_count": el(4, 5), "g_iw_to_tau": el(5, 6), "damping": el(6, 7)}
+        # the search itself (wall clock: it synchronises after every evaluation).  On these synthetic grids (Chebyshev nodes at beta = 700,
+        # DESIGN.md section 3) the fitted G(beta^-) is not accurate enough for N_e(mu) to bracket every target: a failed search is reported, not fatal.
+        try:
+            t0 = time.perf_counter()
+            mu, ne, G_w, n_eval = gw.gw_find_mu(fg["omega"], fg["t_beta"], S, F, Sw, n_target, -1.0, 1.0, 1e-12, cfg.spin_deg, stream=st)
+            closure.update({"find_mu": (time.perf_counter() - t0) * 1e3, "find_mu_evaluations": n_eval, "mu": mu, "n_e_minus_target": ne - n_target})
+        except gw.GWError as e:
+            closure["find_mu"] = {"error": str(e)[:200]}
+        fixed = el(0, 4) + el(5, 7)
+        closure["total_with_45_evaluations"] = fixed + 45 * el(4, 5)
+        closure["fraction_of_sigma_build"] = closure["total_with_45_evaluations"] / ms_per_step
         del H0, S, fg, Gb, gam, J, Sw, F, G_w, G_new
+      except Exception as e:          # never fatal for the headline
+        closure = {"error": str(e)[:300]}
 
     # ---- e2e: the same iteration through the C ABI with HOST buffers (copies inside the timed region) ----
     e2e = None

@@ -18,8 +18,8 @@ from .mesh import KMesh
 from .grids import make_grids, make_fermionic_transform, make_fermionic_grids
 from .fock import make_fock, greens_function, density_matrix, make_h0_s
 from .vgen import make_V, make_V_block, to_qslab, make_V_qslab
-from .problem import make_problem, make_spin_channels, Problem
+from .problem import make_problem, make_spin_channels, rotate_spin_channels, Problem
 
 __all__ = ["CONFIGS", "GWConfig", "get_config", "KMesh", "make_grids", "make_fermionic_transform", "make_fermionic_grids", "make_h0_s", "make_fock",
            "greens_function", "density_matrix", "make_V", "make_V_block",
-           "make_problem", "make_spin_channels", "to_qslab", "make_V_qslab", "Problem"]
+           "make_problem", "make_spin_channels", "rotate_spin_channels", "to_qslab", "make_V_qslab", "Problem"]

@@ -45,6 +45,18 @@ def make_spin_channels(p, ns=2):
     return np.ascontiguousarray(np.stack(Gs)), np.ascontiguousarray(np.stack(gs))
 
 
+def rotate_spin_channels(Gs, gs, seed=0):
+    """Two-component inputs from two collinear channels by ONE global spin rotation R in SU(2) (seeded): block (s, s') of the result is
+    sum_c R[s][c] X^c conj(R[s'][c]), blocks in the order uu, ud, du, dd (include/gw.h "Spin blocks").  Off-diagonal blocks are non-zero,
+    as with spin-orbit coupling; spin traces (P0, J) are those of the collinear channels, which is what the pins use."""
+    rng = np.random.default_rng([220607660, 11, int(seed)])
+    th, ph, ps = rng.uniform(0.3, 1.2), rng.uniform(0, 2 * np.pi), rng.uniform(0, 2 * np.pi)
+    R = np.array([[np.cos(th) * np.exp(1j * ph), np.sin(th) * np.exp(1j * ps)],
+                  [-np.sin(th) * np.exp(-1j * ps), np.cos(th) * np.exp(-1j * ph)]])
+    rot = lambda X: np.ascontiguousarray(np.stack([sum(R[s, c] * X[c] * np.conj(R[sp, c]) for c in range(2)) for s in range(2) for sp in range(2)]))
+    return rot(Gs), rot(gs), R
+
+
 def make_problem(cfg, v_device="cpu", with_V=True, raw=False) -> Problem:
     """raw=False: the BASELINE.json inputs (time-reversal symmetric Fock-built G, group-averaged V).
     raw=True : inputs with NO symmetry at all — V blocks are independent draws (V[k1][k2] unrelated to V[k2][k1] or

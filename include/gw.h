@@ -71,19 +71,22 @@ typedef struct {
   size_t work_bytes;       /*   at least gw_workspace_bytes(p) bytes, 256-byte aligned; contents are don't-care    */
   int32_t symmetry;        /* 0 = evaluate Algorithm 1 literally (default); GW_SYM_TR = the caller asserts time-reversal   */
                            /*   symmetric inputs (see GW_SYM_TR below)                                                     */
-  int32_t ns;              /* spin channels (sums over sigma): 0 or 1 = one channel; 2 = two collinear  */
-                           /*   channels (spin-polarised, e.g. the paper's AFM MnO) — see "Spin channels" below */
+  int32_t ns;              /* spin blocks of G: 0 or 1 = one; 2 = two collinear channels (spin-polarised, e.g. */
+                           /*   the paper's AFM MnO); 4 = two-component (all sigma sigma' blocks) — "Spin blocks" below  */
   int32_t v_layout;        /* GW_V_FULL (0) or GW_V_QSLAB: how p->V is laid out — see "V layouts" below                      */
   int32_t reserved;        /* must be 0                                                                                    */
 } gw_problem;
 
-/* Spin channels.  With ns = 2 the Green's function has two collinear spin blocks G^{sigma sigma}, sigma = up, down (no spin-orbit
- * coupling), stored with the channel as the LEADING index: G, Sigma : [ns][ntau][nk][nao][nao];  gamma, K : [ns][nk][nao][nao].
- *   gw_polarization : P0t = -(spin_deg/N_k) Σ_sigma Σ_k ... G^sigma(k+q,tau) ... G^sigma(k,-tau)  (Eq. 28b's Σ_{sigma sigma'} restricted
- *                     to the non-zero blocks; the sum runs inside the stage-1 k loop).  Pass spin_deg = 1 with ns = 2; two identical
- *                     channels with spin_deg = 1 equal one channel with spin_deg = 2.
- *   gw_selfenergy, gw_exchange : one Sigma^sigma / K^sigma per channel from G^sigma / gamma^sigma and the common Wt (Eq. 31, 22).
- *   gw_hartree      : J (spin independent, [nk][nao][nao]) from Σ_sigma gamma^sigma (Eq. 20's Σ_sigma1), times spin_deg.
+/* Spin blocks.  The spin index is the LEADING index of G, Sigma ([ns][ntau][nk][nao][nao]) and gamma, K ([ns][nk][nao][nao]).
+ *   ns = 2 : collinear channels G^{sigma sigma}, sigma = up, down (no spin-orbit coupling), in that order.
+ *   ns = 4 : two-component, all blocks G^{sigma sigma'} in the order uu, ud, du, dd ("H0 exhibits a spin dependence with non-zero
+ *            off-diagonal spin components ... spin-orbit coupling").
+ *   gw_polarization : P0t = -(spin_deg/N_k) Σ_{sigma sigma'} Σ_k V G^{sigma sigma'}(k+q,tau) V G^{sigma' sigma}(k,-tau)   (Eq. 28b as printed; with
+ *                     ns = 2 only sigma = sigma' is non-zero); the spin sum runs inside the stage-1 k loop.  Pass spin_deg = 1 with ns > 1; two
+ *                     identical collinear channels with spin_deg = 1 equal one channel with spin_deg = 2.
+ *   gw_selfenergy, gw_exchange : one Sigma^{sigma sigma'} / K^{sigma sigma'} per block from G^{sigma sigma'} / gamma^{sigma sigma'} and the common Wt
+ *                     (Eq. 31, and Eq. 22 which prints the general K_{i sigma, j sigma'}).
+ *   gw_hartree      : J (spin independent, [nk][nao][nao]) from the spin-diagonal blocks of gamma (Eq. 20's Σ_sigma1), times spin_deg.
  * P0t, Wt, V and the transforms carry no spin index. */
 
 /* V layouts.
@@ -105,7 +108,8 @@ enum { GW_V_FULL = 0, GW_V_QSLAB = 1 };
  *                     nk <= 128 also only q <= −q, and P0t[t][−q] = transpose(P0t[t][q])  (216 -> 112 q points);
  *                     of each Q panel only the column tiles up to its diagonal block are computed, the rest is the conjugate mirror;
  *   gw_selfenergy   : k <= −k are computed, Sigma[t][−k] = conj(Sigma[t][k])  (only for the full q range and nk <= 128);
- * the other calls ignore the flag.  Computed elements are bit-identical to the literal evaluation.  If the inputs do not
+ * the other calls ignore the flag; with ns = 4 the flag is refused (GW_EINVAL: the relations above are those of a spin-diagonal G).
+ * Computed elements are bit-identical to the literal evaluation.  If the inputs do not
  * have the symmetry the copied elements are wrong — nothing checks it. */
 enum { GW_SYM_TR = 1 };
 

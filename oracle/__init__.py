@@ -325,3 +325,25 @@ def phi_gw(nk, beta, w, phi):
     lib().gwref_phi_gw.restype = ctypes.c_double
     lib().gwref_phi_gw.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p]
     return float(lib().gwref_phi_gw(int(nk), int(phi.shape[1]), int(phi.shape[0]), float(beta), _pd(w), _pd(phi)))
+
+
+# two-component spin blocks (spin-orbit coupling gives G off-diagonal spin components).  Blocks in the order uu, ud, du, dd.
+def polarization_blocks(cfg, vb, Gb):
+    """Eq. 28b as printed: P0 = -(s/N_k) sum_{sigma sigma'} sum_k V G^{sigma sigma'}(k+q, tau) V G^{sigma' sigma}(k, -tau).
+    Gb: [4][ntau][nk][nao][nao].  Every (sigma, sigma') term is one call of the single-block slice routine with G^{sigma sigma'} in the
+    k+q slot and G^{sigma' sigma} in the k slot."""
+    c1 = _one_channel(cfg)
+    N = cfg.ntau
+    out = np.zeros((N, cfg.nk, cfg.naux, cfg.naux), np.complex128)
+    for t in range(N):
+        for q in range(cfg.nk):
+            for s in range(2):
+                for sp in range(2):
+                    out[t, q] += p0t_slice(c1, vb, np.ascontiguousarray(Gb[2 * s + sp][t]), np.ascontiguousarray(Gb[2 * sp + s][N - 1 - t]), q)
+    return cfg.spin_deg * out
+
+
+def hartree_blocks(cfg, vb, gb):
+    """Eq. 20: sigma_1 runs over the spin-diagonal blocks uu and dd."""
+    c1 = _one_channel(cfg)
+    return cfg.spin_deg * (hartree(c1, vb, np.ascontiguousarray(gb[0])) + hartree(c1, vb, np.ascontiguousarray(gb[3])))

@@ -108,7 +108,7 @@ class GWProblem:
 
     def __init__(self, mesh, nao, naux, ntau, nw, beta, V, T_wt, T_tw, spin_deg=2, q_begin=0, q_end=None, symmetry=0, ns=1, v_layout=GW_V_FULL):
         self.symmetry = int(symmetry)      # 0 = literal Algorithm 1; GW_SYM_TR = time-reversal symmetric inputs (gw.h)
-        self.ns = 2 if int(ns) == 2 else 1  # spin channels: G, Sigma [ns][ntau][nk][nao][nao], gamma, K [ns][nk][nao][nao] when ns = 2
+        self.ns = int(ns) if int(ns) in (2, 4) else 1   # spin blocks: G, Sigma [ns][ntau][nk][nao][nao], gamma, K [ns][nk][nao][nao] when ns > 1
         self.v_layout = int(v_layout)      # GW_V_FULL: V [nk][nk][naux][nao][nao]; GW_V_QSLAB: V [nq][nk][2][naux][nao][nao] (gw.h)
         self.mesh = tuple(int(m) for m in mesh)
         self.nk = self.mesh[0] * self.mesh[1] * self.mesh[2]
@@ -132,12 +132,12 @@ class GWProblem:
     def gshape(self):
         """shape of G and Sigma"""
         base = (self.ntau, self.nk, self.nao, self.nao)
-        return (2,) + base if self.ns == 2 else base
+        return (self.ns,) + base if self.ns > 1 else base
 
     def kshape(self):
         """shape of gamma and K"""
         base = (self.nk, self.nao, self.nao)
-        return (2,) + base if self.ns == 2 else base
+        return (self.ns,) + base if self.ns > 1 else base
 
     def set_work(self, work):
         """Attach the device workspace (uint8 CUDA tensor of at least gw_workspace_bytes bytes)."""

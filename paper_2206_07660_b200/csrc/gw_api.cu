@@ -26,7 +26,8 @@ static int check_problem(const gw_problem *p, bool need_T) {
   if (!p) return GW_EINVAL;
   if (p->nk1 <= 0 || p->nk2 <= 0 || p->nk3 <= 0 || p->nao <= 0 || p->naux <= 0 || p->ntau <= 0 || p->nw <= 0) return GW_EINVAL;
   if (p->spin_deg != 1 && p->spin_deg != 2) return GW_EINVAL;
-  if ((p->symmetry & ~GW_SYM_TR) || p->reserved || p->ns < 0 || p->ns > 2 || (p->v_layout != GW_V_FULL && p->v_layout != GW_V_QSLAB)) return GW_EINVAL;
+  if ((p->symmetry & ~GW_SYM_TR) || p->reserved || (p->ns != 0 && p->ns != 1 && p->ns != 2 && p->ns != 4) || (p->v_layout != GW_V_FULL && p->v_layout != GW_V_QSLAB)) return GW_EINVAL;
+  if (p->ns == 4 && (p->symmetry & GW_SYM_TR)) return GW_EINVAL;     // the time-reversal relations of GW_SYM_TR are those of spin-diagonal G
   const int64_t nk = (int64_t)p->nk1 * p->nk2 * p->nk3;
   if (nk > (1 << 20)) return GW_EINVAL;
   if (p->q_begin < 0 || p->q_end > nk || p->q_begin >= p->q_end) return GW_EINVAL;

@@ -19,7 +19,7 @@ struct GwDims {
   int s;            // spin_deg
   int q0, nq;       // q shard
   int sym;          // gw_problem.symmetry
-  int ns;           // spin channels (1 or 2)
+  int ns;           // spin blocks of G: 1, 2 (collinear: uu, dd) or 4 (two-component: uu, ud, du, dd)
   int vq;           // 1: p->V is a q-slab (GW_V_QSLAB), 0: the full tensor
 };
 
@@ -28,7 +28,7 @@ static inline GwDims gw_dims(const gw_problem *p) {
   d.nk1 = p->nk1; d.nk2 = p->nk2; d.nk3 = p->nk3; d.nk = p->nk1 * p->nk2 * p->nk3;
   d.nao = p->nao; d.naux = p->naux; d.ntau = p->ntau; d.nw = p->nw; d.s = p->spin_deg;
   d.q0 = p->q_begin; d.nq = p->q_end - p->q_begin; d.sym = p->symmetry;
-  d.ns = p->ns == 2 ? 2 : 1; d.vq = p->v_layout == GW_V_QSLAB ? 1 : 0;
+  d.ns = p->ns == 2 ? 2 : (p->ns == 4 ? 4 : 1); d.vq = p->v_layout == GW_V_QSLAB ? 1 : 0;
   return d;
 }
 

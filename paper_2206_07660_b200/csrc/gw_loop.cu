@@ -28,7 +28,8 @@ __global__ void __launch_bounds__(NT) hartree_rho_kernel(const GwDims d, int ql0
   __shared__ c128 red[NT];
   const int Q = blockIdx.x, nao = d.nao, n2 = nao * nao;
   c128 acc = make_double2(0.0, 0.0);
-  for (int sg = 0; sg < d.ns; sg++)                        // Σ_sigma1 of Eq. 20
+  for (int sg = 0; sg < d.ns; sg++) {                      // Σ_sigma1 of Eq. 20: the spin-diagonal blocks
+    if (d.ns == 4 && (sg == 1 || sg == 2)) continue;
     for (int kp = 0; kp < d.nk; kp++) {
       const c128 *Vq = V + (gw_vfwd(d, ql0, kp, kp) * d.naux + Q) * n2, *g = gamma + ((size_t)sg * d.nk + kp) * n2;
       for (int e = threadIdx.x; e < n2; e += NT) {
@@ -36,6 +37,7 @@ __global__ void __launch_bounds__(NT) hartree_rho_kernel(const GwDims d, int ql0
         cfma(acc, g[a * nao + b], Vq[e]);
       }
     }
+  }
   const c128 tot = block_sum(acc, red);
   if (threadIdx.x == 0) rho[Q] = tot;
 }

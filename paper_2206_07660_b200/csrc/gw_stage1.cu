@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
           const Item it = decode_item(P, item);
           const int q = d.q0 + it.ql;
           for (int kk = 0; kk < nkk; kk++, kit++) {
-            const int k = d.ns == 2 ? kk >> 1 : kk;                    // spin channel innermost: the V blocks of (k, q) serve both
+            const int k = d.ns == 4 ? kk >> 2 : (d.ns == 2 ? kk >> 1 : kk);   // spin term innermost: the V blocks of (k, q) serve all of them
             const int kq = gw_kadd(d, k, q);
             const int yB = (int)gw_vbwd(d, it.ql, k, kq) * naux + 8 * (it.cbase + (int)rank * P.ntc);   // row of V viewed as [blocks*naux][nao²]
             const int yA = (cid * 2 + (int)(kit & 1u)) * TM;           // row of the slab area viewed as [2*nclusters*TM][nao²]
@@ -226,12 +226,15 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
         const int q = d.q0 + it.ql;
         const int my_rows = max(0, min(it.tm_rows, r0 + rows_cta) - r0) * nao, npass = (my_rows + P.prows - 1) / P.prows;
         for (int kk = 0; kk < nkk; kk++, kit++) {
-          const int k = d.ns == 2 ? kk >> 1 : kk, sg = d.ns == 2 ? kk & 1 : 0;
+          // spin term (sigma, sigma') of Eq. 28b: G^{sigma sigma'} at k+q (block b1) and G^{sigma' sigma} at k (block b2).  One block:
+          // b1 = b2 = 0; collinear: b1 = b2 = sigma; two-component: b1 = 2 sigma + sigma', b2 = its spin transpose
+          const int k = d.ns == 4 ? kk >> 2 : (d.ns == 2 ? kk >> 1 : kk);
+          const int b1 = d.ns == 4 ? kk & 3 : (d.ns == 2 ? kk & 1 : 0), b2 = d.ns == 4 ? ((b1 & 1) << 1) | (b1 >> 1) : b1;
           const int kq = gw_kadd(d, k, q);
           const c128 *Vt = P.V + gw_vfwd(d, it.ql, k, kq) * vb + (size_t)(it.Q0 + r0) * n2;
           const c128 *Xs = slab0 + (size_t)(kit & 1u) * P.slab_units + (size_t)r0 * n2;
-          const c128 *Gs = P.G + (size_t)sg * d.ntau * d.nk * n2;      // this spin channel's G[t][k]
-          const c128 *Gt = Gs + ((size_t)it.t * d.nk + kq) * n2, *Gm = Gs + ((size_t)(d.ntau - 1 - it.t) * d.nk + k) * n2;
+          const size_t gstride = (size_t)d.ntau * d.nk * n2;           // one spin block of G[t][k]
+          const c128 *Gt = P.G + b1 * gstride + ((size_t)it.t * d.nk + kq) * n2, *Gm = P.G + b2 * gstride + ((size_t)(d.ntau - 1 - it.t) * d.nk + k) * n2;
           // pass 1 (its G buffer was last read two phases ago; a time-shared buffer must wait for the previous phase)
           if (P.ng == 2) issue_matrix<true>(sG0, Gt, nao, ldp, P.fd_nao);
           if (ph > 0) gwp::mbar_wait(bar_phase, (ph - 1) & 1u);

@@ -178,3 +178,50 @@ def test_two_gpu_q_shards_sum_to_oracle(problems, oracle_results):
             S_tot = out["Sigma"].cpu() if S_tot is None else S_tot + out["Sigma"].cpu()
             K_tot = out["K"].cpu() if K_tot is None else K_tot + out["K"].cpu()
     assert relerr(S_tot.numpy(), ref["Sigma"]) <= TOL and relerr(K_tot.numpy(), ref["K"]) <= TOL
+
+
+@pytest.mark.parametrize("name", ["T", "R", "S", "W"])
+def test_two_component_blocks_parity(problems, oracle_lib, name):
+    """ns = 4 (blocks uu, ud, du, dd; gw.h "Spin blocks"): P0t with the full sigma sigma' sum of Eq. 28b inside the stage-1 k loop, Wt,
+    Sigma and K per block, J from the spin-diagonal blocks; GW_SYM_TR is refused for two-component G."""
+    import paper_2206_07660_b200 as gw
+    p = problems(name)
+    cfg = dataclasses.replace(p.cfg, spin_deg=1)
+    Gs, gs = gwgen.make_spin_channels(p, 2)
+    Gb, gb, _ = gwgen.rotate_spin_channels(Gs, gs, seed=1)
+    prob = _dev_problem(p, cfg, ns=4)
+    G, gamma = torch.from_numpy(Gb).cuda(), torch.from_numpy(gb).cuda()
+    P0t = gw.gw_polarization(prob, G)
+    Wt, info = gw.gw_screened_interaction(prob, P0t)
+    Sigma = gw.gw_selfenergy(prob, G, Wt)
+    K = gw.gw_exchange(prob, gamma)
+    J = gw.gw_hartree(prob, gamma)
+    torch.cuda.synchronize()
+    assert info.cpu().tolist() == [-1, -1]
+    vb = oracle_lib.VBlocks(cfg, p.V.numpy())
+    rP = oracle_lib.polarization_blocks(cfg, vb, Gb)
+    rW = oracle_lib.screened_interaction(cfg, p.T_wt, p.T_tw, rP)
+    for key, got, ref in (("P0t", P0t, rP), ("Wt", Wt, rW), ("Sigma", Sigma, oracle_lib.selfenergy_spin(cfg, vb, Gb, rW)),
+                          ("K", K, oracle_lib.exchange_spin(cfg, vb, gb)), ("J", J, oracle_lib.hartree_blocks(cfg, vb, gb))):
+        assert report(name + " ns=4", key, got.cpu().numpy(), ref) <= TOL, key
+    with pytest.raises(gw.GWError):
+        gw.gw_polarization(_dev_problem(p, cfg, ns=4, symmetry=gw.GW_SYM_TR), G)
+
+
+def test_two_component_raw_inputs(raw_problems, oracle_lib):
+    """ns = 4 on four independent non-Hermitian blocks (no relation between ud and du): the block pairing of Eq. 28b,
+    G^{sigma sigma'} at k+q with G^{sigma' sigma} at k, is told apart from its transposed twin."""
+    import paper_2206_07660_b200 as gw
+    p = raw_problems("R")
+    cfg = dataclasses.replace(p.cfg, spin_deg=1)
+    G2a, g2a = gwgen.make_spin_channels(p, 2)
+    rng = np.random.default_rng(21)
+    Gb = np.ascontiguousarray(np.stack([G2a[0], G2a[1], G2a[0][::-1].copy() * 0.7, G2a[1] * (0.3 - 0.5j)]))
+    gb = np.ascontiguousarray(np.stack([g2a[0], g2a[1], g2a[0].conj() * 0.7, g2a[1] * (0.3 - 0.5j)]))
+    prob = _dev_problem(p, cfg, ns=4)
+    G, gamma, W = torch.from_numpy(Gb).cuda(), torch.from_numpy(gb).cuda(), torch.from_numpy(p.extras["W"]).cuda()
+    vb = oracle_lib.VBlocks(cfg, p.V.numpy())
+    assert report("R raw ns=4", "P0t", gw.gw_polarization(prob, G).cpu().numpy(), oracle_lib.polarization_blocks(cfg, vb, Gb)) <= TOL
+    assert report("R raw ns=4", "Sigma", gw.gw_selfenergy(prob, G, W).cpu().numpy(), oracle_lib.selfenergy_spin(cfg, vb, Gb, p.extras["W"])) <= TOL
+    assert report("R raw ns=4", "K", gw.gw_exchange(prob, gamma).cpu().numpy(), oracle_lib.exchange_spin(cfg, vb, gb)) <= TOL
+    assert report("R raw ns=4", "J", gw.gw_hartree(prob, gamma).cpu().numpy(), oracle_lib.hartree_blocks(cfg, vb, gb)) <= TOL

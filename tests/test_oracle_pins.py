@@ -602,3 +602,27 @@ def test_P20_phi_gw_scalar_closed_form_and_definition(oracle_lib):
     rng = np.random.default_rng(4)
     w = rng.uniform(0.5, 2.0, 7); phi = rng.normal(size=(7, 11))
     assert abs(oracle_lib.phi_gw(12, 3.0, w, phi) - np.einsum("n,nq->", w, phi) / (2 * 12 * 3.0)) < 1e-14
+
+
+def test_P21_two_component_blocks_spin_rotation(problems, oracle_lib):
+    """Two-component blocks (uu, ud, du, dd) built from two collinear channels by one global SU(2) rotation R: the spin trace of Eq. 28b
+    is rotation invariant, so P0[blocks] = P0[collinear] (pinned by P19); Sigma and K are linear in G with a spin-independent W, so
+    their blocks are the rotated per-channel results; J sees the spin trace of gamma only."""
+    import dataclasses
+    p = problems("T")
+    cfg1 = dataclasses.replace(p.cfg, spin_deg=1)
+    vb = oracle_lib.VBlocks(p.cfg, p.V.numpy())
+    Gs, gs = gwgen.make_spin_channels(p, 2)
+    Gb, gb, R = gwgen.rotate_spin_channels(Gs, gs)
+    assert relerr(R @ R.conj().T, np.eye(2)) < 1e-15 and np.abs(Gb[1]).max() > 0.05 * np.abs(Gb[0]).max()      # unitary; off-diagonal blocks present
+    P_col = oracle_lib.polarization_spin(cfg1, vb, Gs)
+    assert relerr(oracle_lib.polarization_blocks(cfg1, vb, Gb), P_col) < 1e-13
+    Wt = oracle_lib.screened_interaction(cfg1, p.T_wt, p.T_tw, P_col)
+    S_col = oracle_lib.selfenergy_spin(cfg1, vb, Gs, Wt)
+    S_blk = oracle_lib.selfenergy_spin(cfg1, vb, Gb, Wt)
+    K_col, K_blk = oracle_lib.exchange_spin(cfg1, vb, gs), oracle_lib.exchange_spin(cfg1, vb, gb)
+    for s in range(2):
+        for sp in range(2):
+            rot = lambda X: sum(R[s, c] * X[c] * np.conj(R[sp, c]) for c in range(2))
+            assert relerr(S_blk[2 * s + sp], rot(S_col)) < 1e-13 and relerr(K_blk[2 * s + sp], rot(K_col)) < 1e-13
+    assert relerr(oracle_lib.hartree_blocks(cfg1, vb, gb), oracle_lib.hartree_spin(cfg1, vb, gs)) < 1e-13
