@@ -51,6 +51,7 @@ enum {
                          nw > ntau (stage 2 keeps the frequency-domain intermediate in the first nw slices of the Wt buffer);
                          naux > 896 (stage 1: panel columns = 2 CTAs x 2 column passes x 224; the paper's N_aux/N_orb = 3-10,
                          PAPER.md:96, gives naux <= 640 at nao = 64) */
+  GW_ENOBRACKET = -6, /* gw_find_mu only: N_e(mu) did not bracket the target after 60 widenings of [mu_lo, mu_hi] */
   GW_ENOTPD = -5    /* gw_sigma_iteration_host only: a Cholesky factorisation of I - P0(q, iOmega_n) met a non-positive pivot
                        (the device calls report that through `info` instead); Sigma / Wt are then not meaningful */
 };
@@ -210,7 +211,7 @@ int gw_electron_count(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, co
  * until its width <= mu_tol (<= 200 times), return the midpoint and N_e there; G_w then holds G(i omega_n) at that mu.
  * Every N_e evaluation is one gw_dyson_update + gw_electron_count on `stream`; this call SYNCHRONISES the stream after each
  * (it reads N_e back), unlike the calls above.  mu_out, ne_out, n_eval (optional) are HOST pointers.
- * Returns GW_OK, GW_ENOTPD if a matrix was singular, GW_EINVAL also when no bracket was found. */
+ * Returns GW_OK, GW_ENOTPD if a matrix was singular, GW_ENOBRACKET when no bracket was found. */
 int gw_find_mu(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg, const double *omega, const gw_c128 *t_beta, const gw_c128 *S,
                const gw_c128 *F, const gw_c128 *Sigma_w, double n_target, double mu_lo, double mu_hi, double mu_tol, gw_c128 *G_w,
                gw_c128 *partial, double *ne_dev, double *mu_out, double *ne_out, int32_t *n_eval, void *stream);

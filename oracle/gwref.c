@@ -43,7 +43,9 @@
  * literal 4-index evaluation P10, scalar form / series / eigenvalue route of the Eq. 37 summand P11, fermionic
  * transform of a single pole P12; loop closure: non-interacting closed form of Eq. 16 in the generalised eigenbasis P13,
  * Fermi-function electron count and root of the chemical-potential search P14, literal einsum of Eq. 20 P15,
- * back transform of a single pole P16).
+ * back transform of a single pole P16, non-interacting limit of a whole iteration P17, weighted Matsubara sum of Eq. 37 P20).
+ * Spin (oracle/__init__.py writes the sigma sums out over these single-block routines): identical channels = closed shell P18, Lindhard per
+ * channel P19, two-component blocks under a global spin rotation P21.
  * Nothing here is "parity unpinned".
  */
 #include <complex.h>

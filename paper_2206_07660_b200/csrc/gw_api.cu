@@ -307,7 +307,7 @@ extern "C" int gw_find_mu(int32_t nk, int32_t nao, int32_t nwf, int32_t spin_deg
       else { hi += w; if ((rc = NE(hi, &nhi))) goto done; }
       it++;
     }
-    if (nlo > n_target || nhi < n_target) { rc = GW_EINVAL; goto done; }
+    if (nlo > n_target || nhi < n_target) { rc = GW_ENOBRACKET; goto done; }
     for (it = 0; it < 200 && hi - lo > mu_tol; it++) {
       const double mid = 0.5 * (lo + hi);
       if ((rc = NE(mid, &nmid))) goto done;
@@ -527,6 +527,7 @@ extern "C" const char *gw_strerror(int code) {
     case GW_ENOMEM: return "workspace too small";
     case GW_EARCH: return "current device is not sm_100 (B200)";
     case GW_ESHAPE: return "size not supported by the kernels (nao > 64, ntau or nw > 200, nw > ntau, naux > 896)";
+    case GW_ENOBRACKET: return "chemical-potential search: N_e(mu) does not bracket the target";
     case GW_ENOTPD: return "I - P0(q, iOmega) is not positive definite (non-positive Cholesky pivot in stage 2)";
     default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown error";
   }

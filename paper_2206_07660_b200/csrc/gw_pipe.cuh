@@ -74,6 +74,14 @@ __device__ __forceinline__ void pass_compute(const c128 *sStage, const c128 *sG,
   }
 }
 
+// the last n-tile of a pass GEMM is done with plain FMAs when it holds at most two valid columns
+__host__ __device__ __forceinline__ bool pass_tail_fma(int nao, int ndt) { return ndt >= 2 && nao - 8 * (ndt - 1) <= 2; }
+// executed flops of one 8-row m-tile of a pass GEMM (ndt n-tiles, ksp k-steps): DMMA tiles (4 x 512 flops per k-step) plus the FMA tail
+static inline double pass_mtile_flops(int nao, int ndt, int ksp, bool exact_path) {
+  if (exact_path && pass_tail_fma(nao, ndt)) return (double)(ndt - 1) * ksp * 2048.0 + 8.0 * (nao - 8 * (ndt - 1)) * 4.0 * ksp * 8.0;
+  return (double)ndt * ksp * 2048.0;
+}
+
 // pass_compute for ksp == KSP known at compile time (the production shapes: nao = 26 -> 7, nao = 52 -> 13): no branch between
 // the DMMAs of an n-tile, every B fragment loaded PF k-steps (4*PF DMMAs) before its use.  Same sums in the same order as
 // pass_compute.
@@ -107,12 +115,16 @@ __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const 
   }
   ostride = TRANSPOSED ? nao : 1;
   const c128 *bp = sG + g * ldp + c;
+  // A last n-tile with only one or two valid columns (nao = 25, 26: two of eight) is not worth four DMMAs per k-step: those columns
+  // are formed with plain FP64 FMAs from the same A fragments, each lane summing its own k's, the four lanes of a row then adding up
+  const bool tail_fma = pass_tail_fma(nao, NDT);
+  const int ndt_run = tail_fma ? NDT - 1 : NDT;
   double cr[MT][2], ci[MT][2];
   {
     // a real loop over the n-tiles (bounded register pressure); B fragments (and, for long K, A fragments) are streamed
     // PF k-steps ahead
 #pragma unroll 1
-    for (int nt = 0; nt < NDT; nt++) {
+    for (int nt = 0; nt < ndt_run; nt++) {
       const c128 *bq = bp + nt * 8 * ldp;
       c128 b[NB];
 #pragma unroll
@@ -143,6 +155,34 @@ __device__ __forceinline__ void pass_compute_exact_mt(const c128 *sStage, const 
         if (rok[i] && c0) o[i][0] = make_double2(cr[i][0], ci[i][0]);
         if (rok[i] && c1) o[i][ostride] = make_double2(cr[i][1], ci[i][1]);
         o[i] += 8 * ostride;
+      }
+    }
+    if (tail_fma) {
+      const int n0 = 8 * (NDT - 1);
+      const c128 *g0 = sG + n0 * ldp + c;                 // rows n0, n0 + 1 of the [n][k] matrix, this lane's k = 4 ks + c
+      c128 t0[MT], t1[MT];
+#pragma unroll
+      for (int i = 0; i < MT; i++) { t0[i] = make_double2(0.0, 0.0); t1[i] = make_double2(0.0, 0.0); }
+#pragma unroll
+      for (int ks = 0; ks < KSP; ks++) {
+        const c128 b0 = g0[4 * ks], b1 = g0[ldp + 4 * ks];
+#pragma unroll
+        for (int i = 0; i < MT; i++) {
+          const c128 av = CACHE_A ? a[i][CACHE_A ? ks : 0] : ap[i][4 * ks];
+          cfma(t0[i], av, b0);
+          cfma(t1[i], av, b1);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < MT; i++) {
+#pragma unroll
+        for (int off = 1; off <= 2; off <<= 1) {
+          t0[i].x += __shfl_xor_sync(0xffffffffu, t0[i].x, off); t0[i].y += __shfl_xor_sync(0xffffffffu, t0[i].y, off);
+          t1[i].x += __shfl_xor_sync(0xffffffffu, t1[i].x, off); t1[i].y += __shfl_xor_sync(0xffffffffu, t1[i].y, off);
+        }
+        // o[i] points at column n0 + 2c of this lane's row: lane c = 0 stores column n0, lane c = 1 column n0 + 1
+        if (rok[i] && c == 0) o[i][0] = t0[i];
+        if (rok[i] && c == 1 && n0 + 1 < nao) o[i][-ostride] = t1[i];
       }
     }
   }

@@ -498,7 +498,7 @@ double gw_stage1_flops(const gw_problem *p) {
       if (rows < 0) rows = 0;
       mt_pass += (rows * d.nao + 7) / 8;
     }
-    const double pass = 2.0 * mt_pass * pl.ndt * pl.ksp * pl.ncp * 2048.0;
+    const double pass = 2.0 * mt_pass * pl.ncp * gwp::pass_mtile_flops(d.nao, pl.ndt, pl.ksp, pl.ksp == pl.ksp_max);
     const int mtc = (tm_rows + 7) / 8;
     // main: warps whose first m-tile is valid execute MT_W m-tiles x their n-tiles x 2 k-steps per job
     const double mtiles = mtc <= 2 ? (double)mtc : (double)((mtc + s1::MT_W - 1) / s1::MT_W) * s1::MT_W;   // ragged panel: narrow ownership

@@ -337,7 +337,7 @@ static double s3_generic_flops(const gw_problem *p) {
     const int mtc = (tm_rows + 7) / 8;
     const double mtiles = (mtc <= 2) ? (((d.nao + 3) / 4 == 7) ? (double)mtc : 2.0) /* ragged panel shared by all warps; s3 always runs 2 m-tiles */ : (double)((mtc + s3::MT_W - 1) / s3::MT_W) * s3::MT_W;
     tiles += mtiles * pl.nnt * (s3::KC / 4) * nmain;                         // main
-    tiles += (double)((tm_rows * d.nao + 7) / 8) * pl.ndt * pl.ksp;           // pass A
+    tiles += (double)((tm_rows * d.nao + 7) / 8) * gwp::pass_mtile_flops(d.nao, pl.ndt, pl.ksp, pl.ksp == pl.ksp_max) / 2048.0;   // pass A
     tiles += (double)tm_rows * pl.ndt * pl.ndt * pl.kspf * pl.kh;             // final
   }
   short tmp[128];
@@ -848,7 +848,7 @@ static double flops(const gw_problem *p, const Plan &pl) {
     const int mtc = (tm_rows + 7) / 8;
     const double mtiles = (mtc <= 2) ? (double)mtc : (double)((mtc + MT_W - 1) / MT_W) * MT_W;
     fl += mtiles * pl.nnt * (KC / 4) * nmain * 1536.0;                          // main (3M)
-    fl += (double)((tm_rows * d.nao + 7) / 8) * ndt * pl.ksp * 2048.0;           // pass A
+    fl += (double)((tm_rows * d.nao + 7) / 8) * gwp::pass_mtile_flops(d.nao, ndt, pl.ksp, true);   // pass A
     fl += (double)tm_rows * ndt * ndt * pl.ksp * 2048.0;                         // final
   }
   short tmp[128];
