@@ -233,7 +233,8 @@ def traffic_from_ncu(csv_path, cfg_name, scale_to=None):
     except Exception:
         allrec = {}
     out["kernel_revision"] = kernel_revision()
-    out["source"] = os.path.basename(csv_path)
+    ap_ = os.path.abspath(csv_path)
+    out["source"] = os.path.relpath(ap_, ROOT) if ap_.startswith(ROOT + os.sep) else os.path.basename(csv_path)
     allrec[cfg_name] = out
     if scale_to:
         import gwgen

@@ -138,3 +138,13 @@ def test_phi_gw_parity(problems, oracle_lib):
     _, P0w, _ = oracle_lib.screened_interaction(cfg, p.T_wt, p.T_tw, P0, want_freq=True)
     phi_ref = np.array([[oracle_lib.phi(P0w[n, q]) for q in range(cfg.nk)] for n in range(cfg.nw)])
     assert abs(got - oracle_lib.phi_gw(cfg.nk, cfg.beta, w, phi_ref)) <= 1e-10 * abs(ref)
+
+
+def test_find_mu_reports_missing_bracket(problems):
+    """A target above the number of spin orbitals can never be bracketed: GW_ENOBRACKET (-6), not an abort and not a wrong mu."""
+    import paper_2206_07660_b200 as gw
+    p = problems("T")
+    cfg = p.cfg
+    H0, S, fg, dfg = _closure(p)
+    with pytest.raises(gw.GWError, match="bracket"):
+        gw.gw_find_mu(dfg["omega"], dfg["t_beta"], torch.from_numpy(S).cuda(), torch.from_numpy(H0).cuda(), None, cfg.spin_deg * cfg.nao + 1.0, -0.1, 0.1, 1e-12, cfg.spin_deg)

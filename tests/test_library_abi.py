@@ -105,3 +105,24 @@ def test_every_documented_shape_is_plannable(gwlib):
                 if L.gw_workspace_bytes(ctypes.byref(c)) == 0:
                     bad.append((nao, naux, ntau, nw))
     assert not bad, bad[:10]
+
+
+def test_traffic_recording_from_ncu_csv(tmp_path, monkeypatch):
+    """bench.py --traffic-from-ncu: per-launch DRAM bytes of the two dominant kernels from an ncu --csv log, keyed by the kernel-source hash,
+    optionally scaled to another config with the same mesh and basis (host logic only)."""
+    import importlib.util
+    import json
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    csv_path = tmp_path / "k.csv"
+    hdr = '"ID","Process ID","Process Name","Host Name","Kernel Name","Context","Stream","Block Size","Grid Size","Device","CC","Section Name","Metric Name","Metric Unit","Metric Value"\n'
+    row = lambda i, k, m, u, v: f'"{i}","1","python","h","{k}","1","7","(512, 1, 1)","(148, 1, 1)","0","10.0","s","{m}","{u}","{v}"\n'
+    csv_path.write_text(hdr + row(0, "void s1::p0_kernel<7, 1>(x)", "dram__bytes_read.sum", "Gbyte", "10") + row(0, "void s1::p0_kernel<7, 1>(x)", "dram__bytes_write.sum", "Gbyte", "2")
+                        + row(1, "void s3w::sigma_ws_kernel<7>(x)", "dram__bytes_read.sum", "byte", "5000000000") + row(1, "void s3w::sigma_ws_kernel<7>(x)", "dram__bytes_write.sum", "byte", "1000000000"))
+    monkeypatch.setattr(bench, "TRAFFIC_JSON", str(tmp_path / "traffic.json"))
+    assert bench.traffic_from_ncu(str(csv_path), "cfgQ", "4") == 0
+    rec = json.load(open(tmp_path / "traffic.json"))
+    assert rec["cfgQ"]["stage1_bytes"] == 12e9 and rec["cfgQ"]["stage3_bytes"] == 6e9
+    assert rec["cfg4"]["stage1_bytes"] == 12e9 * 15 and "scaled_from" in rec["cfg4"]
+    assert bench.traffic_lookup("cfgQ", 0) == 12e9 and bench.traffic_lookup("cfg2", 0) is None
