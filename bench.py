@@ -437,24 +437,25 @@ def run_ours(args):
         n_target = cfg.spin_deg * (cfg.nao // 2)
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(8)]
         st = run.stream
-        ev[0].record(st)
-        Gb = gw.gw_transform(fg["e_beta"].reshape(1, -1), run.G, stream=st)[0].contiguous()
-        gam = gw.gw_axpby(-1.0, Gb, 0.0, torch.empty_like(Gb), st)
-        ev[1].record(st)
-        J = gw.gw_hartree(run.prob, gam, stream=st)
-        ev[2].record(st)
-        Sw = gw.gw_transform(fg["T_wt_f"], run.Sigma, stream=st)
-        ev[3].record(st)
-        F = gw.gw_axpby(1.0, J, 1.0, gw.gw_axpby(1.0, run.K, 1.0, H0.clone(), st), st)
-        ev[4].record(st)
-        # one N_e(mu) evaluation = Eq. 16 for all (n, k) + Eq. 15 (what the chemical-potential search repeats)
-        G_w, _ = gw.gw_dyson_update(fg["omega"], 0.0, S, F, Sw, stream=st)
-        gw.gw_electron_count(fg["t_beta"], S, G_w, cfg.spin_deg, stream=st)
-        ev[5].record(st)
-        G_new = gw.gw_transform(fg["T_tw_f"], G_w, stream=st)
-        ev[6].record(st)
-        gw.gw_axpby(0.7, G_new, 0.3, run.G.clone(), st)
-        ev[7].record(st)
+        for rep in range(2):                 # the first pass is a warm-up (module load of the small kernels), the second is timed
+            ev[0].record(st)
+            Gb = gw.gw_transform(fg["e_beta"].reshape(1, -1), run.G, stream=st)[0].contiguous()
+            gam = gw.gw_axpby(-1.0, Gb, 0.0, torch.empty_like(Gb), st)
+            ev[1].record(st)
+            J = gw.gw_hartree(run.prob, gam, stream=st)
+            ev[2].record(st)
+            Sw = gw.gw_transform(fg["T_wt_f"], run.Sigma, stream=st)
+            ev[3].record(st)
+            F = gw.gw_axpby(1.0, J, 1.0, gw.gw_axpby(1.0, run.K, 1.0, H0.clone(), st), st)
+            ev[4].record(st)
+            # one N_e(mu) evaluation = Eq. 16 for all (n, k) + Eq. 15 (what the chemical-potential search repeats)
+            G_w, _ = gw.gw_dyson_update(fg["omega"], 0.0, S, F, Sw, stream=st)
+            gw.gw_electron_count(fg["t_beta"], S, G_w, cfg.spin_deg, stream=st)
+            ev[5].record(st)
+            G_new = gw.gw_transform(fg["T_tw_f"], G_w, stream=st)
+            ev[6].record(st)
+            gw.gw_axpby(0.7, G_new, 0.3, run.G.clone(), st)
+            ev[7].record(st)
         torch.cuda.synchronize()
         el = lambda a, b: ev[a].elapsed_time(ev[b])
         closure = {"unit": "ms", "gamma_from_G_beta": el(0, 1), "hartree_J": el(1, 2), "sigma_tau_to_iw": el(2, 3), "fock_assembly": el(3, 4),
