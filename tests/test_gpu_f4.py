@@ -122,15 +122,17 @@ def test_qslab_layout_parity(problems, raw_problems, oracle_lib, name, raw):
             gw.gw_hartree(slab, gamma)                      # the shard holds no q = 0: no diagonal blocks
 
 
-@pytest.mark.parametrize("name,ns,budget_q", [("R", 1, 1), ("R", 1, 5), ("S", 1, 1), ("L", 1, 1), ("R", 2, 4), ("1", 1, 3)])
+@pytest.mark.parametrize("name,ns,budget_q", [("R", 1, 1), ("R", 1, 5), ("S", 1, 1), ("L", 1, 1), ("R", 2, 4), ("R", 4, 5), ("1", 1, 3)])
 def test_streamed_iteration_equals_resident(problems, oracle_results, name, ns, budget_q):
     """gw_sigma_iteration_stream (V in host memory, two device slab buffers of budget_q q-points each): Sigma and K are bit-identical
     to the resident evaluation (the q sums continue across slabs in the same order) and match the oracle."""
     import paper_2206_07660_b200 as gw
     p = problems(name) if name != "1" else gwgen.make_problem("1")
-    cfg = dataclasses.replace(p.cfg, spin_deg=1) if ns == 2 else p.cfg
-    if ns == 2:
+    cfg = dataclasses.replace(p.cfg, spin_deg=1) if ns > 1 else p.cfg
+    if ns > 1:
         Gs, gs = gwgen.make_spin_channels(p, 2)
+        if ns == 4:
+            Gs, gs, _ = gwgen.rotate_spin_channels(Gs, gs, seed=2)
     else:
         Gs, gs = p.G, p.gamma
     G, gamma = torch.from_numpy(Gs), torch.from_numpy(gs)
@@ -153,6 +155,21 @@ def test_streamed_iteration_equals_resident(problems, oracle_results, name, ns, 
         assert relerr(out["Sigma"].numpy(), ref["Sigma"]) <= TOL and relerr(out["K"].numpy(), ref["K"]) <= TOL
     with pytest.raises(gw.GWError):
         gw.gw_sigma_iteration_stream(hprob, G.pin_memory(), gamma.pin_memory(), perq)      # budget below two one-q slabs: GW_ENOMEM
+
+
+def test_streamed_iteration_time_reversal_mode(problems, oracle_results):
+    """The streamed iteration under GW_SYM_TR (stage 1 uses the tau half and the Hermitian tiles per slab; the k reduction of stage 3 needs
+    the full q range and is off): against the oracle."""
+    import paper_2206_07660_b200 as gw
+    p = problems("R")
+    cfg = p.cfg
+    hprob = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, p.V.pin_memory(), torch.from_numpy(p.T_wt), torch.from_numpy(p.T_tw),
+                         cfg.spin_deg, symmetry=gw.GW_SYM_TR)
+    perq = 2 * cfg.nk * cfg.naux * cfg.nao * cfg.nao * 16
+    out = gw.gw_sigma_iteration_stream(hprob, torch.from_numpy(p.G).pin_memory(), torch.from_numpy(p.gamma).pin_memory(), 2 * 4 * perq)
+    ref = oracle_results("R")
+    assert out["stats"]["slabs"] == 3
+    assert relerr(out["Sigma"].numpy(), ref["Sigma"]) <= TOL and relerr(out["K"].numpy(), ref["K"]) <= TOL
 
 
 @pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two GPUs")
