@@ -37,6 +37,8 @@ def parse_args():
     ap.add_argument("--no-tr-mode", action="store_true", help="skip the extra GW_SYM_TR measurement")
     ap.add_argument("--no-largest", action="store_true", help="skip the largest_config leg (config 4) of the default run")
     ap.add_argument("--largest-steps", type=int, default=2)
+    ap.add_argument("--v-layout", default="auto", choices=["auto", "full", "qslab"],
+                    help="layout of V on each rank: the whole tensor, or only the rank's q-slab (gw.h GW_V_QSLAB); auto = qslab iff --gpus > 1")
     ap.add_argument("--no-closure", action="store_true", help="skip the loop-closure leg (Sigma -> G' on the headline config)")
     ap.add_argument("--no-out-of-core", action="store_true", help="skip the out-of-core leg (config 4 with V streamed from host memory)")
     ap.add_argument("--v-budget-gb", type=float, default=24.0, help="HBM budget of the two V slab buffers in the out-of-core leg")
@@ -287,14 +289,14 @@ def roofline_of(cfg, nq, stage_ms, executed, peak, peak_note):
 class DeviceRun:
     """One synthetic problem resident in HBM and the buffers of one iteration (a step = the four C-ABI calls)."""
 
-    def __init__(self, gw, cfg, dev, world, rank, symmetry=0):
+    def __init__(self, gw, cfg, dev, world, rank, symmetry=0, v_layout="auto"):
         import torch
         import gwgen
         from paper_2206_07660_b200.dist import shard_range
         self.gw, self.cfg, self.world = gw, cfg, world
         q0, q1 = shard_range(cfg.nk, world, rank)
         self.q0, self.q1, self.nq = q0, q1, q1 - q0
-        if world > 1:
+        if v_layout == "qslab" or (v_layout == "auto" and world > 1):
             # one rank holds only its q-slab of V: the 2 nk blocks per q of its shard serve all four stages (gw.h "V layouts")
             self.p = gwgen.make_problem(cfg, with_V=False)
             self.p.V = gwgen.make_V_qslab(cfg, self.p.mesh, q0, q1, device=dev)
@@ -390,7 +392,7 @@ def run_ours(args):
     cmma = {k: gw.gw_complex_mma_probe(m, 100.0) for m, k in ((0, "4m"), (1, "3m_sums_in_registers"), (2, "3m_presummed_b"))}
 
     # ---- synthetic inputs, resident in HBM (generation is not timed) ----
-    run = DeviceRun(gw, cfg, dev, world, rank)
+    run = DeviceRun(gw, cfg, dev, world, rank, v_layout=args.v_layout)
     nq = run.nq
     executed = gw.gw_executed_flops(run.prob)
     launches = gw.gw_launch_count(run.prob)
@@ -405,7 +407,8 @@ def run_ours(args):
 
     # ---- the same iteration in the documented time-reversal mode (gw.h GW_SYM_TR): reported beside, never as `value` ----
     tr_mode = None
-    if world == 1 and not args.no_tr_mode:
+    full_v = run.prob.v_layout == gw.GW_V_FULL          # the TR and e2e legs build their problems from the whole tensor
+    if world == 1 and not args.no_tr_mode and full_v:
         prob_tr = gw.GWProblem(cfg.mesh, cfg.nao, cfg.naux, cfg.ntau, cfg.nw, cfg.beta, run.p.V, run.T_wt, run.T_tw, cfg.spin_deg,
                                run.q0, run.q1, gw.GW_SYM_TR)
         S_lit = run.Sigma.clone()
@@ -481,7 +484,7 @@ def run_ours(args):
     e2e = None
     h2d = cfg.bytes_V() + (run.G.numel() + run.gamma.numel() + 2 * cfg.nw * cfg.ntau) * 16
     d2h = (run.Sigma.numel() + run.K.numel()) * 16
-    if not args.no_e2e and world == 1:
+    if not args.no_e2e and world == 1 and full_v:
         p = run.p
         hV = torch.empty(p.V.shape, dtype=torch.complex128, pin_memory=True); hV.copy_(p.V)
         hG = torch.from_numpy(p.G).pin_memory(); hg = torch.from_numpy(p.gamma).pin_memory()
