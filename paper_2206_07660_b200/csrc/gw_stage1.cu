@@ -47,6 +47,8 @@ struct Params {
   const c128 *V, *G;
   c128 *P0t, *scratch;
   int cs;                // CTAs per cluster = column splits of the panel
+  int rsplit;            // cs == 2: panel rows transformed by CTA 0 (CTA 1 takes the other TM - rsplit): 16, or fewer when CTA 0 owns one more
+                         // n-tile of the main GEMM than CTA 1, so that main + pass work of the two CTAs balance
   int ncp;               // column passes: an item covers cs*8*ntc columns of its Q panel (ncp > 1 only for naux > 448; Z is
                          // then produced once per pass)
   int nqt, nitems;       // Q tiles per (t,q); total work items
@@ -165,8 +167,9 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
   const size_t vb = (size_t)naux * n2;
   const int nmain = (n2 + KC - 1) / KC;
   const int nkk = d.nk * d.ns;                            // k loop of Eq. 28b with the spin sum inside
-  const int rows_cta = TM / cs;                           // panel rows transformed by this CTA's pass warps
-  const int r0 = (int)rank * rows_cta;
+  // panel rows transformed by this CTA's pass warps
+  const int rows_cta = cs == 2 ? (rank == 0 ? P.rsplit : TM - P.rsplit) : TM / cs;
+  const int r0 = cs == 2 ? (rank == 0 ? 0 : P.rsplit) : (int)rank * rows_cta;
 
   // zero all dynamic smem once (pad rows/columns must hold finite values: they meet zero operands); init barriers
   {
@@ -424,6 +427,7 @@ static int fill_qirr(const GwDims &d, short *qirr) {
 
 struct Plan {
   int main_off;
+  int rsplit;
   int s3m;               // 1: 3M scheme in the main GEMM (16 n-tiles per CTA), 0: 4-real-GEMM scheme (28 n-tiles per CTA)
   int cs, ncp, ksp_max, nqt, nitems, nteff, nqeff, ldp, ksp, ndt, nt, ntc, main_units, pass_units, prows, nstage, pstage, ng, nclusters;
   size_t smem, slab_units, work_bytes;
@@ -445,6 +449,17 @@ static Plan make_plan(const gw_problem *p) {
   pl.ksp_max = pl.ksp <= 7 ? 7 : (pl.ksp <= 13 ? 13 : 16);
   if (pl.ksp > 16) { pl.ok = false; return pl; }
   pl.ndt = (d.nao + 7) / 8;
+  // row split of the pass work in a 2-CTA cluster: when the n-tiles do not split evenly (naux = 200: 13 + 12) CTA 0 carries one more
+  // n-tile of the main GEMM per job, so it transforms fewer panel rows; weights = tensor instructions per n-tile and per panel row and k
+  pl.rsplit = TM / 2;
+  if (pl.cs == 2 && pl.ncp == 1 && pl.nt > pl.ntc) {
+    const int n0 = pl.ntc, n1 = pl.nt - pl.ntc;
+    const double per_tile = 4.0 * ((d.nao * d.nao + 3) / 4) * (pl.s3m ? 3.0 : 4.0);
+    const double per_row = 2.0 * (d.nao / 8.0) * (gwp::pass_mtile_flops(d.nao, pl.ndt, pl.ksp, pl.ksp == pl.ksp_max) / 512.0);
+    int shift = (int)((n0 - n1) * per_tile / (2.0 * per_row) + 0.5);
+    if (shift > TM / 4) shift = TM / 4;
+    pl.rsplit = TM / 2 - shift;
+  }
   int r4 = pl.ksp * 4; if (r4 % 8 == 0) r4 += 4;
   pl.ldp = r4;
   pl.nqt = (d.naux + TM - 1) / TM;
@@ -493,8 +508,9 @@ double gw_stage1_flops(const gw_problem *p) {
     const int tm_rows = (d.naux - qt * s1::TM) < s1::TM ? (d.naux - qt * s1::TM) : s1::TM;
     double mt_pass = 0.0;                       // 8-row m-tiles of the two passes, per CTA of the cluster
     for (int r = 0; r < pl.cs; r++) {
-      const int r0 = r * (s1::TM / pl.cs);
-      int rows = tm_rows < r0 + s1::TM / pl.cs ? tm_rows - r0 : s1::TM / pl.cs;
+      const int rc = pl.cs == 2 ? (r == 0 ? pl.rsplit : s1::TM - pl.rsplit) : s1::TM / pl.cs;
+      const int r0 = pl.cs == 2 ? (r == 0 ? 0 : pl.rsplit) : r * rc;
+      int rows = tm_rows < r0 + rc ? tm_rows - r0 : rc;
       if (rows < 0) rows = 0;
       mt_pass += (rows * d.nao + 7) / 8;
     }
@@ -549,7 +565,7 @@ int gw_launch_stage1(const gw_problem *p, const c128 *G, c128 *P0t, cudaStream_t
   s1::Params P;
   P.d = gw_dims(p); P.V = (const c128 *)p->V; P.G = G; P.P0t = P0t;
   P.scratch = (c128 *)((char *)p->work + 256);
-  P.cs = pl.cs; P.ncp = pl.ncp; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.herm = (P.d.sym & GW_SYM_TR) ? 1 : 0; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
+  P.cs = pl.cs; P.rsplit = pl.rsplit; P.ncp = pl.ncp; P.nqt = pl.nqt; P.nitems = pl.nitems; P.nteff = pl.nteff; P.herm = (P.d.sym & GW_SYM_TR) ? 1 : 0; P.nqeff = s1::fill_qirr(P.d, P.qirr); P.ldp = pl.ldp; P.ksp = pl.ksp; P.ndt = pl.ndt; P.nt = pl.nt; P.ntc = pl.ntc;
   P.main_units = pl.main_units; P.pass_units = pl.pass_units; P.main_off = pl.main_off; P.prows = pl.prows; P.nstage = pl.nstage; P.pstage = pl.pstage; P.ng = pl.ng;
   P.slab_units = pl.slab_units;
   P.fd_nao = gwp::FastDiv((unsigned)P.d.nao);
