@@ -56,6 +56,9 @@ CONFIGS = {
     # odd sizes inside the compile-time k-step classes (nao = 25..28 -> 7 steps, 49..52 -> 13 steps), naux = one panel + 1 row
     "U": GWConfig("cfgU", (1, 2, 1), 27, 33, 6, 6, 20.0, -2.0, 3.0, 0.04, BASE_SEED + 93),
     "W": GWConfig("cfgW", (2, 1, 1), 49, 17, 6, 6, 20.0, -2.0, 3.0, 0.04, BASE_SEED + 92),
+    # nao = 25: ONE valid line in the last 8-wide tile (the FMA tail of the pass GEMMs and the FMA strips of stage 3's final contraction
+    # with a single column / row), naux = one panel + 9 rows, four k points (four one-q slabs in the streamed call)
+    "Y": GWConfig("cfgY", (2, 1, 2), 25, 41, 6, 6, 20.0, -2.0, 3.0, 0.04, BASE_SEED + 89),
     # config-4-shaped problem with a short tau grid (same per-CTA behaviour, 15x less work)
     "Q": GWConfig("cfgQ", (4, 4, 4), 52, 400, 8, 8, 1000.0, -3.0, 5.0, 0.04, BASE_SEED + 95),
     # config-4-shaped basis (nao=52, naux > 224: the wide-panel / split-K kernel variants) at a size the oracle does in full

@@ -518,7 +518,8 @@ __device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao,
 
 // aux warps: Sigma tiles t = w + 4 i (row tile t / NDT, column tile t % NDT):  acc[i] += A[row tile][K] · B[K][column tile] over
 // the ksn k-steps of the job.  For NDT = 4 the warp's tiles share one column tile: one B fragment per k-step feeds four tiles.
-template <int KSP>
+// NMT < NDT (edge mode, NDT = 4): only the row tiles 0 .. NMT-1 of the warp's column tile; the rest is final_edge_fma's.
+template <int KSP, int NMT = Geo<KSP>::NDT>
 __device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[Geo<KSP>::NTA][2], double (&sgi)[Geo<KSP>::NTA][2], int w, int ksn) {
   using Gm = Geo<KSP>;
   constexpr int NDT = Gm::NDT, NTA = Gm::NTA, ldpf = Gm::LDPF, ldt = Gm::LDT;
@@ -529,11 +530,11 @@ __device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[G
 #pragma unroll
     for (int ks = 0; ks < Gm::KSPF; ks++) {
       const c128 b = bp[4 * ks * ldt + 8 * w];
-      c128 a[NDT];
+      c128 a[NMT];
 #pragma unroll
-      for (int mi = 0; mi < NDT; mi++) a[mi] = ap[8 * mi * ldpf + 4 * ks];
+      for (int mi = 0; mi < NMT; mi++) a[mi] = ap[8 * mi * ldpf + 4 * ks];
 #pragma unroll
-      for (int mi = 0; mi < NDT; mi++) cmma(sgr[mi], sgi[mi], a[mi], b);
+      for (int mi = 0; mi < NMT; mi++) cmma(sgr[mi], sgi[mi], a[mi], b);
     }
   } else {
     int aoff[NTA], boff[NTA];
@@ -552,6 +553,49 @@ __device__ __forceinline__ void final_compute(const c128 *stage, double (&sgr)[G
       }
     }
   }
+}
+
+// Edge mode (nao = 25, 26: gwp::pass_tail_fma; NDT = 4, one K piece).  The 26 x 26 Sigma block is a 3 x 3 grid of full 8 x 8 tiles
+// plus a column strip (rows 0..nao-1 x columns 24, 25) and a row strip (rows 24, 25 x columns 0..23).  Seven of the sixteen tiles of
+// the padded 4 x 4 grid hold those strips with two valid lines of eight; in edge mode aux warps 0..2 run the full tiles of their
+// column tile on the tensor cores and aux warp 3 forms both strips with plain FP64 FMAs from the same fragments: lane (g, c) sums
+// its own k = 4 ks + c,
+//   tc[mi][e] += A[8 mi + g][k] B[k][24 + e]        (column strip; the 2 x 2 corner is its mi = 3, g < 2)
+//   tr[nj][e] += A[24 + e][k]   B[k][8 nj + g]      (row strip)
+// and the four lanes of a group add up once per unit (edge_reduce), so that the sum of a unit does not depend on where a V slab ends
+// (GW_ACC_PARTIAL / GW_ACC_CONTINUE stay bit-identical to the resident call).
+template <int KSP>
+__device__ __forceinline__ void final_edge_fma(const c128 *stage, c128 (&tc)[4][2], c128 (&tr)[3][2]) {
+  using Gm = Geo<KSP>;
+  constexpr int NDT = Gm::NDT, ldpf = Gm::LDPF, ldt = Gm::LDT, N0 = 8 * (NDT - 1);
+  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
+  const c128 *ap = stage + g * ldpf + c;
+  const c128 *ae = stage + N0 * ldpf + c;                       // rows 24, 25 of A (the same address in every lane group)
+  const c128 *bp = stage + 8 * NDT * ldpf + c * ldt + g;
+  const c128 *be = stage + 8 * NDT * ldpf + c * ldt + N0;       // columns 24, 25 of B
+#pragma unroll
+  for (int ks = 0; ks < Gm::KSPF; ks++) {
+    const c128 b0 = be[4 * ks * ldt], b1 = be[4 * ks * ldt + 1];
+    const c128 a0 = ae[4 * ks], a1 = ae[ldpf + 4 * ks];
+    c128 a[NDT], b[NDT - 1];
+#pragma unroll
+    for (int mi = 0; mi < NDT; mi++) a[mi] = ap[8 * mi * ldpf + 4 * ks];
+#pragma unroll
+    for (int nj = 0; nj < NDT - 1; nj++) b[nj] = bp[4 * ks * ldt + 8 * nj];
+#pragma unroll
+    for (int mi = 0; mi < NDT; mi++) { cfma(tc[mi][0], a[mi], b0); cfma(tc[mi][1], a[mi], b1); }
+#pragma unroll
+    for (int nj = 0; nj < NDT - 1; nj++) { cfma(tr[nj][0], a0, b[nj]); cfma(tr[nj][1], a1, b[nj]); }
+  }
+}
+// (pr, pi) += sum of t over the four lanes of a group
+__device__ __forceinline__ void edge_reduce(double &pr, double &pi, c128 t) {
+#pragma unroll
+  for (int off = 1; off <= 2; off <<= 1) {
+    t.x += __shfl_xor_sync(0xffffffffu, t.x, off);
+    t.y += __shfl_xor_sync(0xffffffffu, t.y, off);
+  }
+  pr += t.x; pi += t.y;
 }
 
 template <int KSP>
@@ -660,14 +704,22 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
     // ============================================ aux warps ============================================
     gwp::reg_inc<REG_AUX>();
     const int wa = w - NMAINW, g = lane >> 2, c = lane & 3;
+    constexpr int EN0 = 8 * (NDT - 1);
+    const bool edge = NDT == 4 && gwp::pass_tail_fma(nao, NDT);     // nao = 25, 26 (final_edge_fma)
+    const bool ew = edge && wa == NAUXW - 1;                         // this warp forms the two strips
     Ring ra; ra.full = full_a; ra.empty = empty_a; ra.nstage = P.astage; ra.it = 0; ra.ph = 0;
     unsigned un = 0;
     for (int item = blockIdx.x; item < P.nitems; item += gridDim.x) {
       const int t = item % d.ntau, ik = item / d.ntau, k = P.kof(ik % P.nkeff), sg = ik / P.nkeff;
       c128 *Sst = P.Sigma + ((size_t)sg * d.ntau + t) * d.nk * n2;       // Sigma[sg][t]
       double sgr[NTA][2], sgi[NTA][2];
+      // edge mode, aux warp 3: sgr / sgi[mi] hold the column strip (rows 8 mi + g, columns 24, 25: the places they have in the
+      // accumulator of tile (mi, 3) in lane c = 0), pr the row strip (rows 24, 25, column 8 nj + g)
+      c128 pr[3][2];
 #pragma unroll
       for (int i = 0; i < NTA; i++) { sgr[i][0] = sgr[i][1] = 0.0; sgi[i][0] = sgi[i][1] = 0.0; }
+#pragma unroll
+      for (int i = 0; i < 3; i++) pr[i][0] = pr[i][1] = make_double2(0.0, 0.0);
       if (P.acc_mode & GW_ACC_CONTINUE) {                     // continue the q sum from the unscaled partial sums of the previous V slab
         const c128 *in = Sst + (size_t)k * n2;
 #pragma unroll
@@ -676,9 +728,18 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
           if (tile < NDT * NDT) {
             const int mi = tile / NDT, nj = tile - mi * NDT;
             const int i = 8 * mi + g, j0 = 8 * nj + 2 * c;
-            if (i < nao) {
+            if (i < nao && !(edge && !ew && mi == NDT - 1)) {
               if (j0 < nao) { sgr[ti][0] = in[i * nao + j0].x; sgi[ti][0] = in[i * nao + j0].y; }
               if (j0 + 1 < nao) { sgr[ti][1] = in[i * nao + j0 + 1].x; sgi[ti][1] = in[i * nao + j0 + 1].y; }
+            }
+          }
+        }
+        if (ew) {
+#pragma unroll
+          for (int e = 0; e < 2; e++) {
+            if (EN0 + e < nao) {
+#pragma unroll
+              for (int nj = 0; nj < 3; nj++) pr[nj][e] = in[(EN0 + e) * nao + 8 * nj + g];
             }
           }
         }
@@ -694,12 +755,35 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
           }
           __threadfence(); __syncwarp();
           if (lane == 0) { gwp::mbar_arrive(bar_phase); gwp::mbar_arrive(ufree + (un & 1u)); }
+          c128 tc[4][2], tr[3][2];                              // edge mode: the strips' sums over this unit, per k class
+#pragma unroll
+          for (int e = 0; e < 2; e++) {
+#pragma unroll
+            for (int i = 0; i < 4; i++) tc[i][e] = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int i = 0; i < 3; i++) tr[i][e] = make_double2(0.0, 0.0);
+          }
           for (int j = 0; j < tm_rows; j++) {
 #pragma unroll
             for (int h = 0; h < Gm::KH; h++) {
               const int s = ra.wait();
-              final_compute<KSP>(sAux + s * AUXU, sgr, sgi, wa, min(Gm::KSPF, KSP - Gm::KSPF * h));
+              if constexpr (NDT == 4) {
+                if (ew) final_edge_fma<KSP>(sAux + s * AUXU, tc, tr);
+                else if (edge) final_compute<KSP, NDT - 1>(sAux + s * AUXU, sgr, sgi, wa, Gm::KSPF);
+                else final_compute<KSP>(sAux + s * AUXU, sgr, sgi, wa, Gm::KSPF);
+              } else {
+                final_compute<KSP>(sAux + s * AUXU, sgr, sgi, wa, min(Gm::KSPF, KSP - Gm::KSPF * h));
+              }
               ra.release();
+            }
+          }
+          if (ew) {                                             // the strips of this unit: add the four k classes up
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+#pragma unroll
+              for (int i = 0; i < 4; i++) edge_reduce(sgr[i][e], sgi[i][e], tc[i][e]);
+#pragma unroll
+              for (int i = 0; i < 3; i++) edge_reduce(pr[i][e].x, pr[i][e].y, tr[i][e]);
             }
           }
         }
@@ -718,9 +802,18 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
           if (tile < NDT * NDT) {
             const int mi = tile / NDT, nj = tile - mi * NDT;
             const int i = 8 * mi + g, j0 = 8 * nj + 2 * c;
-            if (i < nao) {
+            if (i < nao && !(edge && !ew && mi == NDT - 1)) {
               if (j0 < nao) out[i * nao + j0] = make_double2(pref * sgr[ti][0], prefi * sgi[ti][0]);
               if (j0 + 1 < nao) out[i * nao + j0 + 1] = make_double2(pref * sgr[ti][1], prefi * sgi[ti][1]);
+            }
+          }
+        }
+        if (ew && c == 0) {
+#pragma unroll
+          for (int e = 0; e < 2; e++) {
+            if (EN0 + e < nao) {
+#pragma unroll
+              for (int nj = 0; nj < 3; nj++) out[(EN0 + e) * nao + 8 * nj + g] = make_double2(pref * pr[nj][e].x, prefi * pr[nj][e].y);
             }
           }
         }
@@ -849,7 +942,9 @@ static double flops(const gw_problem *p, const Plan &pl) {
     const double mtiles = (mtc <= 2) ? (double)mtc : (double)((mtc + MT_W - 1) / MT_W) * MT_W;
     fl += mtiles * pl.nnt * (KC / 4) * nmain * 1536.0;                          // main (3M)
     fl += (double)((tm_rows * d.nao + 7) / 8) * gwp::pass_mtile_flops(d.nao, ndt, pl.ksp, true);   // pass A
-    fl += (double)tm_rows * ndt * ndt * pl.ksp * 2048.0;                         // final
+    if (ndt == 4 && gwp::pass_tail_fma(d.nao, ndt))                               // final, edge mode: 3 x 3 DMMA tiles + 56 FMAs per lane and k-step
+      fl += (double)tm_rows * pl.ksp * ((ndt - 1) * (ndt - 1) * 2048.0 + 56.0 * 32.0 * 2.0);
+    else fl += (double)tm_rows * ndt * ndt * pl.ksp * 2048.0;                    // final
   }
   short tmp[128];
   return fl * (double)d.nq * fill_kirr(d, tmp) * d.ntau * d.ns;

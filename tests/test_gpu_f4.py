@@ -122,7 +122,7 @@ def test_qslab_layout_parity(problems, raw_problems, oracle_lib, name, raw):
             gw.gw_hartree(slab, gamma)                      # the shard holds no q = 0: no diagonal blocks
 
 
-@pytest.mark.parametrize("name,ns,budget_q", [("R", 1, 1), ("R", 1, 5), ("S", 1, 1), ("L", 1, 1), ("R", 2, 4), ("R", 4, 5), ("1", 1, 3)])
+@pytest.mark.parametrize("name,ns,budget_q", [("R", 1, 1), ("R", 1, 5), ("S", 1, 1), ("Y", 1, 1), ("S", 2, 3), ("L", 1, 1), ("R", 2, 4), ("R", 4, 5), ("1", 1, 3)])
 def test_streamed_iteration_equals_resident(problems, oracle_results, name, ns, budget_q):
     """gw_sigma_iteration_stream (V in host memory, two device slab buffers of budget_q q-points each): Sigma and K are bit-identical
     to the resident evaluation (the q sums continue across slabs in the same order) and match the oracle."""

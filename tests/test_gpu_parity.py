@@ -22,7 +22,7 @@ def run_gpu(p, **kw):
     return {k: v.cpu().numpy() for k, v in out.items()}
 
 
-@pytest.mark.parametrize("name", ["0", "T", "R", "S", "U", "W", "L", "M", "X"])
+@pytest.mark.parametrize("name", ["0", "T", "R", "S", "Y", "U", "W", "L", "M", "X"])
 def test_full_parity_small(problems, oracle_results, name):
     p = problems(name)
     ref = oracle_results(name)
@@ -138,7 +138,7 @@ def test_sampled_parity_big(oracle_lib, name):
     torch.cuda.empty_cache()
 
 
-@pytest.mark.parametrize("name", ["T", "R", "S", "L"])
+@pytest.mark.parametrize("name", ["T", "R", "S", "Y", "L"])
 def test_raw_input_parity(raw_problems, oracle_lib, name):
     """Literal mode (symmetry = 0) on inputs with NO symmetry: independent V blocks, non-Hermitian G, gamma and W.  A kernel
     that read conj-transposed V[k][k+q] in place of V[k+q][k], or G^+ in place of G, passes every symmetric-input test and
