@@ -52,6 +52,7 @@ enum {
                          naux > 896 (stage 1: panel columns = 2 CTAs x 2 column passes x 224; the paper's N_aux/N_orb = 3-10,
                          PAPER.md:96, gives naux <= 640 at nao = 64) */
   GW_ENOBRACKET = -6, /* gw_find_mu only: N_e(mu) did not bracket the target after 60 widenings of [mu_lo, mu_hi] */
+  GW_ESTATIC = -7,  /* gw_hartree_static only: naux > GW_STATIC_MAX_NAUX, the problem does not fit the library's static scratch */
   GW_ENOTPD = -5    /* gw_sigma_iteration_host only: a Cholesky factorisation of I - P0(q, iOmega_n) met a non-positive pivot
                        (the device calls report that through `info` instead); Sigma / Wt are then not meaningful */
 };
@@ -189,6 +190,21 @@ int gw_sigma_iteration_host(const gw_problem *p, const gw_c128 *G, const gw_c128
  *   gamma : device [nk][nao][nao] in;  J : device [nk][nao][nao] out.  Reads only the diagonal blocks V[k][k]; uses p->work
  *   (any q shard: J does not depend on q_begin / q_end). */
 int gw_hartree(const gw_problem *p, const gw_c128 *gamma, gw_c128 *J, void *stream);
+
+/* The same Hartree term for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): gw_hartree with its one intermediate, rho[Q] = Σ_k' Σ_ab gamma[k'][a][b] V[k'][k'][Q][b][a],
+ * kept in a static device array inside the library instead of p->work.
+ *   Arguments, layouts and result as gw_hartree (bit-identical: same sums, same order); p->work / p->work_bytes are ignored
+ *   and may be NULL / 0.  The call allocates nothing (no cudaMalloc, cudaFree or allocating library routine); its only set-up
+ *   is one symbol-address lookup per device, on the first call with that device current.
+ *   Limit: naux <= GW_STATIC_MAX_NAUX (= gw_static_max_naux()); beyond it the call returns GW_ESTATIC and launches nothing.
+ *   Cost: GW_STATIC_MAX_NAUX * 16 bytes = 8 KB of device memory on every GPU that loads the library, held until exit.
+ *   Sharing: every call on a device uses the same array.  Nothing in it has to start at zero (each entry is written before it
+ *   is read within a call), but calls that overlap on the GPU — different streams without an ordering between them, or two
+ *   host threads on one device — race on it: order them (same stream, or an event). */
+#define GW_STATIC_MAX_NAUX 512
+int gw_hartree_static(const gw_problem *p, const gw_c128 *gamma, gw_c128 *J, void *stream);
+int gw_static_max_naux(void);
 
 /* Dyson equation, Eq. 16, for every (n, k):
  *   G_w[n][k] = [ (i omega[n] + mu) S[k] − F[k] − Sigma_w[n][k] ]^-1        ("matrix inversion in spin-orbital space")

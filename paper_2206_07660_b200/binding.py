@@ -68,7 +68,7 @@ def lib():
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version",
-                  "gw_hartree", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe"):
+                  "gw_hartree", "gw_hartree_static", "gw_static_max_naux", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -352,6 +352,20 @@ def gw_hartree(prob, gamma, J=None, stream=None):
     if J is None:
         J = torch.empty(shape, dtype=torch.complex128, device=gamma.device)
     _check(lib().gw_hartree(prob.ref(), _dev(gamma, prob.kshape(), "gamma"), _dev(J, shape, "J"), _stream(stream)), "gw_hartree")
+    return J
+
+
+def gw_static_max_naux():
+    """Largest naux gw_hartree_static accepts (the size of the library's static device scratch, in complex numbers)."""
+    return int(lib().gw_static_max_naux())
+
+
+def gw_hartree_static(prob, gamma, J, stream=None):
+    """gw_hartree without any device allocation: the intermediate rho[Q] lives in a static device array of the library
+    (naux <= gw_static_max_naux(), else GWError / GW_ESTATIC); prob.work is not used.  J is the caller's output buffer.
+    Calls that overlap on one GPU race on the shared array (include/gw.h)."""
+    shape = (prob.nk, prob.nao, prob.nao)
+    _check(lib().gw_hartree_static(prob.ref(), _dev(gamma, prob.kshape(), "gamma"), _dev(J, shape, "J"), _stream(stream)), "gw_hartree_static")
     return J
 
 

@@ -528,6 +528,7 @@ extern "C" const char *gw_strerror(int code) {
     case GW_EARCH: return "current device is not sm_100 (B200)";
     case GW_ESHAPE: return "size not supported by the kernels (nao > 64, ntau or nw > 200, nw > ntau, naux > 896)";
     case GW_ENOBRACKET: return "chemical-potential search: N_e(mu) does not bracket the target";
+    case GW_ESTATIC: return "problem too large for the static scratch of gw_hartree_static (naux > 512): use gw_hartree with a workspace";
     case GW_ENOTPD: return "I - P0(q, iOmega) is not positive definite (non-positive Cholesky pivot in stage 2)";
     default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown error";
   }
