@@ -391,6 +391,10 @@ def run_ours(args):
     # the three complex tile-product schemes in the bare inner loop (context for the 3M / 4M choice, profiles/r02_3m_vs_4m.md)
     cmma = {k: gw.gw_complex_mma_probe(m, 100.0) for m, k in ((0, "4m"), (1, "3m_sums_in_registers"), (2, "3m_presummed_b"))}
 
+    # which warps share an FP64 pipe (profiles/r02_fp64_subcores.md): one warp on each of the four SM sub-partitions, four warps on one
+    # sub-partition, two warps on each, the eight warps of two sub-partitions
+    subcores = {k: gw.gw_fp64_subcore_probe(m) for m, k in ((0x000F, "warps_0-3"), (0x1111, "warps_0_4_8_12"), (0x00FF, "warps_0-7"), (0x5555, "even_warps"))}
+
     # ---- synthetic inputs, resident in HBM (generation is not timed) ----
     run = DeviceRun(gw, cfg, dev, world, rank, v_layout=args.v_layout)
     nq = run.nq
@@ -404,6 +408,39 @@ def run_ours(args):
         total_ms, stage_ms = float(tt[0]), [float(x) for x in tt[1:]]
     ms_per_step = total_ms / args.steps
     Sig_dev_check = run.Sigma.cpu()      # result of the literal device-resident run (the e2e leg must reproduce it bit for bit)
+
+    # ---- stage 2 taken apart (north_star: "achieved HBM GB/s for the memory-bound transforms"): the tau -> i Omega transform kernel timed alone
+    #      through gw_transform on the P buffer of the last step (same kernel, same shape as inside gw_screened_interaction: nw x ntau times
+    #      [ntau][nq naux^2], in place), its algorithmic bytes (one read of the ntau slices, one write of the nw slices) against the measured HBM
+    #      copy bandwidth and its flops against the FP64 peak; the Dyson solves take the rest of the stage ----
+    stage2 = None
+    if world == 1:
+        n_t = 5
+        gw.gw_transform(run.T_wt, run.P, run.P[:cfg.nw], stream=run.stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(run.stream)
+        for _ in range(n_t):
+            gw.gw_transform(run.T_wt, run.P, run.P[:cfg.nw], stream=run.stream)
+        e1.record(run.stream)
+        torch.cuda.synchronize()
+        t_ms = e0.elapsed_time(e1) / n_t
+        ln = nq * cfg.naux * cfg.naux
+        t_bytes = 16.0 * ln * (cfg.ntau + cfg.nw)
+        t_flops = 8.0 * ln * cfg.ntau * cfg.nw
+        hbm = None
+        try:
+            hbm = float(json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "MEASURED_PEAKS.json")))["hbm_gbs"])
+        except Exception:
+            pass
+        hbm_note = "MEASURED_PEAKS.json hbm_gbs" if hbm else "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+        hbm = hbm or 6552.0
+        gbs, tfl = t_bytes / (t_ms * 1e-3) * 1e-9, t_flops / (t_ms * 1e-3) * 1e-12
+        stage2 = {"transform_ms": t_ms, "transform_calls_per_step": 2, "dyson_ms": stage_ms[1] - 2.0 * t_ms,
+                  "transform": {"algorithmic_gb": t_bytes * 1e-9, "achieved_gbs": gbs, "hbm_peak_gbs": hbm, "frac_hbm": gbs / hbm, "hbm_peak_source": hbm_note,
+                                "algorithmic_tflop": t_flops * 1e-12, "achieved_tflops": tfl, "frac_fp64": tfl / peak,
+                                "bound": "tensor" if tfl / peak > gbs / hbm else "hbm",
+                                "note": "8 ntau nw / (16 (ntau + nw)) flop per byte: %.1f at this grid against a ridge of %.1f" %
+                                        (t_flops / t_bytes, peak * 1e3 / hbm)}}
 
     # ---- the same iteration in the documented time-reversal mode (gw.h GW_SYM_TR): reported beside, never as `value` ----
     tr_mode = None
@@ -585,10 +622,12 @@ def run_ours(args):
            "frac_of_fp64_peak_nominal": total_nom / (ms_per_step * 1e-3) * 1e-12 / peak / world,
            "fp64_peak_tflops_measured": peak, "fp64_peak_dmma": peak_dmma, "fp64_peak_dfma": peak_dfma,
            "complex_mma_inner_loop_algorithmic_tflops": cmma,
+           "fp64_subcore_probe_tflops": subcores,
            "stage_ms": {"polarization": stage_ms[0], "screened_interaction": stage_ms[1], "selfenergy": stage_ms[2],
                         "exchange": stage_ms[3], "allreduce": stage_ms[4]},
            "roofline": roof, "gpu_launches": launches * args.steps,
            "clocks": clocks, "info": [-1, -1], "kernel_revision": kernel_revision()}
+    out["stage2"] = stage2
     out["loop_closure"] = closure
     out["time_reversal_mode"] = tr_mode
     out["largest_config"] = largest

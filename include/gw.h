@@ -269,6 +269,12 @@ int gw_fp64_peak_dfma(double ms, double *tflops, void *stream);
  * *tflops = ALGORITHMIC TFLOP/s, 8 flops per complex multiply-add. */
 int gw_complex_mma_probe(int32_t mode, double ms, double *tflops, void *stream);
 
+/* Diagnostic: which warps share an FP64 tensor pipe.  One CTA of 16 warps per SM; only the warps whose bit is set in warp_mask run a
+ * register-resident DMMA.8x8x4 loop (12 independent accumulators), the others exit.  *tflops = executed TFLOP/s over the chip.
+ * On B200 every SM sub-partition (warp id mod 4) has its own pipe: mask 0x000F (one warp on each) reaches the chip's peak, mask
+ * 0x1111 (four warps on one sub-partition) a quarter of it (profiles/r02_fp64_subcores.md).  warp_mask != 0, bits 0..15. */
+int gw_fp64_subcore_probe(uint32_t warp_mask, double *tflops, void *stream);
+
 const char *gw_strerror(int code);
 int gw_version(void);
 

@@ -7,12 +7,12 @@ There is no CPU fallback: if the shared library is missing or the device is not 
 import ctypes
 import os
 
-from .binding import (GWProblem, GWError, GW_SYM_TR, GW_V_FULL, GW_V_QSLAB, gw_sigma_iteration_stream, gw_phi_gw, gw_complex_mma_probe, lib, lib_path, gw_polarization, gw_screened_interaction, gw_screened_interaction_phi, gw_transform,
+from .binding import (GWProblem, GWError, GW_SYM_TR, GW_V_FULL, GW_V_QSLAB, gw_sigma_iteration_stream, gw_phi_gw, gw_complex_mma_probe, gw_fp64_subcore_probe, lib, lib_path, gw_polarization, gw_screened_interaction, gw_screened_interaction_phi, gw_transform,
                       gw_selfenergy, gw_exchange, gw_workspace_bytes, gw_sigma_iteration, gw_sigma_iteration_host,
                       gw_executed_flops, gw_launch_count, gw_fp64_peak, gw_fp64_peak_dfma, gw_strerror, gw_version,
                       gw_hartree, gw_hartree_static, gw_static_max_naux, gw_dyson_update, gw_electron_count, gw_find_mu, gw_axpby, gw_scgw_iteration)
 
-__all__ = ["GWProblem", "GWError", "GW_SYM_TR", "GW_V_FULL", "GW_V_QSLAB", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe", "lib", "lib_path", "gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy",
+__all__ = ["GWProblem", "GWError", "GW_SYM_TR", "GW_V_FULL", "GW_V_QSLAB", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe", "gw_fp64_subcore_probe", "lib", "lib_path", "gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy",
            "gw_exchange", "gw_workspace_bytes", "gw_sigma_iteration", "gw_sigma_iteration_host", "gw_executed_flops",
            "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_strerror", "gw_version",
            "gw_hartree", "gw_hartree_static", "gw_static_max_naux", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_scgw_iteration"]

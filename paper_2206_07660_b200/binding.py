@@ -68,7 +68,7 @@ def lib():
         L.gw_strerror.restype = ctypes.c_char_p
         for n in ("gw_polarization", "gw_screened_interaction", "gw_screened_interaction_phi", "gw_transform", "gw_selfenergy", "gw_exchange",
                   "gw_sigma_iteration_host", "gw_executed_flops", "gw_launch_count", "gw_fp64_peak", "gw_fp64_peak_dfma", "gw_version",
-                  "gw_hartree", "gw_hartree_static", "gw_static_max_naux", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe"):
+                  "gw_hartree", "gw_hartree_static", "gw_static_max_naux", "gw_dyson_update", "gw_electron_count", "gw_find_mu", "gw_axpby", "gw_sigma_iteration_stream", "gw_phi_gw", "gw_complex_mma_probe", "gw_fp64_subcore_probe"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -322,6 +322,13 @@ def gw_complex_mma_probe(mode, ms=100.0, stream=None):
     """Algorithmic TFLOP/s of the main-GEMM inner loop alone: mode 0 = 4M, 1 = 3M with sums in registers, 2 = 3M with pre-summed B."""
     out = ctypes.c_double(0.0)
     _check(lib().gw_complex_mma_probe(int(mode), ctypes.c_double(ms), ctypes.byref(out), _stream(stream)), "gw_complex_mma_probe")
+    return out.value
+
+
+def gw_fp64_subcore_probe(warp_mask, stream=None):
+    """Executed TFLOP/s of a DMMA loop run by the warps of warp_mask only (one 16-warp CTA per SM): which warps share an FP64 pipe."""
+    out = ctypes.c_double(0.0)
+    _check(lib().gw_fp64_subcore_probe(ctypes.c_uint32(int(warp_mask)), ctypes.byref(out), _stream(stream)), "gw_fp64_subcore_probe")
     return out.value
 
 

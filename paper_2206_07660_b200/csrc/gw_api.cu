@@ -375,6 +375,48 @@ done:
   return rc;
 }
 
+// ---- which warps share an FP64 pipe: the DMMA loop on the warps of warp_mask only (one 16-warp CTA per SM) ----
+__global__ void __launch_bounds__(512, 1) fp64_subcore_kernel(unsigned mask, int iters, double *out) {
+  const int w = threadIdx.x >> 5;
+  if (!((mask >> w) & 1u)) return;
+  double acc[12][2];
+#pragma unroll
+  for (int i = 0; i < 12; i++) { acc[i][0] = threadIdx.x * 1e-3 + i; acc[i][1] = i; }
+  const double a = 1e-3 + threadIdx.x * 1e-9, b = 1e-3;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 12; i++) dmma884(acc[i][0], acc[i][1], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 12; i++) s += acc[i][0] + acc[i][1];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int gw_fp64_subcore_probe(uint32_t warp_mask, double *tflops, void *stream) {
+  if (!tflops || !warp_mask || (warp_mask >> 16)) return GW_EINVAL;
+  int rc = check_arch(); if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nsm = gw_sm_count();
+  double *out = 0; cudaEvent_t e0 = 0, e1 = 0; float t = 0;
+  const int iters = 50000;
+  int nw = 0;
+  for (int i = 0; i < 16; i++) nw += (warp_mask >> i) & 1u;
+  const double fl = 512.0 * 12 * (double)iters * nw * nsm;       // 512 flops per DMMA.8x8x4
+  CU(cudaMalloc(&out, sizeof(double) * nsm * 512));
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  fp64_subcore_kernel<<<nsm, 512, 0, st>>>(warp_mask, 1000, out);   // warm-up
+  CU(cudaEventRecord(e0, st));
+  fp64_subcore_kernel<<<nsm, 512, 0, st>>>(warp_mask, iters, out);
+  CU(cudaEventRecord(e1, st));
+  CU(cudaEventSynchronize(e1));
+  CU(cudaEventElapsedTime(&t, e0, e1));
+  *tflops = fl / (t * 1e-3) * 1e-12;
+done:
+  cudaFree(out); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1);
+  return rc;
+}
+
 // ---- the same probe with plain DFMA (no tensor-core instruction): 16 independent chains per thread ----
 __global__ void __launch_bounds__(256) fp64_dfma_kernel(double *out, int iters) {
   double acc[16];
