@@ -14,6 +14,7 @@
 namespace s2 {
 
 constexpr int NTHR = 256;
+constexpr int NTHR_D = 512;   // Dyson kernel: 16 warps (four per SM sub-partition) hide the latency of its global-memory updates
 constexpr int NC = 64;   // columns per transform block
 
 // ---------------- Eq. 28a / Eq. 30:  Y[o][m] = Σ_i T[o][i] X[i][m],  m over `len` ----------------
@@ -84,6 +85,7 @@ __global__ void __launch_bounds__(NTHR, 1) transform_kernel(int n_out, int n_in,
 struct DysonParams {
   int n, nb, batch, nq, q0;
   int ldpan, ldn;          // smem strides: panel [row][ldpan]; block rows [k][ldn]
+  int prow;                // rows of the panel buffer: every row an 8-row tile of an update can touch
   c128 *PW;                // batch matrices, n*n each (index = freq*nq + ql); overwritten by the solution
   c128 *slabs;             // per-CTA copy for A / L
   int32_t *info;
@@ -98,7 +100,7 @@ template <bool AK_MAJOR, bool B_NMAJOR_CONJ, bool LOWER>
 __device__ __forceinline__ void update_tiles(c128 *Cg, int ldc, int M, int N, const c128 *sA, int lda, const c128 *sB, int ldb, int ksteps) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
   const int mtiles = (M + 7) / 8, ngroups = (N + 31) / 32;    // a work unit = one m-tile x four n-tiles
-  for (int unit = w; unit < mtiles * ngroups; unit += NTHR / 32) {
+  for (int unit = w; unit < mtiles * ngroups; unit += NTHR_D / 32) {
     const int mt = unit / ngroups, ng = unit - mt * ngroups;
     const int r0 = 8 * mt, c0 = 32 * ng;
     if (LOWER && c0 > r0 + 7) continue;
@@ -106,6 +108,16 @@ __device__ __forceinline__ void update_tiles(c128 *Cg, int ldc, int M, int N, co
 #pragma unroll
     for (int j = 0; j < 4; j++) { cr[j][0] = cr[j][1] = 0.0; ci[j][0] = ci[j][1] = 0.0; }
     const int r = r0 + g;
+    // the C elements of this unit are loaded before the K loop, so that the global-memory latency runs under the DMMAs
+    c128 cv[4][2];
+#pragma unroll
+    for (int j = 0; j < 4; j++)
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        const int col = c0 + 8 * j + 2 * c + e;
+        const bool on = r < M && c0 + 8 * j < N && !(LOWER && c0 + 8 * j > r0 + 7) && col < N;
+        cv[j][e] = on ? Cg[(size_t)r * ldc + col] : make_double2(0.0, 0.0);
+      }
     for (int ks = 0; ks < ksteps; ks++) {
       const int k = 4 * ks + c;
       c128 a;
@@ -127,12 +139,7 @@ __device__ __forceinline__ void update_tiles(c128 *Cg, int ldc, int M, int N, co
 #pragma unroll
           for (int e = 0; e < 2; e++) {
             const int col = c0 + 8 * j + 2 * c + e;
-            if (col < N) {
-              c128 *p = Cg + (size_t)r * ldc + col;
-              c128 v = *p;
-              v.x -= cr[j][e]; v.y -= ci[j][e];
-              *p = v;
-            }
+            if (col < N) Cg[(size_t)r * ldc + col] = make_double2(cv[j][e].x - cr[j][e], cv[j][e].y - ci[j][e]);
           }
         }
       }
@@ -140,18 +147,18 @@ __device__ __forceinline__ void update_tiles(c128 *Cg, int ldc, int M, int N, co
   }
 }
 
-__global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
+__global__ void __launch_bounds__(NTHR_D, 1) dyson_kernel(const DysonParams P) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   c128 *smem = reinterpret_cast<c128 *>(smem_raw);
   const int n = P.n, nb = P.nb, ldpan = P.ldpan, ldn = P.ldn;
   const int npad = (n + 7) / 8 * 8;
   c128 *sPan = smem;                          // [npad][ldpan]  (also reused as [nb][ldn] block row of L in the back solve)
   const int kst4 = 4 * ((nb + 3) / 4);
-  const int pan_units = (npad + 8) * ldpan > kst4 * ldn ? (npad + 8) * ldpan : kst4 * ldn;
+  const int pan_units = P.prow * ldpan > kst4 * ldn ? P.prow * ldpan : kst4 * ldn;
   c128 *sBlk = smem + pan_units;              // [nb][ldn]
   __shared__ int s_bad;
   __shared__ double s_piv;
-  __shared__ double s_red[NTHR];
+  double *s_red = reinterpret_cast<double *>(smem);    // the panel buffer is free when the reduction runs (>= NTHR_D doubles)
   c128 *A = P.slabs + (size_t)blockIdx.x * n * n;
   const int kst = (nb + 3) / 4;
 
@@ -159,7 +166,7 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
     c128 *Pm = P.PW + (size_t)mi * n * n;
     if (threadIdx.x == 0) s_bad = 0;
     double trp = 0.0;                                  // this thread's share of Re tr P0w (fixed order: deterministic)
-    for (int e = threadIdx.x; e < n * n; e += NTHR) {
+    for (int e = threadIdx.x; e < n * n; e += NTHR_D) {
       const int i = e / n, j = e - i * n;
       const c128 v = Pm[e];
       if (i == j) trp += v.x;
@@ -169,7 +176,7 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
     // ---------- blocked right-looking Cholesky of A (lower) ----------
     for (int j0 = 0; j0 < n; j0 += nb) {
       const int jb = min(nb, n - j0), m = n - j0;
-      for (int e = threadIdx.x; e < (npad + 8) * 4 * kst; e += NTHR) { // panel rows r < m, cols < 4*kst (zero padded)
+      for (int e = threadIdx.x; e < P.prow * 4 * kst; e += NTHR_D) { // panel rows r < m, cols < 4*kst (zero padded)
         const int r = e / (4 * kst), cc = e - r * (4 * kst);
         sPan[r * ldpan + cc] = (r < m && cc < jb) ? A[(size_t)(j0 + r) * n + j0 + cc] : make_double2(0.0, 0.0);
       }
@@ -183,10 +190,10 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
         }
         __syncthreads();
         const double inv = 1.0 / s_piv;
-        for (int i = cc + 1 + threadIdx.x; i < jb; i += NTHR) { c128 v = sPan[i * ldpan + cc]; sPan[i * ldpan + cc] = make_double2(v.x * inv, v.y * inv); }
+        for (int i = cc + 1 + threadIdx.x; i < jb; i += NTHR_D) { c128 v = sPan[i * ldpan + cc]; sPan[i * ldpan + cc] = make_double2(v.x * inv, v.y * inv); }
         __syncthreads();
         const int rem = jb - cc - 1;
-        for (int e = threadIdx.x; e < rem * rem; e += NTHR) {
+        for (int e = threadIdx.x; e < rem * rem; e += NTHR_D) {
           const int i = cc + 1 + e / rem, c2 = cc + 1 + e % rem;
           if (c2 <= i) {
             const c128 li = sPan[i * ldpan + cc], lc = sPan[c2 * ldpan + cc];
@@ -198,7 +205,7 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
         __syncthreads();
       }
       // panel rows below the block: L_i = A_i L_jj^{-H}  (one thread per row)
-      for (int i = jb + threadIdx.x; i < m; i += NTHR) {
+      for (int i = jb + threadIdx.x; i < m; i += NTHR_D) {
         c128 *row = sPan + i * ldpan;
         for (int cc = 0; cc < jb; cc++) {
           c128 s = row[cc];
@@ -209,7 +216,7 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
         }
       }
       __syncthreads();
-      for (int e = threadIdx.x; e < m * jb; e += NTHR) {              // write the factored panel back (lower part)
+      for (int e = threadIdx.x; e < m * jb; e += NTHR_D) {              // write the factored panel back (lower part)
         const int r = e / jb, cc = e - r * jb;
         A[(size_t)(j0 + r) * n + j0 + cc] = (r >= cc) ? sPan[r * ldpan + cc] : make_double2(0.0, 0.0);
       }
@@ -221,28 +228,29 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
     if (P.phi) {
       // Eq. 37 summand: tr ln[I - P0w] + tr P0w = 2 Σ_i ln L_ii + tr P0w  (tree reduction in a fixed order)
       double v = trp;
-      for (int i = threadIdx.x; i < n; i += NTHR) v += 2.0 * log(A[(size_t)i * n + i].x);
+      for (int i = threadIdx.x; i < n; i += NTHR_D) v += 2.0 * log(A[(size_t)i * n + i].x);
       s_red[threadIdx.x] = v;
       __syncthreads();
-      for (int h = NTHR / 2; h > 0; h >>= 1) {
+      for (int h = NTHR_D / 2; h > 0; h >>= 1) {
         if (threadIdx.x < h) s_red[threadIdx.x] += s_red[threadIdx.x + h];
         __syncthreads();
       }
       if (threadIdx.x == 0) P.phi[mi] = s_red[0];
+      __syncthreads();                                  // s_red lives in the panel buffer, which the forward solve fills next
     }
     // ---------- forward solve L Y = P (in place on Pm) ----------
     for (int j0 = 0; j0 < n; j0 += nb) {
       const int jb = min(nb, n - j0), m = n - j0;
-      for (int e = threadIdx.x; e < (npad + 8) * 4 * kst; e += NTHR) {
+      for (int e = threadIdx.x; e < P.prow * 4 * kst; e += NTHR_D) {
         const int r = e / (4 * kst), cc = e - r * (4 * kst);
         sPan[r * ldpan + cc] = (r < m && cc < jb) ? A[(size_t)(j0 + r) * n + j0 + cc] : make_double2(0.0, 0.0);
       }
-      for (int e = threadIdx.x; e < 4 * kst * npad; e += NTHR) {
+      for (int e = threadIdx.x; e < 4 * kst * npad; e += NTHR_D) {
         const int r = e / npad, col = e - r * npad;
         sBlk[r * ldn + col] = (r < jb && col < n) ? Pm[(size_t)(j0 + r) * n + col] : make_double2(0.0, 0.0);
       }
       __syncthreads();
-      for (int col = threadIdx.x; col < n; col += NTHR) {
+      for (int col = threadIdx.x; col < n; col += NTHR_D) {
         for (int r = 0; r < jb; r++) {
           c128 s = sBlk[r * ldn + col];
           const c128 *lr = sPan + r * ldpan;
@@ -263,13 +271,13 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
     for (int bj = nblk - 1; bj >= 0; bj--) {
       const int j0 = bj * nb, jb = min(nb, n - j0);
       c128 *sRow = sPan;    // block row of L: sRow[k][i] = L[j0+k][i], i < j0 + jb
-      for (int e = threadIdx.x; e < 4 * kst * npad; e += NTHR) {
+      for (int e = threadIdx.x; e < 4 * kst * npad; e += NTHR_D) {
         const int r = e / npad, col = e - r * npad;
         sRow[r * ldn + col] = (r < jb && col < j0 + jb) ? A[(size_t)(j0 + r) * n + col] : make_double2(0.0, 0.0);
         sBlk[r * ldn + col] = (r < jb && col < n) ? Pm[(size_t)(j0 + r) * n + col] : make_double2(0.0, 0.0);
       }
       __syncthreads();
-      for (int col = threadIdx.x; col < n; col += NTHR) {
+      for (int col = threadIdx.x; col < n; col += NTHR_D) {
         for (int r = jb - 1; r >= 0; r--) {
           c128 s = sBlk[r * ldn + col];
           for (int k = r + 1; k < jb; k++) { const c128 l = sRow[k * ldn + j0 + r], x = sBlk[k * ldn + col]; s.x -= l.x * x.x + l.y * x.y; s.y -= l.x * x.y - l.y * x.x; }
@@ -293,7 +301,7 @@ __global__ void __launch_bounds__(NTHR, 1) dyson_kernel(const DysonParams P) {
 
 __global__ void set_info_kernel2(int32_t *info) { info[0] = -1; info[1] = -1; }
 
-struct Plan { int nb, ldpan, ldn, grid_d, grid_t, nblocks; size_t smem_d, smem_t, work_bytes; bool ok; };
+struct Plan { int nb, ldpan, ldn, prow, grid_d, grid_t, nblocks; size_t smem_d, smem_t, work_bytes; bool ok; };
 
 static Plan make_plan(const gw_problem *p) {
   Plan pl; memset(&pl, 0, sizeof(pl));
@@ -304,10 +312,12 @@ static Plan make_plan(const gw_problem *p) {
   for (int nb = 32; nb >= 4; nb /= 2) {
     const int kst4 = (nb + 3) / 4 * 4;
     const int ldpan = kst4 + 4;
-    size_t pan = (size_t)(npad + 8) * ldpan; const size_t alt = (size_t)kst4 * pl.ldn;
+    int prow = n > nb ? nb + (n - nb + 7) / 8 * 8 : npad;
+    if (prow < npad) prow = npad;
+    size_t pan = (size_t)prow * ldpan; const size_t alt = (size_t)kst4 * pl.ldn;
     if (alt > pan) pan = alt;
     const size_t bytes = (pan + (size_t)kst4 * pl.ldn) * sizeof(c128);
-    if (bytes <= 220 * 1024) { pl.nb = nb; pl.ldpan = ldpan; pl.smem_d = bytes; pl.ok = true; break; }
+    if (bytes <= 226 * 1024 && bytes >= NTHR_D * sizeof(double)) { pl.nb = nb; pl.ldpan = ldpan; pl.prow = prow; pl.smem_d = bytes; pl.ok = true; break; }
   }
   const int nsm = gwp::gw_num_sms();
   const int batch = d.nw * d.nq;
@@ -342,9 +352,9 @@ int gw_launch_stage2(const gw_problem *p, const c128 *P0t, c128 *Wt, int32_t *in
   if (info) s2::set_info_kernel2<<<1, 1, 0, st>>>(info);
   s2::transform_kernel<<<pl.grid_t, s2::NTHR, pl.smem_t, st>>>(d.nw, d.ntau, (const c128 *)p->T_wt, P0t, Wt, len, pl.nblocks);
   s2::DysonParams D;
-  D.n = d.naux; D.nb = pl.nb; D.batch = d.nw * d.nq; D.nq = d.nq; D.q0 = d.q0; D.ldpan = pl.ldpan; D.ldn = pl.ldn;
+  D.n = d.naux; D.nb = pl.nb; D.batch = d.nw * d.nq; D.nq = d.nq; D.q0 = d.q0; D.ldpan = pl.ldpan; D.ldn = pl.ldn; D.prow = pl.prow;
   D.PW = Wt; D.slabs = (c128 *)((char *)p->work + 256); D.info = info; D.phi = phi;
-  s2::dyson_kernel<<<pl.grid_d, s2::NTHR, pl.smem_d, st>>>(D);
+  s2::dyson_kernel<<<pl.grid_d, s2::NTHR_D, pl.smem_d, st>>>(D);
   s2::transform_kernel<<<pl.grid_t, s2::NTHR, pl.smem_t, st>>>(d.ntau, d.nw, (const c128 *)p->T_tw, Wt, Wt, len, pl.nblocks);
   return (int)cudaGetLastError();
 }
