@@ -267,7 +267,11 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
   } else if (w >= NMAINW) {
     // ========================================= pass warps =========================================
     if constexpr (REG_PASS > 65536 / NTHR1) gwp::reg_inc<REG_PASS>(); else gwp::reg_dec<REG_PASS>();
-    const int wp = w - NMAINW;
+    // m-tile slot of this warp in a pass job.  Pass warp 8 + s runs on SM sub-partition s (each has its own FP64 pipe,
+    // profiles/r02_fp64_subcores.md); sub-partition 0 also carries the main-ring producer and, in CTA 0 of a cluster with an odd n-tile
+    // count, a main warp with one more n-tile.  When a CTA's rows do not fill the last pass job, the last slots are the empty ones: the
+    // warp of sub-partition 0 takes the last slot (measured on config P: stage 1 272.0 -> 266.6 ms).
+    const int wp = (w - NMAINW + NPASSW - 1) & (NPASSW - 1);
     constexpr int PMT = KSP_MAX <= 8 ? 2 : 1;          // m-tiles per pass warp on the exact path (prows = 32*PMT there)
     Ring rp; rp.full = full_p; rp.empty = empty_p; rp.nstage = P.pstage; rp.it = 0; rp.ph = 0;
     unsigned kit = 0, ph = 0;
@@ -325,12 +329,15 @@ __global__ void __launch_bounds__(NTHR1, 1) p0_kernel(const Params P, const __gr
       const int ncols = max(0, min(naux - col0, 8 * P.ntc));
       const int ntc_mine = (ncols + 7) / 8;
       const int mtc = (it.tm_rows + 7) / 8;
-      // tile ownership.  Full panels: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile.  Ragged last panel
+      // tile ownership.  Full panels: warp w owns m-tiles 2*mh, 2*mh+1 (mh = w >> 2) and every 4th n-tile, starting at column group
+      // noff.  Group 0 is the one with an extra n-tile when the count is not a multiple of four; it goes to warps 1 and 6, i.e. to SM
+      // sub-partitions 1 and 2, which carry no producer warp (sub-partition 0: the TMA issuer, 3: the cp.async producer).  Measured on
+      // config Q: stage 1 4 221 -> 4 186 ms against group 0 on sub-partitions 0 and 1; level on config P.  Ragged last panel
       // (<= 16 rows): all eight warps share m-tiles 0 (and 1), every 8th n-tile each, so the panel costs time in proportion
       // to its rows instead of a full panel's.
       const bool narrow = mtc <= 2;
       const int mh = narrow ? 0 : (w >> 2);
-      const int noff = narrow ? w : (((w & 3) - mh + 4) & 3);
+      const int noff = narrow ? w : (((w & 3) - mh + 3) & 3);
       const int nstride = narrow ? 8 : 4;
       const int mtw = (narrow && mtc == 1) ? 1 : MT_W;
       // Hermitian mode: columns right of the panel's diagonal block come from the mirror writes of the later panels
