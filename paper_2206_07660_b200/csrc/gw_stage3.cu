@@ -404,7 +404,7 @@ namespace s3w {
 
 using gwp::FastDiv;
 constexpr int NMAINW = 8, NAUXW = 4, NTHR = 512;
-constexpr int T_APROD = 480, N_APROD = 32;
+// aux-ring producer threads: the last NAP threads of the CTA (Geo<KSP>::NAP)
 constexpr int KC = 8, MT_W = 2, NJ = 4, TM = 32;
 constexpr int AROWS = 32;                     // pass A: rows per job (one m-tile per aux warp)
 constexpr int NST_MAX = 8, AST_MAX = 4;
@@ -414,6 +414,9 @@ constexpr int REG_MAIN = 152, REG_AUX = 168, REG_PROD = 40;   // 256*152 + 128*1
 template <int KSP> struct Geo {
   static constexpr int NDT = (KSP + 1) / 2;                       // 8-wide tiles over nao
   static constexpr int NTA = (NDT * NDT + NAUXW - 1) / NAUXW;     // Sigma tiles per aux warp
+  // aux-ring producer threads: warp 15, or warps 13-15 for the wide basis class (1 664-2 080 cp.async per aux job there).  Measured on
+  // config Q, stage 3: 4 440 ms with 32 threads, 4 358 with 64, 4 346 with 96; at nao = 26 more producer threads cost (config P 296 -> 301 ms with 64)
+  static constexpr int NAP = KSP <= 8 ? 32 : 96;
   static constexpr int KH = KSP <= 8 ? 1 : 3;                     // K pieces of one Q's final contraction (shared-memory budget)
   static constexpr int KSPF = (KSP + KH - 1) / KH;                // k-steps per piece (the last piece may have fewer)
   static constexpr int LDP = (4 * KSP) % 8 == 0 ? 4 * KSP + 4 : 4 * KSP;       // ≡ 4 (mod 8): conflict-free K-contiguous fragments
@@ -475,7 +478,9 @@ __device__ __forceinline__ void main_compute(const c128 *sAw, const c128 *sBw, d
 }
 
 // aux ring jobs (producer warp 15)
+template <int NAP>
 __device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row0, int rows_total, int nao, int ldp, FastDiv fd) {
+  constexpr int T_APROD = NTHR - NAP, N_APROD = NAP;
   const int nrow = min(AROWS, rows_total - row0);
   const int total = nrow * nao;
   const c128 *s = src + (size_t)row0 * nao;
@@ -486,8 +491,9 @@ __device__ __forceinline__ void issue_rows(c128 *stage, const c128 *src, int row
 }
 // final job for the K range [a0, a0 + 4 ksn) of one Q: A = V1[Q][i][a0..] -> stage[i][ldpf]; B = T[Q][a0..][j] -> [a - a0][ldt];
 // K beyond nao is zero filled
-template <int NDT>
+template <int NDT, int NAP>
 __device__ __forceinline__ void issue_final(c128 *stage, const c128 *Aq, const c128 *Bq, int nao, int ldpf, int ldt, int a0, int ksn, FastDiv fd) {
+  constexpr int T_APROD = NTHR - NAP, N_APROD = NAP;
   const int lane = threadIdx.x - T_APROD, kw = 4 * ksn;
   if (a0 == 0 && kw >= nao) {                            // whole rows (one piece per Q)
     for (int i = lane; i < nao * nao; i += N_APROD) {
@@ -509,7 +515,9 @@ __device__ __forceinline__ void issue_final(c128 *stage, const c128 *Aq, const c
     gwp::cp_async16_zfill(sB + r * ldt + (i - r * nao), ok ? Bq + (size_t)a0 * nao + i : Bq, ok);
   }
 }
+template <int NAP>
 __device__ __forceinline__ void issue_matrix(c128 *sG, const c128 *src, int nao, int ldp, FastDiv fd) {
+  constexpr int T_APROD = NTHR - NAP, N_APROD = NAP;
   for (int i = threadIdx.x - T_APROD; i < nao * nao; i += N_APROD) {
     const int r = (int)fd.div((unsigned)i), cc = i - r * nao;
     cp_async16(sG + r * ldp + cc, src + i);
@@ -601,7 +609,7 @@ __device__ __forceinline__ void edge_reduce(double &pr, double &pi, c128 t) {
 template <int KSP>
 __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmV) {
   using Gm = Geo<KSP>;
-  constexpr int NDT = Gm::NDT, NTA = Gm::NTA, ldp = Gm::LDP, ldpf = Gm::LDPF, ldt = Gm::LDT, AUXU = Gm::AUX_UNITS;
+  constexpr int NDT = Gm::NDT, NTA = Gm::NTA, ldp = Gm::LDP, ldpf = Gm::LDPF, ldt = Gm::LDT, AUXU = Gm::AUX_UNITS, N_APROD = Gm::NAP;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   // the TMA destinations (128-byte swizzle) need 1024-byte alignment: the launch asks for 1 KB of slack
   c128 *smem = reinterpret_cast<c128 *>(smem_raw + ((1024u - (gwp::smem_u32(smem_raw) & 1023u)) & 1023u));
@@ -633,7 +641,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
 
   if (w >= NMAINW + NAUXW) {
     gwp::reg_dec<REG_PROD>();
-    if (w < 15) {
+    if (w < 16 - N_APROD / 32) {
       // ---- main-ring producer: the 32 lanes of warp 12 issue the TMA box loads of a job in one go (lane 0 arms the stage's
       //      mbarrier with the byte count, lanes < ntc load one 8 x 8 box of V2 each, lane 31 loads the W panel K slice) ----
       if (w == NMAINW + NAUXW) {
@@ -676,12 +684,12 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
             const int Q0 = qt * TM, tm_rows = min(TM, naux - Q0), rows = tm_rows * nao, npass = (rows + AROWS - 1) / AROWS;
             const c128 *U = slabU + (size_t)(un & 1u) * P.slab_units;
             // sG is free: pass A of the previous unit completed before its final jobs were issued
-            if (qt == 0) issue_matrix(sG, Gs + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
+            if (qt == 0) issue_matrix<N_APROD>(sG, Gs + ((size_t)t * d.nk + kp) * n2, nao, ldp, P.fd_nao);
             gwp::cp_async_arrive_noinc(bar_g);
             gwp::mbar_wait(uready + (un & 1u), (un >> 1) & 1u);
             for (int j = 0; j < npass; j++) {
               const int s = ra.acquire();
-              issue_rows(sAux + s * AUXU, U, j * AROWS, rows, nao, ldp, P.fd_nao);
+              issue_rows<N_APROD>(sAux + s * AUXU, U, j * AROWS, rows, nao, ldp, P.fd_nao);
               ra.commit();
             }
             gwp::mbar_wait(bar_phase, un & 1u);                     // T of this unit is in slabT
@@ -690,7 +698,7 @@ __global__ void __launch_bounds__(NTHR, 1) sigma_ws_kernel(const Params P, const
 #pragma unroll
               for (int h = 0; h < Gm::KH; h++) {
                 const int s = ra.acquire();
-                issue_final<NDT>(sAux + s * AUXU, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldpf, ldt, 4 * Gm::KSPF * h,
+                issue_final<NDT, N_APROD>(sAux + s * AUXU, V1t + (size_t)j * n2, slabT + (size_t)j * n2, nao, ldpf, ldt, 4 * Gm::KSPF * h,
                                  min(Gm::KSPF, KSP - Gm::KSPF * h), P.fd_nao);
                 ra.commit();
               }
